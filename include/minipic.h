@@ -1,0 +1,191 @@
+/*
+ * minipic.h - C ABI of the MiniPIC hot path for NVIDIA B200 (sm_100a).
+ *
+ * Paged attention over a position-encoding-free KV cache (arxiv/paper_2606_13126, "MiniPIC";
+ * citations below are PAPER.md:<line>):
+ *
+ *   - keys are stored UNROTATED in fixed-size physical blocks shared across requests
+ *     (PAPER.md:14, :47, :100, :105);
+ *   - RoPE is applied to every K tile inside the attention kernel at the request's per-token
+ *     logical position pi(j); Q is rotated at its own logical position
+ *     (Eq. 2:  score(t,j) = (R_t q_t)^T (R_pi(j) k~_j) / sqrt(d));
+ *   - scores are masked by the block-level causal structure the span primitives induce
+ *     (PAPER.md:57, :90, :123-128, :143): query row t sees sequence index j iff
+ *     q_vis_lo[t] <= j <= q_seq_idx[t]  (span token: vis_lo = first index of its span;
+ *     system / suffix token: vis_lo = 0).
+ *
+ * Conventions (every entry point):
+ *   * All array arguments are DEVICE pointers owned by the caller unless the name ends in
+ *     `_host` (see the *_host entry points at the end).  The library allocates nothing on the
+ *     device path, keeps no state between calls and never synchronises the stream.
+ *   * `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
+ *   * The return value is a minipic_status.  Argument errors are detected on the host before
+ *     any launch.  Out-of-range block ids / slots / positions are undefined behaviour.
+ *   * Layouts (row-major, innermost last):
+ *       k_cache, v_cache : [num_blocks, num_kv_heads, block_size, head_dim]   (library-defined;
+ *                          one (block, head) is one contiguous 16*head_dim*sizeof chunk)
+ *       k_new, v_new, q, out : [tokens, heads, head_dim]
+ *       lse              : float32 [tokens, num_q_heads], natural log of the sum of exp of the
+ *                          SCALED scores over the visible keys
+ *       block_tables     : int32 [num_reqs, max_blocks_per_req]; sequence index j of request r
+ *                          lives in block block_tables[r][j / block_size], row j % block_size
+ *       kv_positions     : int32 [sum kv_lens]; kv_positions[cu_kv_lens[r] + j] = pi_r(j) >= 0
+ *   * Causality is by SEQUENCE INDEX, RoPE by LOGICAL POSITION ("position exists only
+ *     as per-request metadata consumed inside attention").
+ *   * The same physical block id may appear in many block tables and several times in one
+ *     (PAPER.md:145, :232): attention only reads the caches.
+ *   * A query row with no visible key returns out = 0, lse = -inf.
+ *   * Supported: block_size 16; head_dim 64 or 128; num_q_heads % num_kv_heads == 0;
+ *     dtype bf16 or f32 (q, k, v, caches and out share it).  Anything else returns
+ *     MINIPIC_ERR_UNSUPPORTED.  There is no CPU fallback.
+ */
+#ifndef MINIPIC_H_
+#define MINIPIC_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  MINIPIC_OK = 0,
+  MINIPIC_ERR_INVALID_ARG = 1,
+  MINIPIC_ERR_UNSUPPORTED = 2,
+  MINIPIC_ERR_WORKSPACE_TOO_SMALL = 3,
+  MINIPIC_ERR_CUDA = 4
+} minipic_status;
+
+typedef enum { MINIPIC_BF16 = 0, MINIPIC_F32 = 1 } minipic_dtype;
+
+enum {
+  MINIPIC_Q_PREROTATED = 1u, /* caller already applied R(pos) to Q (the paper's own flow) */
+  MINIPIC_K_PREROTATED = 2u, /* CONTROL ONLY: the cache holds rotated K, kernels skip the K RoPE step   */
+  MINIPIC_FORCE_SIMT   = 4u  /* DEBUG: run the generic fp32 CUDA-core attention kernels instead of the  */
+                             /* tensor-core ones (bf16, head_dim 128 normally take the latter)          */
+};
+
+typedef struct {
+  int32_t num_q_heads;   /* Hq                                                     */
+  int32_t num_kv_heads;  /* Hkv, divides Hq (GQA group G = Hq / Hkv)               */
+  int32_t head_dim;      /* D: 64 or 128                                           */
+  int32_t block_size;    /* 16                                      */
+  int32_t num_blocks;    /* physical pool size                                     */
+  int32_t dtype;         /* minipic_dtype of q, k, v, caches, out                  */
+  double  rope_theta;    /* RoPE base; f_i = theta^(-2i/D), rotate-half pairing    */
+  float   softmax_scale; /* 0 => 1/sqrt(head_dim) (Eq. 2)                          */
+  uint32_t flags;        /* MINIPIC_* bits                                         */
+  /* Optional cos/sin table ("a cos/sin table lookup"): device float2
+   * [rope_table_len][head_dim/2] = (cos, sin)(p * f_i), built by minipic_rope_table_build for this
+   * (rope_theta, head_dim).  Positions >= rope_table_len (or a NULL table) are computed inside the
+   * kernels from a 64-bit fixed-point phase, to the same accuracy (~2e-7). */
+  const void* rope_table;
+  int32_t rope_table_len;
+  int32_t reserved;
+} minipic_config;
+
+/* ---- a0: RoPE table (optional accelerator; not needed for correctness) ------------------------
+ * Fills table[p][i] = (cos(p f_i), sin(p f_i)), p in [0, num_positions), i in [0, head_dim/2),
+ * evaluated in fp64 on the device and rounded once to fp32.  Bytes = num_positions*head_dim/2*8. */
+size_t minipic_rope_table_bytes(const minipic_config* cfg, int32_t num_positions);
+int minipic_rope_table_build(const minipic_config* cfg, int32_t num_positions, void* table, void* cuda_stream);
+
+/* ---- a1: paged cache write ("V vectors are unchanged" :113) -----------------
+ * cache[slot / B, h, slot % B, :] = new[t, h, :] for every token t with slot_mapping[t] >= 0.
+ * Raw byte copy: no rotation, no conversion - bit exact.  slot < 0 => the token is skipped.
+ * Duplicate slots in one call are a caller error (undefined winner).  The caller orders this before
+ * attention on the same stream. */
+int minipic_cache_write(const minipic_config* cfg,
+                        const void* k_new, const void* v_new,   /* [num_tokens, Hkv, D]            */
+                        const int64_t* slot_mapping,            /* [num_tokens], block*B + offset  */
+                        int32_t num_tokens,
+                        void* k_cache, void* v_cache, void* cuda_stream);
+
+/* ---- a2-a9: prefill attention (PAPER.md:100-113, Eq. 2; mask :57, :90, :123-128, :143) ---------
+ * For every query row t of request r (rows cu_q_lens[r] .. cu_q_lens[r+1]) and head h:
+ *   q' = R(pi_r(q_seq_idx[t])) q[t,h]      (skipped under MINIPIC_Q_PREROTATED)
+ *   k_j = R(pi_r(j)) k~_j  gathered through block_tables[r]   (skipped under MINIPIC_K_PREROTATED)
+ *   out[t,h] = softmax_j(q'.k_j * scale) V_j over q_vis_lo[t] <= j <= q_seq_idx[t];  lse[t,h].
+ * Requires q_seq_idx[t] < kv_lens[r].  workspace: device scratch of at least
+ * minipic_prefill_workspace_bytes(...) bytes, 256-byte aligned; contents are overwritten. */
+size_t minipic_prefill_workspace_bytes(const minipic_config* cfg, int32_t num_reqs, int32_t num_q_tokens);
+int minipic_prefill_attention(const minipic_config* cfg,
+                              const void* q,                    /* [Tq, Hq, D]                       */
+                              const void* k_cache, const void* v_cache,
+                              const int32_t* block_tables, int32_t max_blocks_per_req,
+                              const int32_t* cu_q_lens,         /* [R+1]                             */
+                              const int32_t* kv_lens,           /* [R]                               */
+                              const int32_t* cu_kv_lens,        /* [R+1] offsets into kv_positions   */
+                              const int32_t* kv_positions,      /* [sum kv_lens]                     */
+                              const int32_t* q_seq_idx,         /* [Tq] sequence index of the query  */
+                              const int32_t* q_vis_lo,          /* [Tq] lowest visible sequence idx  */
+                              int32_t num_reqs, int32_t num_q_tokens, int32_t max_kv_len,
+                              void* out, float* lse,            /* [Tq,Hq,D], [Tq,Hq]                */
+                              void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---- a10-a11: decode attention = split-KV partial kernel + LSE-merge kernel ------
+ * One query per sequence, sitting at sequence index kv_lens[r]-1 (its K/V must already be in the
+ * cache).  q_vis_lo may be NULL (=> 0).  Partials (o_s normalised over its split, lse_s) go to the
+ * workspace and are merged by  lse = ln sum_s e^{lse_s},  o = sum_s e^{lse_s - lse} o_s. */
+size_t minipic_decode_workspace_bytes(const minipic_config* cfg, int32_t num_seqs, int32_t max_kv_len);
+int minipic_decode_attention(const minipic_config* cfg,
+                             const void* q,                     /* [R, Hq, D]                        */
+                             const void* k_cache, const void* v_cache,
+                             const int32_t* block_tables, int32_t max_blocks_per_req,
+                             const int32_t* kv_lens, const int32_t* cu_kv_lens, const int32_t* kv_positions,
+                             const int32_t* q_vis_lo,           /* [R] or NULL                       */
+                             int32_t num_seqs, int32_t max_kv_len,
+                             void* out, float* lse, void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* ---- end-to-end entry points with HOST buffers ---------------------------------------------------
+ * Same computation as cache_write followed by prefill / decode attention, but every per-step input
+ * (new K/V rows, slot mapping, Q, index tables) is read from HOST memory and the result (out, lse)
+ * is written to HOST memory; the resident KV cache stays on the device.  `arena` is caller-owned
+ * DEVICE scratch of at least minipic_*_host_arena_bytes(...) bytes (256-byte aligned) that receives
+ * the staged inputs, the workspace and the device-side result.  All copies and kernels are enqueued
+ * on `cuda_stream` (cudaMemcpyAsync: pin the host buffers for true asynchrony); the call does not
+ * synchronise - outputs are valid once the stream has drained.  num_new_tokens may be 0. */
+size_t minipic_prefill_host_arena_bytes(const minipic_config* cfg, int32_t num_reqs, int32_t num_q_tokens,
+                                        int32_t num_new_tokens, int32_t max_blocks_per_req, int32_t total_kv_len);
+int minipic_prefill_step_host(const minipic_config* cfg,
+                              const void* k_new_host, const void* v_new_host, const int64_t* slot_mapping_host,
+                              int32_t num_new_tokens,
+                              const void* q_host,
+                              void* k_cache, void* v_cache,     /* DEVICE */
+                              const int32_t* block_tables_host, int32_t max_blocks_per_req,
+                              const int32_t* cu_q_lens_host, const int32_t* kv_lens_host,
+                              const int32_t* cu_kv_lens_host, const int32_t* kv_positions_host,
+                              const int32_t* q_seq_idx_host, const int32_t* q_vis_lo_host,
+                              int32_t num_reqs, int32_t num_q_tokens, int32_t max_kv_len,
+                              void* out_host, float* lse_host,
+                              void* arena, size_t arena_bytes, void* cuda_stream);
+
+size_t minipic_decode_host_arena_bytes(const minipic_config* cfg, int32_t num_seqs, int32_t num_new_tokens,
+                                       int32_t max_blocks_per_req, int32_t total_kv_len, int32_t max_kv_len);
+int minipic_decode_step_host(const minipic_config* cfg,
+                             const void* k_new_host, const void* v_new_host, const int64_t* slot_mapping_host,
+                             int32_t num_new_tokens,
+                             const void* q_host,
+                             void* k_cache, void* v_cache,      /* DEVICE */
+                             const int32_t* block_tables_host, int32_t max_blocks_per_req,
+                             const int32_t* kv_lens_host, const int32_t* cu_kv_lens_host,
+                             const int32_t* kv_positions_host, const int32_t* q_vis_lo_host /* or NULL */,
+                             int32_t num_seqs, int32_t max_kv_len,
+                             void* out_host, float* lse_host,
+                             void* arena, size_t arena_bytes, void* cuda_stream);
+
+/* ---- misc ---------------------------------------------------------------------------------------*/
+const char* minipic_status_string(int status);
+/* Text of the last CUDA error seen by this thread inside the library ("" if none). */
+const char* minipic_last_cuda_error(void);
+/* Number of kernels the library has launched in this process since load (for bench accounting). */
+uint64_t minipic_launch_count(void);
+/* Name of the attention kernel variant the last prefill / decode call on this thread dispatched to
+ * ("prefill_sm100_tcgen05", "prefill_simt", "decode_mma", "decode_simt", ...). */
+const char* minipic_last_variant(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MINIPIC_H_ */

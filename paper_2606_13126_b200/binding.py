@@ -1,0 +1,212 @@
+"""Thin ctypes binding over libminipic.so - argument marshalling only.
+
+Every function here has the name of the C entry point it forwards to (include/minipic.h); every
+step of the hot path runs inside the library's CUDA kernels.  PyTorch appears only as the owner of
+device memory and streams (``tensor.data_ptr()``, ``torch.cuda.current_stream()``).
+
+There is no fallback: ``lib()`` raises if the shared library has not been built
+(``python -m paper_2606_13126_b200.build``), and nothing here imports ``oracle/``.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libminipic.so")
+
+MINIPIC_OK = 0
+MINIPIC_ERR_INVALID_ARG = 1
+MINIPIC_ERR_UNSUPPORTED = 2
+MINIPIC_ERR_WORKSPACE_TOO_SMALL = 3
+MINIPIC_ERR_CUDA = 4
+MINIPIC_BF16, MINIPIC_F32 = 0, 1
+MINIPIC_Q_PREROTATED, MINIPIC_K_PREROTATED, MINIPIC_FORCE_SIMT = 1, 2, 4
+
+# every symbol include/minipic.h declares (tests check the library exports all of them)
+EXPORTS = [
+    "minipic_rope_table_bytes", "minipic_rope_table_build", "minipic_cache_write",
+    "minipic_prefill_workspace_bytes", "minipic_prefill_attention",
+    "minipic_decode_workspace_bytes", "minipic_decode_attention",
+    "minipic_prefill_host_arena_bytes", "minipic_prefill_step_host",
+    "minipic_decode_host_arena_bytes", "minipic_decode_step_host",
+    "minipic_status_string", "minipic_last_cuda_error", "minipic_launch_count", "minipic_last_variant",
+]
+
+
+class minipic_config(C.Structure):
+    _fields_ = [("num_q_heads", C.c_int32), ("num_kv_heads", C.c_int32), ("head_dim", C.c_int32),
+                ("block_size", C.c_int32), ("num_blocks", C.c_int32), ("dtype", C.c_int32),
+                ("rope_theta", C.c_double), ("softmax_scale", C.c_float), ("flags", C.c_uint32),
+                ("rope_table", C.c_void_p), ("rope_table_len", C.c_int32), ("reserved", C.c_int32)]
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load libminipic.so (once).  Fails loudly if it is missing - there is no CPU path."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise RuntimeError(f"{LIB_PATH} not built: run `python -m paper_2606_13126_b200.build` "
+                           "(the MiniPIC hot path has no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    P, I32, SZ, VP = C.POINTER(minipic_config), C.c_int32, C.c_size_t, C.c_void_p
+    L.minipic_rope_table_bytes.restype = SZ
+    L.minipic_rope_table_bytes.argtypes = [P, I32]
+    L.minipic_rope_table_build.restype = C.c_int
+    L.minipic_rope_table_build.argtypes = [P, I32, VP, VP]
+    L.minipic_cache_write.restype = C.c_int
+    L.minipic_cache_write.argtypes = [P, VP, VP, VP, I32, VP, VP, VP]
+    L.minipic_prefill_workspace_bytes.restype = SZ
+    L.minipic_prefill_workspace_bytes.argtypes = [P, I32, I32]
+    L.minipic_prefill_attention.restype = C.c_int
+    L.minipic_prefill_attention.argtypes = [P, VP, VP, VP, VP, I32, VP, VP, VP, VP, VP, VP, I32, I32, I32, VP, VP, VP, SZ, VP]
+    L.minipic_decode_workspace_bytes.restype = SZ
+    L.minipic_decode_workspace_bytes.argtypes = [P, I32, I32]
+    L.minipic_decode_attention.restype = C.c_int
+    L.minipic_decode_attention.argtypes = [P, VP, VP, VP, VP, I32, VP, VP, VP, VP, I32, I32, VP, VP, VP, SZ, VP]
+    L.minipic_prefill_host_arena_bytes.restype = SZ
+    L.minipic_prefill_host_arena_bytes.argtypes = [P, I32, I32, I32, I32, I32]
+    L.minipic_prefill_step_host.restype = C.c_int
+    L.minipic_prefill_step_host.argtypes = [P, VP, VP, VP, I32, VP, VP, VP, VP, I32, VP, VP, VP, VP, VP, VP,
+                                            I32, I32, I32, VP, VP, VP, SZ, VP]
+    L.minipic_decode_host_arena_bytes.restype = SZ
+    L.minipic_decode_host_arena_bytes.argtypes = [P, I32, I32, I32, I32, I32]
+    L.minipic_decode_step_host.restype = C.c_int
+    L.minipic_decode_step_host.argtypes = [P, VP, VP, VP, I32, VP, VP, VP, VP, I32, VP, VP, VP, VP, I32, I32,
+                                           VP, VP, VP, SZ, VP]
+    L.minipic_status_string.restype = C.c_char_p
+    L.minipic_status_string.argtypes = [C.c_int]
+    L.minipic_last_cuda_error.restype = C.c_char_p
+    L.minipic_launch_count.restype = C.c_uint64
+    L.minipic_last_variant.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+class MinipicError(RuntimeError):
+    def __init__(self, status: int):
+        L = lib()
+        self.status = status
+        msg = L.minipic_status_string(status).decode()
+        if status == MINIPIC_ERR_CUDA:
+            msg += ": " + L.minipic_last_cuda_error().decode()
+        super().__init__(msg)
+
+
+def _check(status: int) -> None:
+    if status != MINIPIC_OK:
+        raise MinipicError(status)
+
+
+def _ptr(x) -> Optional[int]:
+    """Address of a torch tensor / numpy array / raw int; None -> NULL."""
+    if x is None:
+        return None
+    if isinstance(x, int):
+        return x
+    if hasattr(x, "data_ptr"):
+        return x.data_ptr()
+    return x.ctypes.data  # numpy (host entry points)
+
+
+def _stream(stream) -> Optional[int]:
+    if stream is None:
+        import torch
+        return torch.cuda.current_stream().cuda_stream
+    return stream if isinstance(stream, int) else stream.cuda_stream
+
+
+def make_config(*, num_q_heads, num_kv_heads, head_dim, num_blocks, dtype, rope_theta, block_size=16,
+                softmax_scale=0.0, flags=0, rope_table=None, rope_table_len=0) -> minipic_config:
+    return minipic_config(num_q_heads, num_kv_heads, head_dim, block_size, num_blocks,
+                          MINIPIC_BF16 if dtype in ("bf16", MINIPIC_BF16) else MINIPIC_F32,
+                          float(rope_theta), float(softmax_scale), int(flags), _ptr(rope_table), int(rope_table_len), 0)
+
+
+# ----------------------------------------------------------------------------- forwarding calls
+def minipic_rope_table_bytes(cfg, num_positions: int) -> int:
+    return lib().minipic_rope_table_bytes(C.byref(cfg), num_positions)
+
+
+def minipic_rope_table_build(cfg, num_positions: int, table, stream=None) -> None:
+    _check(lib().minipic_rope_table_build(C.byref(cfg), num_positions, _ptr(table), _stream(stream)))
+
+
+def minipic_cache_write(cfg, k_new, v_new, slot_mapping, num_tokens, k_cache, v_cache, stream=None) -> None:
+    _check(lib().minipic_cache_write(C.byref(cfg), _ptr(k_new), _ptr(v_new), _ptr(slot_mapping), num_tokens,
+                                     _ptr(k_cache), _ptr(v_cache), _stream(stream)))
+
+
+def minipic_prefill_workspace_bytes(cfg, num_reqs: int, num_q_tokens: int) -> int:
+    return lib().minipic_prefill_workspace_bytes(C.byref(cfg), num_reqs, num_q_tokens)
+
+
+def minipic_prefill_attention(cfg, q, k_cache, v_cache, block_tables, max_blocks_per_req, cu_q_lens, kv_lens,
+                              cu_kv_lens, kv_positions, q_seq_idx, q_vis_lo, num_reqs, num_q_tokens, max_kv_len,
+                              out, lse, workspace, workspace_bytes, stream=None) -> None:
+    _check(lib().minipic_prefill_attention(
+        C.byref(cfg), _ptr(q), _ptr(k_cache), _ptr(v_cache), _ptr(block_tables), max_blocks_per_req, _ptr(cu_q_lens),
+        _ptr(kv_lens), _ptr(cu_kv_lens), _ptr(kv_positions), _ptr(q_seq_idx), _ptr(q_vis_lo), num_reqs, num_q_tokens,
+        max_kv_len, _ptr(out), _ptr(lse), _ptr(workspace), workspace_bytes, _stream(stream)))
+
+
+def minipic_decode_workspace_bytes(cfg, num_seqs: int, max_kv_len: int) -> int:
+    return lib().minipic_decode_workspace_bytes(C.byref(cfg), num_seqs, max_kv_len)
+
+
+def minipic_decode_attention(cfg, q, k_cache, v_cache, block_tables, max_blocks_per_req, kv_lens, cu_kv_lens,
+                             kv_positions, q_vis_lo, num_seqs, max_kv_len, out, lse, workspace, workspace_bytes,
+                             stream=None) -> None:
+    _check(lib().minipic_decode_attention(
+        C.byref(cfg), _ptr(q), _ptr(k_cache), _ptr(v_cache), _ptr(block_tables), max_blocks_per_req, _ptr(kv_lens),
+        _ptr(cu_kv_lens), _ptr(kv_positions), _ptr(q_vis_lo), num_seqs, max_kv_len, _ptr(out), _ptr(lse),
+        _ptr(workspace), workspace_bytes, _stream(stream)))
+
+
+def minipic_prefill_host_arena_bytes(cfg, num_reqs, num_q_tokens, num_new_tokens, max_blocks_per_req, total_kv_len) -> int:
+    return lib().minipic_prefill_host_arena_bytes(C.byref(cfg), num_reqs, num_q_tokens, num_new_tokens,
+                                                  max_blocks_per_req, total_kv_len)
+
+
+def minipic_prefill_step_host(cfg, k_new_host, v_new_host, slot_mapping_host, num_new_tokens, q_host, k_cache, v_cache,
+                              block_tables_host, max_blocks_per_req, cu_q_lens_host, kv_lens_host, cu_kv_lens_host,
+                              kv_positions_host, q_seq_idx_host, q_vis_lo_host, num_reqs, num_q_tokens, max_kv_len,
+                              out_host, lse_host, arena, arena_bytes, stream=None) -> None:
+    _check(lib().minipic_prefill_step_host(
+        C.byref(cfg), _ptr(k_new_host), _ptr(v_new_host), _ptr(slot_mapping_host), num_new_tokens, _ptr(q_host),
+        _ptr(k_cache), _ptr(v_cache), _ptr(block_tables_host), max_blocks_per_req, _ptr(cu_q_lens_host),
+        _ptr(kv_lens_host), _ptr(cu_kv_lens_host), _ptr(kv_positions_host), _ptr(q_seq_idx_host), _ptr(q_vis_lo_host),
+        num_reqs, num_q_tokens, max_kv_len, _ptr(out_host), _ptr(lse_host), _ptr(arena), arena_bytes, _stream(stream)))
+
+
+def minipic_decode_host_arena_bytes(cfg, num_seqs, num_new_tokens, max_blocks_per_req, total_kv_len, max_kv_len) -> int:
+    return lib().minipic_decode_host_arena_bytes(C.byref(cfg), num_seqs, num_new_tokens, max_blocks_per_req,
+                                                 total_kv_len, max_kv_len)
+
+
+def minipic_decode_step_host(cfg, k_new_host, v_new_host, slot_mapping_host, num_new_tokens, q_host, k_cache, v_cache,
+                             block_tables_host, max_blocks_per_req, kv_lens_host, cu_kv_lens_host, kv_positions_host,
+                             q_vis_lo_host, num_seqs, max_kv_len, out_host, lse_host, arena, arena_bytes,
+                             stream=None) -> None:
+    _check(lib().minipic_decode_step_host(
+        C.byref(cfg), _ptr(k_new_host), _ptr(v_new_host), _ptr(slot_mapping_host), num_new_tokens, _ptr(q_host),
+        _ptr(k_cache), _ptr(v_cache), _ptr(block_tables_host), max_blocks_per_req, _ptr(kv_lens_host),
+        _ptr(cu_kv_lens_host), _ptr(kv_positions_host), _ptr(q_vis_lo_host), num_seqs, max_kv_len, _ptr(out_host),
+        _ptr(lse_host), _ptr(arena), arena_bytes, _stream(stream)))
+
+
+def minipic_status_string(status: int) -> str:
+    return lib().minipic_status_string(status).decode()
+
+
+def minipic_launch_count() -> int:
+    return int(lib().minipic_launch_count())
+
+
+def minipic_last_variant() -> str:
+    return lib().minipic_last_variant().decode()

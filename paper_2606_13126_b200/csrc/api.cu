@@ -1,0 +1,372 @@
+// extern "C" boundary of libminipic.so: argument validation, dispatch, host-buffer entry points.
+// See include/minipic.h for the contract of every call.
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+
+#include "internal.h"
+
+namespace minipic {
+
+static std::atomic<uint64_t> g_launches{0};
+static thread_local char g_cuda_err[256] = "";
+static thread_local const char* g_variant = "";
+
+void note_launch(int n) { g_launches.fetch_add((uint64_t)n, std::memory_order_relaxed); }
+bool check_launch(const char* what) {
+  cudaError_t e = cudaGetLastError();
+  if (e == cudaSuccess) return true;
+  snprintf(g_cuda_err, sizeof(g_cuda_err), "%s: %s", what, cudaGetErrorString(e));
+  return false;
+}
+
+static int validate_cfg(const minipic_config* cfg) {
+  if (!cfg) return MINIPIC_ERR_INVALID_ARG;
+  if (cfg->num_q_heads <= 0 || cfg->num_kv_heads <= 0 || cfg->num_blocks <= 0) return MINIPIC_ERR_INVALID_ARG;
+  if (cfg->num_q_heads % cfg->num_kv_heads) return MINIPIC_ERR_INVALID_ARG;
+  if (!(cfg->rope_theta > 0.0)) return MINIPIC_ERR_INVALID_ARG;
+  if (cfg->rope_table_len < 0 || (cfg->rope_table_len > 0 && !cfg->rope_table)) return MINIPIC_ERR_INVALID_ARG;
+  if (cfg->block_size != kBlock) return MINIPIC_ERR_UNSUPPORTED;
+  if (cfg->head_dim != 64 && cfg->head_dim != 128) return MINIPIC_ERR_UNSUPPORTED;
+  if (cfg->dtype != MINIPIC_BF16 && cfg->dtype != MINIPIC_F32) return MINIPIC_ERR_UNSUPPORTED;
+  return MINIPIC_OK;
+}
+
+static void make_rope(const minipic_config* cfg, RopeParams* rp) {
+  const int half = cfg->head_dim / 2;
+  const long double two_pi = 6.283185307179586476925286766559L;
+  for (int i = 0; i < 64; ++i) rp->phase_inc[i] = 0;
+  for (int i = 0; i < half; ++i) {
+    // f_i = theta^(-2i/D) (reading A2); F_i = f_i / 2pi in 0.64 fixed point
+    const long double f = powl((long double)cfg->rope_theta, -2.0L * (long double)i / (long double)cfg->head_dim);
+    const long double turns = f / two_pi;  // in (0, 0.16]
+    rp->phase_inc[i] = (unsigned long long)ldexpl(turns, 64);
+  }
+  rp->table = (const float2*)cfg->rope_table;
+  rp->table_len = cfg->rope_table ? cfg->rope_table_len : 0;
+  rp->half = half;
+}
+
+static void make_ctx(const minipic_config* cfg, void* stream, Ctx* c) {
+  c->hq = cfg->num_q_heads; c->hkv = cfg->num_kv_heads; c->d = cfg->head_dim; c->group = c->hq / c->hkv;
+  c->num_blocks = cfg->num_blocks; c->dtype = cfg->dtype; c->flags = cfg->flags;
+  c->scale = cfg->softmax_scale > 0.f ? cfg->softmax_scale : (float)(1.0 / std::sqrt((double)cfg->head_dim));
+  c->scale_log2 = (float)((double)c->scale * 1.4426950408889634);
+  make_rope(cfg, &c->rope);
+  c->stream = (cudaStream_t)stream;
+}
+
+static inline size_t align_up(size_t x, size_t a = 256) { return (x + a - 1) / a * a; }
+static inline int itemsize(const minipic_config* cfg) { return cfg->dtype == MINIPIC_BF16 ? 2 : 4; }
+
+SplitPlan decode_split_plan(const Ctx& c, int num_seqs, int max_kv_len) {
+  // Fixed-length splits (a multiple of 64 keys) so every CTA streams the same number of bytes; chosen from host
+  // scalars only so that the grid has >= ~6 waves of CTAs when the batch allows it.
+  SplitPlan sp;
+  int sms = 148;
+  const long long want_ctas = (long long)sms * 2 * 6;
+  long long per_seq = (want_ctas + num_seqs - 1) / (num_seqs > 0 ? num_seqs : 1);
+  if (per_seq < 1) per_seq = 1;
+  long long len = (max_kv_len + per_seq - 1) / per_seq;
+  len = (len + 63) / 64 * 64;
+  if (len < 256) len = 256;
+  if (len > 2048) len = 2048;
+  sp.split_len = (int)len;
+  sp.max_splits = max_kv_len > 0 ? (max_kv_len + sp.split_len - 1) / sp.split_len : 1;
+  return sp;
+}
+size_t decode_workspace_bytes(const Ctx& c, int num_seqs, int max_kv_len) {
+  const SplitPlan sp = decode_split_plan(c, num_seqs, max_kv_len);
+  const size_t rows = (size_t)num_seqs * c.hq * sp.max_splits;
+  return align_up(rows * c.d * sizeof(float)) + align_up(rows * sizeof(float));
+}
+
+}  // namespace minipic
+
+using namespace minipic;
+
+extern "C" {
+
+const char* minipic_status_string(int status) {
+  switch (status) {
+    case MINIPIC_OK: return "MINIPIC_OK";
+    case MINIPIC_ERR_INVALID_ARG: return "MINIPIC_ERR_INVALID_ARG";
+    case MINIPIC_ERR_UNSUPPORTED: return "MINIPIC_ERR_UNSUPPORTED";
+    case MINIPIC_ERR_WORKSPACE_TOO_SMALL: return "MINIPIC_ERR_WORKSPACE_TOO_SMALL";
+    case MINIPIC_ERR_CUDA: return "MINIPIC_ERR_CUDA";
+    default: return "MINIPIC_ERR_UNKNOWN";
+  }
+}
+const char* minipic_last_cuda_error(void) { return g_cuda_err; }
+uint64_t minipic_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+const char* minipic_last_variant(void) { return g_variant; }
+
+size_t minipic_rope_table_bytes(const minipic_config* cfg, int32_t num_positions) {
+  if (validate_cfg(cfg) != MINIPIC_OK || num_positions < 0) return 0;
+  return (size_t)num_positions * (cfg->head_dim / 2) * sizeof(float2);
+}
+int minipic_rope_table_build(const minipic_config* cfg, int32_t num_positions, void* table, void* cuda_stream) {
+  int st = validate_cfg(cfg);
+  if (st != MINIPIC_OK) return st;
+  if (num_positions < 0 || (num_positions > 0 && !table)) return MINIPIC_ERR_INVALID_ARG;
+  RopeParams rp;
+  make_rope(cfg, &rp);
+  rp.table = nullptr; rp.table_len = 0;
+  launch_rope_table(rp, num_positions, (float2*)table, (cudaStream_t)cuda_stream);
+  return check_launch("rope_table") ? MINIPIC_OK : MINIPIC_ERR_CUDA;
+}
+
+int minipic_cache_write(const minipic_config* cfg, const void* k_new, const void* v_new, const int64_t* slot_mapping,
+                        int32_t num_tokens, void* k_cache, void* v_cache, void* cuda_stream) {
+  int st = validate_cfg(cfg);
+  if (st != MINIPIC_OK) return st;
+  if (num_tokens < 0) return MINIPIC_ERR_INVALID_ARG;
+  if (num_tokens == 0) return MINIPIC_OK;
+  if (!k_new || !v_new || !slot_mapping || !k_cache || !v_cache) return MINIPIC_ERR_INVALID_ARG;
+  if (((uintptr_t)k_new | (uintptr_t)v_new | (uintptr_t)k_cache | (uintptr_t)v_cache) & 15) return MINIPIC_ERR_INVALID_ARG;
+  launch_cache_write(itemsize(cfg), cfg->num_kv_heads, cfg->head_dim, k_new, v_new, slot_mapping, num_tokens, k_cache,
+                     v_cache, (cudaStream_t)cuda_stream);
+  return check_launch("cache_write") ? MINIPIC_OK : MINIPIC_ERR_CUDA;
+}
+
+size_t minipic_prefill_workspace_bytes(const minipic_config* cfg, int32_t num_reqs, int32_t num_q_tokens) {
+  if (validate_cfg(cfg) != MINIPIC_OK || num_reqs < 0 || num_q_tokens < 0) return 0;
+  Ctx c; make_ctx(cfg, nullptr, &c);
+  size_t b = 256;
+  if (prefill_sm100_supported(c)) b += prefill_sm100_workspace_bytes(c, num_reqs, num_q_tokens);
+  return b;
+}
+
+int minipic_prefill_attention(const minipic_config* cfg, const void* q, const void* k_cache, const void* v_cache,
+                              const int32_t* block_tables, int32_t max_blocks_per_req, const int32_t* cu_q_lens,
+                              const int32_t* kv_lens, const int32_t* cu_kv_lens, const int32_t* kv_positions,
+                              const int32_t* q_seq_idx, const int32_t* q_vis_lo, int32_t num_reqs, int32_t num_q_tokens,
+                              int32_t max_kv_len, void* out, float* lse, void* workspace, size_t workspace_bytes,
+                              void* cuda_stream) {
+  int st = validate_cfg(cfg);
+  if (st != MINIPIC_OK) return st;
+  if (num_reqs < 0 || num_q_tokens < 0 || max_kv_len < 0 || max_blocks_per_req < 0) return MINIPIC_ERR_INVALID_ARG;
+  if (num_q_tokens == 0 || num_reqs == 0) return MINIPIC_OK;
+  if (!q || !k_cache || !v_cache || !block_tables || !cu_q_lens || !kv_lens || !cu_kv_lens || !kv_positions ||
+      !q_seq_idx || !q_vis_lo || !out || !lse)
+    return MINIPIC_ERR_INVALID_ARG;
+  if ((long long)max_blocks_per_req * kBlock < max_kv_len) return MINIPIC_ERR_INVALID_ARG;
+  if (((uintptr_t)q | (uintptr_t)k_cache | (uintptr_t)v_cache | (uintptr_t)out) & 15) return MINIPIC_ERR_INVALID_ARG;
+  const size_t need = minipic_prefill_workspace_bytes(cfg, num_reqs, num_q_tokens);
+  if (workspace_bytes < need || (need && !workspace)) return MINIPIC_ERR_WORKSPACE_TOO_SMALL;
+  if ((uintptr_t)workspace & 255) return MINIPIC_ERR_INVALID_ARG;
+  Ctx c; make_ctx(cfg, cuda_stream, &c);
+  PrefillArgs a{q, k_cache, v_cache, block_tables, max_blocks_per_req, cu_q_lens, kv_lens, cu_kv_lens, kv_positions,
+                q_seq_idx, q_vis_lo, num_reqs, num_q_tokens, max_kv_len, out, lse, workspace, workspace_bytes};
+  if (!(c.flags & MINIPIC_FORCE_SIMT) && prefill_sm100_supported(c)) {
+    g_variant = "prefill_sm100_tcgen05";
+    if (!launch_prefill_sm100(c, a)) return MINIPIC_ERR_CUDA;
+  } else {
+    g_variant = "prefill_simt";
+    launch_prefill_simt(c, a);
+  }
+  return check_launch("prefill_attention") ? MINIPIC_OK : MINIPIC_ERR_CUDA;
+}
+
+size_t minipic_decode_workspace_bytes(const minipic_config* cfg, int32_t num_seqs, int32_t max_kv_len) {
+  if (validate_cfg(cfg) != MINIPIC_OK || num_seqs < 0 || max_kv_len < 0) return 0;
+  Ctx c; make_ctx(cfg, nullptr, &c);
+  return decode_workspace_bytes(c, num_seqs, max_kv_len);
+}
+
+int minipic_decode_attention(const minipic_config* cfg, const void* q, const void* k_cache, const void* v_cache,
+                             const int32_t* block_tables, int32_t max_blocks_per_req, const int32_t* kv_lens,
+                             const int32_t* cu_kv_lens, const int32_t* kv_positions, const int32_t* q_vis_lo,
+                             int32_t num_seqs, int32_t max_kv_len, void* out, float* lse, void* workspace,
+                             size_t workspace_bytes, void* cuda_stream) {
+  int st = validate_cfg(cfg);
+  if (st != MINIPIC_OK) return st;
+  if (num_seqs < 0 || max_kv_len < 0 || max_blocks_per_req < 0) return MINIPIC_ERR_INVALID_ARG;
+  if (num_seqs == 0) return MINIPIC_OK;
+  if (!q || !k_cache || !v_cache || !block_tables || !kv_lens || !cu_kv_lens || !kv_positions || !out || !lse)
+    return MINIPIC_ERR_INVALID_ARG;
+  if ((long long)max_blocks_per_req * kBlock < max_kv_len) return MINIPIC_ERR_INVALID_ARG;
+  if (((uintptr_t)q | (uintptr_t)k_cache | (uintptr_t)v_cache | (uintptr_t)out) & 15) return MINIPIC_ERR_INVALID_ARG;
+  Ctx c; make_ctx(cfg, cuda_stream, &c);
+  const size_t need = decode_workspace_bytes(c, num_seqs, max_kv_len);
+  if (workspace_bytes < need || !workspace) return MINIPIC_ERR_WORKSPACE_TOO_SMALL;
+  if ((uintptr_t)workspace & 255) return MINIPIC_ERR_INVALID_ARG;
+  const SplitPlan sp = decode_split_plan(c, num_seqs, max_kv_len);
+  const size_t rows = (size_t)num_seqs * c.hq * sp.max_splits;
+  float* o_part = (float*)workspace;
+  float* lse_part = (float*)((char*)workspace + align_up(rows * c.d * sizeof(float)));
+  DecodeArgs a{q, k_cache, v_cache, block_tables, max_blocks_per_req, kv_lens, cu_kv_lens, kv_positions, q_vis_lo,
+               num_seqs, max_kv_len, out, lse, workspace, workspace_bytes};
+  if (!(c.flags & MINIPIC_FORCE_SIMT) && decode_mma_supported(c)) {
+    g_variant = "decode_mma";
+    launch_decode_mma(c, a, sp, o_part, lse_part);
+  } else {
+    g_variant = "decode_simt";
+    launch_decode_simt(c, a, sp, o_part, lse_part);
+  }
+  if (!check_launch("decode_partial")) return MINIPIC_ERR_CUDA;
+  launch_lse_merge(c, a, sp, o_part, lse_part);
+  return check_launch("lse_merge") ? MINIPIC_OK : MINIPIC_ERR_CUDA;
+}
+
+}  // extern "C"
+
+// ------------------------------------------------------------------------------------------------ host-buffer steps
+namespace {
+struct Arena {
+  char* base; size_t size; size_t off = 0; bool ok = true;
+  void* take(size_t bytes) {
+    size_t o = align_up(off);
+    if (o + bytes > size) { ok = false; return nullptr; }
+    off = o + bytes;
+    return base + o;
+  }
+};
+struct ArenaSizer {
+  size_t off = 0;
+  void take(size_t bytes) { off = align_up(off) + bytes; }
+};
+template <typename A>
+void* up(A& ar, const void* host, size_t bytes, cudaStream_t s, bool* ok) {
+  if (bytes == 0) return nullptr;
+  void* d = ar.take(bytes);
+  if (!d) { *ok = false; return nullptr; }
+  if (cudaMemcpyAsync(d, host, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) *ok = false;
+  return d;
+}
+}  // namespace
+
+extern "C" {
+
+size_t minipic_prefill_host_arena_bytes(const minipic_config* cfg, int32_t num_reqs, int32_t num_q_tokens,
+                                        int32_t num_new_tokens, int32_t max_blocks_per_req, int32_t total_kv_len) {
+  if (validate_cfg(cfg) != MINIPIC_OK) return 0;
+  const size_t is = itemsize(cfg), d = cfg->head_dim;
+  ArenaSizer a;
+  a.take((size_t)num_new_tokens * cfg->num_kv_heads * d * is); a.take((size_t)num_new_tokens * cfg->num_kv_heads * d * is);
+  a.take((size_t)num_new_tokens * 8);
+  a.take((size_t)num_q_tokens * cfg->num_q_heads * d * is);
+  a.take((size_t)num_reqs * max_blocks_per_req * 4);
+  a.take((size_t)(num_reqs + 1) * 4); a.take((size_t)num_reqs * 4); a.take((size_t)(num_reqs + 1) * 4);
+  a.take((size_t)total_kv_len * 4); a.take((size_t)num_q_tokens * 4); a.take((size_t)num_q_tokens * 4);
+  a.take((size_t)num_q_tokens * cfg->num_q_heads * d * is); a.take((size_t)num_q_tokens * cfg->num_q_heads * 4);
+  a.take(minipic_prefill_workspace_bytes(cfg, num_reqs, num_q_tokens));
+  return align_up(a.off) + 256;
+}
+
+int minipic_prefill_step_host(const minipic_config* cfg, const void* k_new_host, const void* v_new_host,
+                              const int64_t* slot_mapping_host, int32_t num_new_tokens, const void* q_host, void* k_cache,
+                              void* v_cache, const int32_t* block_tables_host, int32_t max_blocks_per_req,
+                              const int32_t* cu_q_lens_host, const int32_t* kv_lens_host, const int32_t* cu_kv_lens_host,
+                              const int32_t* kv_positions_host, const int32_t* q_seq_idx_host,
+                              const int32_t* q_vis_lo_host, int32_t num_reqs, int32_t num_q_tokens, int32_t max_kv_len,
+                              void* out_host, float* lse_host, void* arena, size_t arena_bytes, void* cuda_stream) {
+  int st = validate_cfg(cfg);
+  if (st != MINIPIC_OK) return st;
+  if (num_reqs <= 0 || num_q_tokens <= 0 || num_new_tokens < 0 || !arena || ((uintptr_t)arena & 255)) return MINIPIC_ERR_INVALID_ARG;
+  if (!q_host || !cu_kv_lens_host || !out_host || !lse_host) return MINIPIC_ERR_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const size_t is = itemsize(cfg), d = cfg->head_dim;
+  const int total_kv = cu_kv_lens_host[num_reqs];
+  Arena ar{(char*)arena, arena_bytes};
+  bool ok = true;
+  const size_t kvb = (size_t)num_new_tokens * cfg->num_kv_heads * d * is;
+  void* dk = up(ar, k_new_host, kvb, s, &ok);
+  void* dv = up(ar, v_new_host, kvb, s, &ok);
+  void* dslots = up(ar, slot_mapping_host, (size_t)num_new_tokens * 8, s, &ok);
+  const size_t qb = (size_t)num_q_tokens * cfg->num_q_heads * d * is;
+  void* dq = up(ar, q_host, qb, s, &ok);
+  void* dbt = up(ar, block_tables_host, (size_t)num_reqs * max_blocks_per_req * 4, s, &ok);
+  void* dcuq = up(ar, cu_q_lens_host, (size_t)(num_reqs + 1) * 4, s, &ok);
+  void* dkvl = up(ar, kv_lens_host, (size_t)num_reqs * 4, s, &ok);
+  void* dcukv = up(ar, cu_kv_lens_host, (size_t)(num_reqs + 1) * 4, s, &ok);
+  void* dpos = up(ar, kv_positions_host, (size_t)total_kv * 4, s, &ok);
+  void* didx = up(ar, q_seq_idx_host, (size_t)num_q_tokens * 4, s, &ok);
+  void* dlo = up(ar, q_vis_lo_host, (size_t)num_q_tokens * 4, s, &ok);
+  void* dout = ar.take(qb);
+  float* dlse = (float*)ar.take((size_t)num_q_tokens * cfg->num_q_heads * 4);
+  const size_t wsb = minipic_prefill_workspace_bytes(cfg, num_reqs, num_q_tokens);
+  void* ws = ar.take(wsb);
+  if (!ar.ok || !dout || !dlse || !ws) return MINIPIC_ERR_WORKSPACE_TOO_SMALL;
+  if (!ok) { check_launch("h2d"); return MINIPIC_ERR_CUDA; }
+  if (num_new_tokens) {
+    st = minipic_cache_write(cfg, dk, dv, (const int64_t*)dslots, num_new_tokens, k_cache, v_cache, cuda_stream);
+    if (st != MINIPIC_OK) return st;
+  }
+  st = minipic_prefill_attention(cfg, dq, k_cache, v_cache, (const int*)dbt, max_blocks_per_req, (const int*)dcuq,
+                                 (const int*)dkvl, (const int*)dcukv, (const int*)dpos, (const int*)didx, (const int*)dlo,
+                                 num_reqs, num_q_tokens, max_kv_len, dout, dlse, ws, wsb, cuda_stream);
+  if (st != MINIPIC_OK) return st;
+  if (cudaMemcpyAsync(out_host, dout, qb, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+      cudaMemcpyAsync(lse_host, dlse, (size_t)num_q_tokens * cfg->num_q_heads * 4, cudaMemcpyDeviceToHost, s) != cudaSuccess) {
+    check_launch("d2h");
+    return MINIPIC_ERR_CUDA;
+  }
+  return MINIPIC_OK;
+}
+
+size_t minipic_decode_host_arena_bytes(const minipic_config* cfg, int32_t num_seqs, int32_t num_new_tokens,
+                                       int32_t max_blocks_per_req, int32_t total_kv_len, int32_t max_kv_len) {
+  if (validate_cfg(cfg) != MINIPIC_OK) return 0;
+  const size_t is = itemsize(cfg), d = cfg->head_dim;
+  ArenaSizer a;
+  a.take((size_t)num_new_tokens * cfg->num_kv_heads * d * is); a.take((size_t)num_new_tokens * cfg->num_kv_heads * d * is);
+  a.take((size_t)num_new_tokens * 8);
+  a.take((size_t)num_seqs * cfg->num_q_heads * d * is);
+  a.take((size_t)num_seqs * max_blocks_per_req * 4);
+  a.take((size_t)num_seqs * 4); a.take((size_t)(num_seqs + 1) * 4); a.take((size_t)total_kv_len * 4); a.take((size_t)num_seqs * 4);
+  a.take((size_t)num_seqs * cfg->num_q_heads * d * is); a.take((size_t)num_seqs * cfg->num_q_heads * 4);
+  a.take(minipic_decode_workspace_bytes(cfg, num_seqs, max_kv_len));
+  return align_up(a.off) + 256;
+}
+
+int minipic_decode_step_host(const minipic_config* cfg, const void* k_new_host, const void* v_new_host,
+                             const int64_t* slot_mapping_host, int32_t num_new_tokens, const void* q_host, void* k_cache,
+                             void* v_cache, const int32_t* block_tables_host, int32_t max_blocks_per_req,
+                             const int32_t* kv_lens_host, const int32_t* cu_kv_lens_host, const int32_t* kv_positions_host,
+                             const int32_t* q_vis_lo_host, int32_t num_seqs, int32_t max_kv_len, void* out_host,
+                             float* lse_host, void* arena, size_t arena_bytes, void* cuda_stream) {
+  int st = validate_cfg(cfg);
+  if (st != MINIPIC_OK) return st;
+  if (num_seqs <= 0 || num_new_tokens < 0 || !arena || ((uintptr_t)arena & 255)) return MINIPIC_ERR_INVALID_ARG;
+  if (!q_host || !cu_kv_lens_host || !out_host || !lse_host) return MINIPIC_ERR_INVALID_ARG;
+  cudaStream_t s = (cudaStream_t)cuda_stream;
+  const size_t is = itemsize(cfg), d = cfg->head_dim;
+  const int total_kv = cu_kv_lens_host[num_seqs];
+  Arena ar{(char*)arena, arena_bytes};
+  bool ok = true;
+  const size_t kvb = (size_t)num_new_tokens * cfg->num_kv_heads * d * is;
+  void* dk = up(ar, k_new_host, kvb, s, &ok);
+  void* dv = up(ar, v_new_host, kvb, s, &ok);
+  void* dslots = up(ar, slot_mapping_host, (size_t)num_new_tokens * 8, s, &ok);
+  const size_t qb = (size_t)num_seqs * cfg->num_q_heads * d * is;
+  void* dq = up(ar, q_host, qb, s, &ok);
+  void* dbt = up(ar, block_tables_host, (size_t)num_seqs * max_blocks_per_req * 4, s, &ok);
+  void* dkvl = up(ar, kv_lens_host, (size_t)num_seqs * 4, s, &ok);
+  void* dcukv = up(ar, cu_kv_lens_host, (size_t)(num_seqs + 1) * 4, s, &ok);
+  void* dpos = up(ar, kv_positions_host, (size_t)total_kv * 4, s, &ok);
+  void* dlo = q_vis_lo_host ? up(ar, q_vis_lo_host, (size_t)num_seqs * 4, s, &ok) : nullptr;
+  void* dout = ar.take(qb);
+  float* dlse = (float*)ar.take((size_t)num_seqs * cfg->num_q_heads * 4);
+  const size_t wsb = minipic_decode_workspace_bytes(cfg, num_seqs, max_kv_len);
+  void* ws = ar.take(wsb);
+  if (!ar.ok || !dout || !dlse || !ws) return MINIPIC_ERR_WORKSPACE_TOO_SMALL;
+  if (!ok) { check_launch("h2d"); return MINIPIC_ERR_CUDA; }
+  if (num_new_tokens) {
+    st = minipic_cache_write(cfg, dk, dv, (const int64_t*)dslots, num_new_tokens, k_cache, v_cache, cuda_stream);
+    if (st != MINIPIC_OK) return st;
+  }
+  st = minipic_decode_attention(cfg, dq, k_cache, v_cache, (const int*)dbt, max_blocks_per_req, (const int*)dkvl,
+                                (const int*)dcukv, (const int*)dpos, (const int*)dlo, num_seqs, max_kv_len, dout, dlse, ws,
+                                wsb, cuda_stream);
+  if (st != MINIPIC_OK) return st;
+  if (cudaMemcpyAsync(out_host, dout, qb, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
+      cudaMemcpyAsync(lse_host, dlse, (size_t)num_seqs * cfg->num_q_heads * 4, cudaMemcpyDeviceToHost, s) != cudaSuccess) {
+    check_launch("d2h");
+    return MINIPIC_ERR_CUDA;
+  }
+  return MINIPIC_OK;
+}
+
+}  // extern "C"

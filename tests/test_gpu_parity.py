@@ -1,0 +1,277 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle, element by element, on the same
+seeded inputs.  All tests here need a GPU (-m gpu).
+
+Bars (BASELINE.json north_star, reading R1):
+  * cache write, block-table indexing: bit exact.
+  * bf16 I/O attention output: max-abs <= 2e-2 and mean-abs <= 2e-3 against the pure-fp64 oracle (mode F).
+  * LSE: max-abs <= 1e-3 against the oracle whose score operands have the kernel's precision
+    (mode Q = q', k_j rounded to bf16 for the tensor-core kernels; mode F for the fp32 CUDA-core kernels),
+    and mean-abs <= 1e-3 against mode F.
+  * fp32 I/O (config 1): out and LSE within 1e-4 of mode F.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import minipic_oracle as O
+from paper_2606_13126_b200 import binding as mp
+from paper_2606_13126_b200 import workloads as W
+from paper_2606_13126_b200.runner import DeviceWorkload, HostStep
+
+pytestmark = pytest.mark.gpu
+
+OUT_MAX, OUT_MEAN, LSE_TOL = 2e-2, 2e-3, 1e-3
+
+
+def compare(dw, rows=None, heads=None, oracle_cache=None, expect_variant=None, k_prerot=False):
+    w = dw.w
+    kc, vc = oracle_cache if oracle_cache is not None else O.build_cache(w)
+    of, lf = O.run_workload(w, kc, vc, mode="F", rows=rows, heads=heads, k_prerotated=k_prerot)
+    variant = mp.minipic_last_variant()
+    if expect_variant:
+        assert variant == expect_variant, variant
+    go, gl = dw.out_f64(), dw.lse_f64()
+    sel = ~np.isnan(lf)
+    assert sel.any()
+    do = np.abs(go - of)[sel]
+    dl = np.abs(gl - lf)[sel]
+    stats = dict(variant=variant, out_max=float(do.max()), out_mean=float(do.mean()), lse_max_F=float(dl.max()),
+                 lse_mean_F=float(dl.mean()))
+    if w.dtype == "f32":
+        assert do.max() <= 1e-4 and dl.max() <= 1e-4, stats
+        return stats
+    assert do.max() <= OUT_MAX and do.mean() <= OUT_MEAN, stats
+    assert dl.mean() <= LSE_TOL, stats
+    if "simt" in variant:
+        assert dl.max() <= LSE_TOL, stats
+    else:
+        _, lq = O.run_workload(w, kc, vc, mode="Q", rows=rows, heads=heads, k_prerotated=k_prerot)
+        dq = np.abs(gl - lq)[sel]
+        stats["lse_max_Q"] = float(dq.max())
+        assert dq.max() <= LSE_TOL, stats
+    return stats
+
+
+# --------------------------------------------------------------------------- a1 cache write: bit exact
+@pytest.mark.parametrize("dtype", ["bf16", "f32"])
+def test_cache_write_bit_exact_with_sentinel(dtype):
+    w = W.small_variants()[1] if dtype == "bf16" else W.config1()
+    fill = 0x5A5A if dtype == "bf16" else None
+    dw = DeviceWorkload(w, cache_fill=(0x5A5A if dtype == "bf16" else -7), upload_resident=True)
+    dw.write_new()
+    torch.cuda.synchronize()
+    gk, gv = dw.cache_bits()
+    kc, vc = O.build_cache(w, fill=(0x5A5A if dtype == "bf16" else -7))
+    assert gk.tobytes() == kc.tobytes() and gv.tobytes() == vc.tobytes()
+
+
+def test_cache_write_skips_negative_slots_and_all_bit_patterns():
+    rng = np.random.default_rng(3)
+    hkv, d, nb, T = 8, 128, 40, 333
+    k = rng.integers(0, 65536, (T, hkv, d)).astype(np.uint16)
+    v = rng.integers(0, 65536, (T, hkv, d)).astype(np.uint16)
+    slots = rng.permutation(nb * 16)[:T].astype(np.int64)
+    slots[[0, 5, 77, 332]] = [-1, -9, -1, -2]
+    kc = O.new_cache(nb, hkv, 16, d, "bf16", 0x1234); vc = O.new_cache(nb, hkv, 16, d, "bf16", 0x1234)
+    O.cache_write(kc, vc, k, v, slots)
+    cfg = mp.make_config(num_q_heads=8, num_kv_heads=hkv, head_dim=d, num_blocks=nb, dtype="bf16", rope_theta=1e4)
+    dk = torch.from_numpy(k.view(np.int16)).cuda(); dv = torch.from_numpy(v.view(np.int16)).cuda()
+    ds = torch.from_numpy(slots).cuda()
+    gk = torch.full((nb, hkv, 16, d), 0x1234, dtype=torch.int16, device="cuda"); gv = gk.clone()
+    mp.minipic_cache_write(cfg, dk, dv, ds, T, gk, gv)
+    torch.cuda.synchronize()
+    assert gk.cpu().numpy().view(np.uint16).tobytes() == kc.tobytes()
+    assert gv.cpu().numpy().view(np.uint16).tobytes() == vc.tobytes()
+    mp.minipic_cache_write(cfg, dk, dv, ds, 0, gk, gv)      # empty write is a no-op
+    torch.cuda.synchronize()
+    assert gk.cpu().numpy().view(np.uint16).tobytes() == kc.tobytes()
+
+
+# --------------------------------------------------------------------------- config 1 (fp32, tiny)
+def test_config1_fp32_prefill_and_decode():
+    w = W.config1()
+    dw = DeviceWorkload(w)
+    dw.step(); torch.cuda.synchronize()
+    st = compare(dw, expect_variant="prefill_simt")
+    wd = W.decode_from_prefill(w)
+    dd = DeviceWorkload(wd)
+    dd.step(); torch.cuda.synchronize()
+    compare(dd, expect_variant="decode_simt")
+    # with a cos/sin table the result is the same within fp32 rounding
+    dt = DeviceWorkload(w, rope_table_positions=112)
+    dt.step(); torch.cuda.synchronize()
+    compare(dt)
+    # positions beyond the table fall back to the in-kernel phase computation
+    dt2 = DeviceWorkload(w, rope_table_positions=40)
+    dt2.step(); torch.cuda.synchronize()
+    compare(dt2)
+
+
+# --------------------------------------------------------------------------- small relatives of configs 2-5, all paths
+@pytest.mark.parametrize("which", [0, 1, 2, 3])
+@pytest.mark.parametrize("force_simt", [False, True])
+@pytest.mark.parametrize("table", [False, True])
+def test_small_variants_full_parity(which, force_simt, table):
+    w = W.small_variants()[which]
+    dw = DeviceWorkload(w, flags=mp.MINIPIC_FORCE_SIMT if force_simt else 0,
+                        rope_table_positions=(w.max_kv_len + 5) if table else None)
+    dw.step(); torch.cuda.synchronize()
+    compare(dw)
+
+
+@pytest.mark.parametrize("seed", [101, 202, 303])
+def test_seed_sweep_ragged_shapes(seed):
+    """Ragged spans (lengths not multiples of the 128-key tile), several requests, G=4 and G=8."""
+    w = W.rag_partial_prefill(name="ragged", seed=seed, hq=16, hkv=2, pool_spans=9, span_min=17, span_max=300,
+                              num_reqs=4, spans_per_req=3, prefix_len=16, suffix_len=48)
+    dw = DeviceWorkload(w); dw.step(); torch.cuda.synchronize()
+    compare(dw)
+    wd = W.shared_pool_decode(name="ragged_dec", seed=seed, hq=8, hkv=2, num_seqs=7, ctx_min=1, ctx_max=700,
+                              span_len=64, pool_spans=12)
+    dd = DeviceWorkload(wd); dd.step(); torch.cuda.synchronize()
+    compare(dd)
+
+
+def test_position_shift_invariance_and_large_positions_on_gpu():
+    """PAPER.md:30, :127 on the CUDA path: shifting every logical position of a request by a constant leaves
+    the output unchanged within tolerance, including positions far beyond any table (c = 10^6)."""
+    base = W.single_request_prefill(name="shift", hq=8, hkv=2, d=128, theta=5e5, dtype="bf16", sigma=1.0,
+                                    span_lens=[160, 96], suffix_len=32, num_blocks=40, seed=5)
+    kc, vc = O.build_cache(base)
+    for c in (0, 4096, 10 ** 6):
+        w = W.single_request_prefill(name="shift", hq=8, hkv=2, d=128, theta=5e5, dtype="bf16", sigma=1.0,
+                                     span_lens=[160, 96], suffix_len=32, num_blocks=40, seed=5, pos_offset=c)
+        dw = DeviceWorkload(w, rope_table_positions=512 if c else None)
+        dw.step(); torch.cuda.synchronize()
+        compare(dw, oracle_cache=(kc, vc))
+
+
+def test_k_prerotated_control_matches():
+    """MINIPIC_K_PREROTATED control: a cache holding oracle-rotated keys (rounded to bf16) with the in-kernel
+    K RoPE switched off gives the same attention within the same tolerances."""
+    w = W.small_variants()[0]
+    kc, vc = O.build_cache(w)
+    # oracle-side pre-rotation of the written K rows at their logical positions (single request: pos = index)
+    nb = w.new[0]
+    pos = np.empty(nb.slots.shape[0], np.int64)
+    bt = w.block_tables[0]
+    inv = {int(b): i for i, b in enumerate(bt.tolist())}
+    for t, s in enumerate(nb.slots.tolist()):
+        pos[t] = inv[s // 16] * 16 + s % 16
+    kr = O.round_to_dtype(O.rope_rotate(O.to_f64(nb.k, "bf16"), pos[:, None], w.rope_theta), "bf16")
+    kr_bits = W.f32_to_bf16_bits(kr.astype(np.float32))
+    w2 = W.Workload(**{**w.__dict__, "new": [W.WriteBatch(kr_bits, nb.v, nb.slots, "prerot")]})
+    dw = DeviceWorkload(w2, flags=mp.MINIPIC_K_PREROTATED)
+    dw.step(); torch.cuda.synchronize()
+    kc2, vc2 = O.build_cache(w2)
+    compare(dw, oracle_cache=(kc2, vc2), k_prerot=True)
+    # and it agrees with the in-kernel-RoPE run on the unrotated cache
+    d0 = DeviceWorkload(w); d0.step(); torch.cuda.synchronize()
+    assert np.abs(d0.out_f64() - dw.out_f64()).max() <= OUT_MAX
+    assert np.abs(d0.lse_f64() - dw.lse_f64()).max() <= 2e-2
+
+
+def test_shared_and_duplicate_blocks_on_gpu():
+    """one physical block in several requests at different offsets, and twice in one."""
+    w = W.small_variants()[1]
+    w = W.Workload(**w.__dict__)
+    bt = w.block_tables.copy()
+    bt[1, 3] = bt[0, 2]; bt[2, 5] = bt[0, 2]; bt[2, 6] = bt[0, 2]          # same block at offsets 2 / 3 / 5 / 6
+    w.block_tables = bt
+    dw = DeviceWorkload(w); dw.step(); torch.cuda.synchronize()
+    compare(dw)
+
+
+def test_run_to_run_determinism():
+    w = W.small_variants()[3]
+    dw = DeviceWorkload(w)
+    dw.step(); torch.cuda.synchronize()
+    o1, l1 = dw.out.clone(), dw.lse.clone()
+    for _ in range(3):
+        dw.attention(); torch.cuda.synchronize()
+        assert torch.equal(o1, dw.out) and torch.equal(l1, dw.lse)
+    wd = W.small_variants()[2]
+    dd = DeviceWorkload(wd); dd.step(); torch.cuda.synchronize()
+    o1, l1 = dd.out.clone(), dd.lse.clone()
+    dd.attention(); torch.cuda.synchronize()
+    assert torch.equal(o1, dd.out) and torch.equal(l1, dd.lse)
+
+
+def test_degenerate_inputs():
+    # a query that sees only itself; a one-token context; vis_lo > idx (no visible key)
+    w = W.single_request_prefill(name="deg", hq=8, hkv=2, d=128, theta=5e5, dtype="bf16", sigma=1.0,
+                                 span_lens=[16], suffix_len=0, num_blocks=4, seed=9)
+    w.q_vis_lo = w.q_seq_idx.copy()
+    w.q_vis_lo[3] = 7                                   # row 3 (idx 3): vis_lo > idx -> out 0, lse -inf
+    dw = DeviceWorkload(w); dw.step(); torch.cuda.synchronize()
+    go, gl = dw.out_f64(), dw.lse_f64()
+    assert np.isneginf(gl[3]).all() and (go[3] == 0).all()
+    kc, vc = O.build_cache(w)
+    of, lf = O.run_workload(w, kc, vc)
+    keep = np.arange(16) != 3
+    assert np.abs(go[keep] - of[keep]).max() <= OUT_MAX
+    wd = W.shared_pool_decode(name="one", seed=1, hq=8, hkv=2, num_seqs=3, ctx_min=1, ctx_max=1, span_len=64, pool_spans=2)
+    dd = DeviceWorkload(wd); dd.step(); torch.cuda.synchronize()
+    compare(dd)
+    # empty batch: no launch, OK status
+    cfg = dw.cfg
+    mp.minipic_prefill_attention(cfg, dw.q, dw.k_cache, dw.v_cache, dw.block_tables, 1, dw.cu_q_lens, dw.kv_lens,
+                                 dw.cu_kv_lens, dw.kv_positions, dw.q_seq_idx, dw.q_vis_lo, 1, 0, 16, dw.out, dw.lse,
+                                 dw.workspace, dw.ws_bytes)
+
+
+def test_host_step_entry_points_match_device_path():
+    for w in (W.small_variants()[0], W.small_variants()[2]):
+        dw = DeviceWorkload(w)
+        hs = HostStep(dw)
+        hs.run(); torch.cuda.synchronize()
+        dw2 = DeviceWorkload(w); dw2.step(); torch.cuda.synchronize()
+        assert np.array_equal(hs.out_f64(), dw2.out_f64()) and np.array_equal(hs.lse_f64(), dw2.lse_f64())
+        assert hs.h2d_bytes > 0 and hs.d2h_bytes > 0
+
+
+# --------------------------------------------------------------------------- BASELINE configs at full size
+def _sampled(w, n_rows, n_heads, seed=0):
+    rng = np.random.default_rng(seed)
+    rows = np.sort(rng.choice(w.num_q_tokens, size=min(n_rows, w.num_q_tokens), replace=False))
+    # always include first / last row of the batch and of some span boundaries
+    rows = np.unique(np.concatenate([rows, [0, w.num_q_tokens - 1]]))
+    heads = np.sort(rng.choice(w.num_q_heads, size=min(n_heads, w.num_q_heads), replace=False))
+    return rows, heads
+
+
+def test_config2_full():
+    w = W.config2()
+    dw = DeviceWorkload(w, rope_table_positions=2112)
+    dw.step(); torch.cuda.synchronize()
+    compare(dw, heads=np.array([0, 5, 17, 31]))
+    gk, gv = dw.cache_bits(); kc, vc = O.build_cache(w)
+    assert gk.tobytes() == kc.tobytes() and gv.tobytes() == vc.tobytes()
+
+
+def test_config3_full_sampled():
+    w = W.config3()
+    dw = DeviceWorkload(w, rope_table_positions=w.max_kv_len)
+    dw.step(); torch.cuda.synchronize()
+    rows, heads = _sampled(w, 160, 3)
+    compare(dw, rows=rows, heads=heads)
+    gk, gv = dw.cache_bits(); kc, vc = O.build_cache(w)
+    assert gk.tobytes() == kc.tobytes() and gv.tobytes() == vc.tobytes()
+
+
+def test_config4_full_sampled():
+    w = W.config4()
+    dw = DeviceWorkload(w, rope_table_positions=8192)
+    dw.step(); torch.cuda.synchronize()
+    compare(dw, rows=np.array([0, 1, 17, 100, 255]), heads=np.array([0, 9, 31]))
+
+
+def test_config5_full_sampled():
+    w = W.config5()
+    dw = DeviceWorkload(w, rope_table_positions=w.max_kv_len)
+    dw.step(); torch.cuda.synchronize()
+    rows, heads = _sampled(w, 96, 2)
+    # add suffix rows of every request (they see ~33K keys) and first rows of a span
+    extra = [int(w.cu_q_lens[r + 1]) - 1 for r in range(w.num_reqs)] + [int(w.cu_q_lens[r]) for r in range(w.num_reqs)]
+    rows = np.unique(np.concatenate([rows, extra]))
+    compare(dw, rows=rows, heads=heads)
