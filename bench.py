@@ -1,0 +1,360 @@
+#!/usr/bin/env python
+"""bench.py - MiniPIC hot path on B200: one JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--no-extras]
+
+A *step* is one pass of the whole hot path over one batch of synthetic input:
+    config 5 (long-context prefill, Llama-3-70B shapes): cache_write(new K/V) -> prefill attention
+    config 4 (decode over shared position-free blocks) : cache_write(new K/V) -> split-KV decode -> LSE merge
+`value` = query tokens of both legs / device time, inputs resident in HBM.  `e2e` = the same through the
+*_step_host C entry points (pinned host inputs, H2D + kernels + D2H inside the timed region).
+N > 1 runs N independent replicas (the path does not shard: DESIGN.md "Multi-GPU"), no data-path collective.
+`--impl reference` times the CPU oracle (oracle/) on a bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "attention_tokens_per_s"
+UNIT = "tokens/s"
+WORKLOAD = ("c5_long_context_prefill(R=4,Hq=64,Hkv=8,D=128,64x512-token spans+256 suffix,half cached) + "
+            "c4_decode_shared_pool(R=256,Hq=32,Hkv=8,D=128,ctx U[4096,8192])")
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        j = json.load(open(p))
+        return dict(hbm_gbs=float(j["hbm_gbs"]), bf16_tflops=float(j["bf16_tflops"]),
+                    bf16_tflops_sustained=float(j.get("bf16_tflops_sustained", j["bf16_tflops"])), source="measured")
+    return dict(hbm_gbs=6650.0, bf16_tflops=1590.0, bf16_tflops_sustained=1400.0, source="fallback")
+
+
+def load_traffic():
+    """dram bytes per launch from the committed ncu --set full capture (profiles/traffic.json), else None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        try:
+            return json.load(open(p))
+        except Exception:
+            return {}
+    return {}
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock + throttle reasons through NVML while the timed region runs."""
+    REASONS = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+               0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting"}
+
+    def __init__(self, index: int, period: float = 0.02):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.stop_flag = threading.Event()
+        self.sm, self.reasons, self.max_sm, self.ok = [], set(), None, False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_sm = int(pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM))
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        while not self.stop_flag.is_set():
+            try:
+                self.sm.append(int(self.nv.nvmlDeviceGetClockInfo(self.h, self.nv.NVML_CLOCK_SM)))
+                bits = int(self.nv.nvmlDeviceGetCurrentClocksEventReasons(self.h))
+                for b, name in self.REASONS.items():
+                    if bits & b:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def summary(self):
+        if not self.ok or not self.sm:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_sm, "reasons": ["unavailable"]}
+        return {"sm_mhz": float(np.median(self.sm)), "sm_max_mhz": self.max_sm, "reasons": sorted(self.reasons),
+                "samples": len(self.sm)}
+
+
+# ------------------------------------------------------------------------------------------- CPU oracle leg
+_ORACLE_CACHES = {}
+
+
+def oracle_sample_time(w5, w4, span_rows=1024, suffix_rows=256, heads5=1, seqs4=4, heads4=1):
+    """Time the oracle, as it stands, on a bounded sample of the step's workload; extrapolate by visible
+    (query, key, head) pair count.  Returns (seconds_per_full_step_estimate, sample description, seconds)."""
+    from oracle import minipic_oracle as O
+    for w in (w5, w4):
+        if id(w) not in _ORACLE_CACHES:
+            _ORACLE_CACHES[id(w)] = O.build_cache(w)
+    (kc5, vc5), (kc4, vc4) = _ORACLE_CACHES[id(w5)], _ORACLE_CACHES[id(w4)]
+    # config 5, request 0: the first `span_rows` span-local rows and the last `suffix_rows` suffix rows
+    t0, t1 = int(w5.cu_q_lens[0]), int(w5.cu_q_lens[1])
+    rows = np.concatenate([np.arange(t0, t0 + span_rows), np.arange(t1 - suffix_rows, t1)])
+    h5, s4, h4 = np.arange(heads5), np.arange(seqs4), np.arange(heads4)
+    tic = time.perf_counter()
+    O.run_workload(w5, kc5, vc5, mode="F", rows=rows, heads=h5)
+    O.run_workload(w4, kc4, vc4, mode="F", rows=s4, heads=h4)
+    sec = time.perf_counter() - tic
+    pairs5 = int((w5.q_seq_idx[rows].astype(np.int64) - w5.q_vis_lo[rows] + 1).sum()) * heads5
+    pairs4 = int(w4.kv_lens[s4].astype(np.int64).sum()) * heads4
+    total = w5.visible_pairs() * w5.num_q_heads + w4.visible_pairs() * w4.num_q_heads
+    est_full = sec * total / (pairs5 + pairs4)
+    desc = (f"c5 request 0: first {span_rows} span rows + last {suffix_rows} suffix rows x {heads5} head; "
+            f"c4: {seqs4} sequences x {heads4} head; fp64 numpy oracle (cache build untimed); extrapolated to the full "
+            f"step by visible (query,key,head) pairs ({pairs5 + pairs4:.3g} of {total:.3g})")
+    return est_full, desc, sec
+
+
+def host_threads():
+    try:
+        from threadpoolctl import threadpool_info
+        n = [i.get("num_threads", 1) for i in threadpool_info()]
+        return max(n) if n else 1
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    from paper_2606_13126_b200 import workloads as W
+    w5, w4 = W.config5(), W.config4()
+    tokens = w5.num_q_tokens + w4.num_q_tokens
+    for _ in range(args.warmup):
+        oracle_sample_time(w5, w4, span_rows=128, suffix_rows=32, seqs4=1)
+    secs, ests, desc = [], [], ""
+    tic = time.perf_counter()
+    for _ in range(args.steps):
+        est, desc, sec = oracle_sample_time(w5, w4, span_rows=512, suffix_rows=64, seqs4=2)
+        ests.append(est); secs.append(sec)
+    est = float(np.mean(ests))
+    val = tokens / est
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": est * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "note": "each timed step is a bounded sample of the workload, "
+                       "ms_per_step is the extrapolated full-step time"},
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": host_threads(), "kind": "oracle", "sample": desc},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0, "sample_seconds_per_step": float(np.mean(secs))}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ------------------------------------------------------------------------------------------- CUDA leg
+def time_calls(fn, iters, warmup, torch):
+    for _ in range(warmup):
+        fn()
+    torch.cuda.synchronize()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(iters)]
+    for a, b in evs:
+        a.record(); fn(); b.record()
+    torch.cuda.synchronize()
+    ms = np.array([a.elapsed_time(b) for a, b in evs])
+    return float(np.median(ms)), float(ms.min())
+
+
+def run_ours(args):
+    import torch
+    from paper_2606_13126_b200 import binding as mp
+    from paper_2606_13126_b200 import build as mpbuild
+    from paper_2606_13126_b200 import dist
+    from paper_2606_13126_b200 import workloads as W
+    from paper_2606_13126_b200.runner import DeviceWorkload, HostStep
+
+    rank, local_rank, world = dist.init()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the MiniPIC hot path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    if rank == 0:
+        mpbuild.build()
+    dist.barrier()
+    mp.lib()
+    peaks = load_peaks()
+
+    w5 = W.config5(seed=4 + 1000 * rank)
+    w4 = W.config4(seed=3 + 1000 * rank)
+    d5 = DeviceWorkload(w5, device=dev, rope_table_positions=w5.max_kv_len)
+    d4 = DeviceWorkload(w4, device=dev, rope_table_positions=w4.max_kv_len)
+    tokens_per_step = w5.num_q_tokens + w4.num_q_tokens
+
+    def step(ev=None):
+        if ev: ev[0].record()
+        d5.write_new()
+        if ev: ev[1].record()
+        d5.attention()
+        if ev: ev[2].record()
+        d4.write_new()
+        if ev: ev[3].record()
+        d4.attention()
+        if ev: ev[4].record()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    variant5 = None
+    d5.attention(); variant5 = mp.minipic_last_variant()
+    d4.attention(); variant4 = mp.minipic_last_variant()
+    torch.cuda.synchronize()
+
+    evs = [[torch.cuda.Event(enable_timing=True) for _ in range(5)] for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank)
+    launches0 = mp.minipic_launch_count()
+    dist.barrier(); torch.cuda.synchronize()
+    sampler.start()
+    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_start.record()
+    for k in range(args.steps):
+        step(evs[k])
+    t_end.record()
+    torch.cuda.synchronize(); dist.barrier()
+    sampler.stop_flag.set(); sampler.join(2.0)
+    launches = mp.minipic_launch_count() - launches0
+    total_s = t_start.elapsed_time(t_end) * 1e-3
+    agg = dist.aggregate(tokens_per_step * args.steps, total_s)
+    seg = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(4)] for e in evs])   # ms: write5, prefill, write4, decode
+    seg_mean = seg.mean(axis=0)
+
+    # ---- roofline of the dominant kernel (prefill attention, tensor-bound on config 5)
+    flops5 = w5.attention_flops()
+    prefill_s = seg_mean[1] * 1e-3
+    tf = flops5 / prefill_s / 1e12
+    traffic = load_traffic()
+    roofline = {"kernel": variant5, "bound": "tensor", "achieved": tf, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
+                "frac": tf / peaks["bf16_tflops"], "traffic": traffic.get("prefill_dram_bytes_per_launch"),
+                "peak_source": peaks["source"] + " (bf16 burst)", "frac_of_nominal_2250": tf / 2250.0,
+                "algorithmic_flops_per_launch": flops5, "ms_per_launch": seg_mean[1]}
+    kvb4 = w4.logical_kv_bytes()
+    dec_gbs = kvb4 / (seg_mean[3] * 1e-3) / 1e9
+    roofline_decode = {"kernel": variant4 + " + lse_merge", "bound": "hbm", "achieved": dec_gbs, "peak": peaks["hbm_gbs"],
+                       "unit": "GB/s", "frac": dec_gbs / peaks["hbm_gbs"], "traffic": traffic.get("decode_dram_bytes_per_launch"),
+                       "peak_source": peaks["source"], "frac_of_nominal_8000": dec_gbs / 8000.0,
+                       "algorithmic_bytes_per_launch": kvb4, "ms_per_launch": seg_mean[3],
+                       "note": "logical KV bytes; the 134 MB shared pool is ~L2-sized, see extras.c4_private_pool"}
+    wbytes5 = 2 * w5.written_tokens() * w5.num_kv_heads * w5.head_dim * 2 * w5.itemsize
+    cw_gbs = wbytes5 / (seg_mean[0] * 1e-3) / 1e9
+    roofline_cache_write = {"kernel": "cache_write_kernel", "bound": "hbm", "achieved": cw_gbs, "peak": peaks["hbm_gbs"],
+                            "unit": "GB/s", "frac": cw_gbs / peaks["hbm_gbs"], "algorithmic_bytes_per_launch": wbytes5,
+                            "ms_per_launch": seg_mean[0], "traffic": traffic.get("cache_write_dram_bytes_per_launch")}
+
+    line = {"metric": METRIC, "value": agg["throughput"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": max(args.warmup, 3), "ms_per_step": agg["seconds"] / args.steps * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
+                       "l2": "inputs larger than L2: each step touches ~3.5 GB (Q/O 2.2 GB) between repeats of any kernel",
+                       "rope": "cos/sin table lookup (PAPER.md:113), in-kernel K and Q rotation",
+                       "tokens_per_step": tokens_per_step},
+            "roofline": roofline, "roofline_decode": roofline_decode, "roofline_cache_write": roofline_cache_write,
+            "kernels_ms": {"c5_cache_write": seg_mean[0], "c5_prefill": seg_mean[1], "c4_cache_write": seg_mean[2],
+                           "c4_decode+merge": seg_mean[3]},
+            "prefill_tokens_per_s": w5.num_q_tokens / prefill_s,
+            "gpu_launches": int(launches), "clocks": sampler.summary()}
+
+    # ---- e2e through the host-buffer C entry points (rank-local, then aggregated the same way)
+    h5, h4 = HostStep(d5), HostStep(d4)
+    def e2e_step():
+        h5.run(); h4.run()
+    e2e_step(); torch.cuda.synchronize()
+    n_e2e = 3
+    dist.barrier(); torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(n_e2e):
+        e2e_step()
+    b.record(); torch.cuda.synchronize(); dist.barrier()
+    e2e = dist.aggregate(tokens_per_step * n_e2e, a.elapsed_time(b) * 1e-3)
+    line["e2e"] = {"value": e2e["throughput"], "unit": UNIT, "h2d_bytes_per_step": int(h5.h2d_bytes + h4.h2d_bytes),
+                   "d2h_bytes_per_step": int(h5.d2h_bytes + h4.d2h_bytes), "ms_per_step": e2e["seconds"] / n_e2e * 1e3,
+                   "steps": n_e2e, "api": "minipic_prefill_step_host + minipic_decode_step_host (pinned host buffers)"}
+    del h5, h4
+
+    # ---- extras: other BASELINE configs, controls (rank 0, single GPU only; bounded)
+    if rank == 0 and world == 1 and not args.no_extras:
+        extras = {}
+        try:
+            # in-kernel RoPE overhead: same kernel with MINIPIC_K_PREROTATED (timing only: values irrelevant)
+            t_rope = time_calls(d5.attention, 10, 2, torch)
+            d5.set_flags(mp.MINIPIC_K_PREROTATED)
+            t_pre = time_calls(d5.attention, 10, 2, torch)
+            d5.set_flags(0)
+            extras["c5_rope_overhead"] = {"ms_rope": t_rope[0], "ms_prerotated": t_pre[0], "overhead": t_rope[0] / t_pre[0] - 1.0}
+            t_rope = time_calls(d4.attention, 10, 2, torch)
+            d4.set_flags(mp.MINIPIC_K_PREROTATED)
+            t_pre = time_calls(d4.attention, 10, 2, torch)
+            d4.set_flags(0)
+            extras["c4_rope_overhead"] = {"ms_rope": t_rope[0], "ms_prerotated": t_pre[0], "overhead": t_rope[0] / t_pre[0] - 1.0}
+            flush = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device=dev)
+            for name, mk in (("c2", W.config2), ("c3", W.config3)):
+                w = mk()
+                dw = DeviceWorkload(w, device=dev, rope_table_positions=w.max_kv_len)
+                def f():
+                    flush.zero_()
+                    dw.attention()
+                def g():
+                    flush.zero_()
+                both = time_calls(f, 20, 3, torch)[0]
+                only = time_calls(g, 20, 3, torch)[0]
+                warm = time_calls(dw.attention, 50, 5, torch)
+                fl = w.attention_flops()
+                extras[name] = {"ms_cold_l2": max(both - only, 1e-6), "ms_warm_l2": warm[0], "ms_best": warm[1],
+                                "tokens_per_s_warm": w.num_q_tokens / (warm[0] * 1e-3),
+                                "tflops_warm": fl / (warm[0] * 1e-3) / 1e12, "variant": mp.minipic_last_variant()}
+                del dw
+            wp = W.config4(private_pool=True)
+            dp = DeviceWorkload(wp, device=dev, rope_table_positions=wp.max_kv_len)
+            dp.step(); torch.cuda.synchronize()
+            tp = time_calls(dp.attention, 20, 3, torch)
+            gb = wp.logical_kv_bytes() / (tp[0] * 1e-3) / 1e9
+            extras["c4_private_pool"] = {"ms": tp[0], "ms_best": tp[1], "kv_gbs": gb, "frac_hbm_measured": gb / peaks["hbm_gbs"],
+                                         "resident_kv_bytes": wp.logical_kv_bytes()}
+            del dp, flush
+        except Exception as e:  # extras never break the contract line
+            extras["error"] = repr(e)
+        line["extras"] = extras
+
+    # ---- CPU oracle baseline (rank 0, N = 1 only)
+    if rank == 0 and world == 1:
+        est, desc, sec = oracle_sample_time(w5, w4)
+        line["cpu_baseline"] = {"value": tokens_per_step / est, "unit": UNIT, "cores": host_threads(), "kind": "oracle",
+                                "sample": desc, "sample_seconds": sec}
+    if rank == 0:
+        print(json.dumps(line), flush=True)
+    dist.shutdown()
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-extras", action="store_true")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -209,8 +209,9 @@ def prefill_attention(*, q, k_cache, v_cache, block_tables, cu_q_lens, kv_lens, 
                 qr = round_to_dtype(qr, dtype)
             for c0 in range(0, sel.size, row_chunk):
                 c1 = min(c0 + row_chunk, sel.size)
-                hi = int(idx[c0:c1].max()) + 1
-                o, l = _attend_rows(qr[c0:c1], kk[:hi], vv[:hi], idx[c0:c1], lo[c0:c1], scale)  # steps 5-6
+                # keys outside [min vis_lo, max idx] of the chunk are invisible to every row of it
+                klo, hi = max(int(lo[c0:c1].min()), 0), int(idx[c0:c1].max()) + 1
+                o, l = _attend_rows(qr[c0:c1], kk[klo:hi], vv[klo:hi], idx[c0:c1] - klo, lo[c0:c1] - klo, scale)  # steps 5-6
                 out[sel[c0:c1], h, :] = o
                 lse[sel[c0:c1], h] = l
     return out, lse
