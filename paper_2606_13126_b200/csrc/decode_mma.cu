@@ -31,21 +31,18 @@ __device__ __forceinline__ void mma16816(float (&d)[4], unsigned a0, unsigned a1
       : "r"(a0), "r"(a1), "r"(a2), "r"(a3), "r"(b0), "r"(b1));
 }
 
-// cos/sin of 8 consecutive frequencies i0..i0+7 at position p
-__device__ __forceinline__ void rope_cs8(const RopeParams& rp, int p, int i0, float (&c)[8], float (&s)[8]) {
-  if (p < rp.table_len) {
-    const float4* t = reinterpret_cast<const float4*>(rp.table + (size_t)p * rp.half + i0);
+// cos/sin of 8 consecutive frequencies i0..i0+7 at position p, computed in registers: exact 64-bit fixed-point phase
+// (common.cuh) -> signed half-turns -> MUFU sin/cos on the reduced angle in [-pi, pi) (|err| < 1e-6, far below the
+// bf16 rounding of the rotated operand).  No memory traffic: in this HBM-bound kernel a cos/sin table lookup
+// costs as many L1 wavefronts as the KV stream itself (ncu: l1tex 92% with the table, profiles/).
+__device__ __forceinline__ void rope_cs8(const unsigned long long* __restrict__ finc, int p, int i0, float (&c)[8],
+                                         float (&s)[8]) {
 #pragma unroll
-    for (int e = 0; e < 4; ++e) {
-      const float4 v = __ldg(t + e);
-      c[2 * e] = v.x; s[2 * e] = v.y; c[2 * e + 1] = v.z; s[2 * e + 1] = v.w;
-    }
-  } else {
-#pragma unroll
-    for (int e = 0; e < 8; ++e) {
-      const float2 v = rope_cs_fast(rp, p, i0 + e);
-      c[e] = v.x; s[e] = v.y;
-    }
+  for (int e = 0; e < 8; ++e) {
+    const unsigned long long ph = (unsigned long long)(unsigned)p * finc[i0 + e];
+    const float a = (float)(int)(ph >> 32) * 1.4629180792671596e-9f;  // * pi * 2^-31 -> radians in [-pi, pi)
+    c[e] = __cosf(a);
+    s[e] = __sinf(a);
   }
 }
 
@@ -68,6 +65,9 @@ __global__ void __launch_bounds__(256, 2)
 decode_mma_kernel(DecodeArgs a, int hq, int hkv, int group, float scale_log2, RopeParams rp, unsigned flags,
                   int split_len, int max_splits, float* __restrict__ o_part, float* __restrict__ lse_part) {
   constexpr int D = 128;
+  __shared__ unsigned long long finc[64];  // F_i: 64-bit fixed-point phase increments (turns per position)
+  if (threadIdx.x < 64) finc[threadIdx.x] = rp.phase_inc[threadIdx.x];
+  __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int g = lane >> 2, q4 = lane & 3;
   const int s = blockIdx.x, r = blockIdx.y;
@@ -94,7 +94,7 @@ decode_mma_kernel(DecodeArgs a, int hq, int hkv, int group, float scale_log2, Ro
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
           float c[8], sn[8];
-          rope_cs8(rp, qpos, (q4 + 4 * j) * 8, c, sn);
+          rope_cs8(finc, qpos, (q4 + 4 * j) * 8, c, sn);
           rotate_chunks(ch[j], ch[j + 2], c, sn);
         }
       }
@@ -134,7 +134,7 @@ decode_mma_kernel(DecodeArgs a, int hq, int hkv, int group, float scale_log2, Ro
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
           float c[8], sn[8];
-          rope_cs8(rp, p, (q4 + 4 * j) * 8, c, sn);
+          rope_cs8(finc, p, (q4 + 4 * j) * 8, c, sn);
           rotate_chunks(kr[t][j], kr[t][j + 2], c, sn);
         }
       }
