@@ -54,6 +54,10 @@ static void make_ctx(const minipic_config* cfg, void* stream, Ctx* c) {
   c->scale = cfg->softmax_scale > 0.f ? cfg->softmax_scale : (float)(1.0 / std::sqrt((double)cfg->head_dim));
   c->scale_log2 = (float)((double)c->scale * 1.4426950408889634);
   make_rope(cfg, &c->rope);
+  for (int i = 0; i < 64; ++i) {
+    const double f = i < cfg->head_dim / 2 ? std::pow(cfg->rope_theta, -2.0 * (double)i / (double)cfg->head_dim) : 0.0;
+    c->rope_step_cos[i] = std::cos(f); c->rope_step_sin[i] = std::sin(f);
+  }
   c->stream = (cudaStream_t)stream;
 }
 

@@ -75,6 +75,7 @@ struct Ctx {  // what every launcher needs, derived once from minipic_config
   float scale_log2;  // scale * log2(e)
   unsigned flags;
   RopeParams rope;
+  double rope_step_cos[64], rope_step_sin[64];  // cos / sin of f_i: the one-position RoPE step (prefill recurrence)
   cudaStream_t stream;
 };
 

@@ -1,22 +1,26 @@
 // a2-a9: fused RoPE-in-attention prefill for sm_100a (bf16, head_dim 128, GQA group 1/2/4/8).
 //
-// Work item = (Q tile, KV head).  A Q tile is up to 128/G consecutive query tokens of one request that share
-// vis_lo (one span, or suffix rows); its 128 MMA rows are (token, head-in-group) pairs, so one rotated K tile
-// serves the whole GQA group.  A tiny plan kernel (a2) cuts the query rows into tiles, computes each tile's KV
-// range [floor16(vis_lo), idx_last] (span-mask TILE SKIPPING: keys outside it are never touched) and sorts the
-// tiles longest-first; a persistent kernel (one CTA per SM, 10 warps) then runs, per KV tile of 128 keys:
+// Work item = (Q super-tile, KV head).  A super-tile is up to 2 * (128/G) consecutive query tokens of one request
+// that share vis_lo (one span, or suffix rows); it is processed as TWO 128-row MMA tiles, A and B, whose rows are
+// (token, head-in-group) pairs, so one gathered + rotated K tile serves 256 score rows (the whole GQA group of up
+// to 2*128/G tokens).  Plan kernels (a2) cut the query rows into super-tiles, compute each one's KV range
+// [floor16(vis_lo), idx_last] (span-mask TILE SKIPPING: keys outside it are never touched) and sort the tiles
+// longest-first; a persistent kernel (one CTA per SM, 16 warps) pulls items from an atomic counter and runs, per
+// KV tile of 128 keys:
 //
-//   warp 8     TMA producer : gathers the tile's 8 physical blocks through the block table with
-//                             cp.async.bulk.tensor (SWIZZLE_128B boxes of 16 keys x 64 dims) into smem  (a4)
-//   warps 4-7  rotation     : Q load + RoPE once per item (a3); K tile RoPE in place, smem -> registers -> smem,
-//                             one key per thread, cos/sin by table lookup or in-register phase (a5)
-//   warp 9     MMA issuer   : tcgen05.mma S = Q' K'^T into TMEM (double-buffered), O += P V              (a6, a8)
-//   warps 0-3  softmax      : tcgen05.ld S (one row per thread - no shuffles needed), mask, online softmax with
-//                             lazy rescale, P -> bf16 -> smem; epilogue O / l -> out, LSE                 (a7, a9)
+//   warp 12      TMA producer  : scheduler ring; Q super-tile (3-D box) and the KV tile's 8 physical blocks through
+//                                the block table with cp.async.bulk.tensor (SWIZZLE_128B boxes) into smem       (a4)
+//   warps 8-11   rotation      : in-place RoPE of the Q tiles (a3) and of every K tile (a5): smem -> registers ->
+//                                smem; a lane owns two frequencies and walks the keys of a 16-token block, cos/sin
+//                                restarted exactly (64-bit fixed-point phase + MUFU) at every block / position jump
+//                                and advanced by the angle-addition recurrence in between (packed f32x2 FMAs)
+//   warp 13      MMA issuer    : tcgen05.mma S_X = Q_X K'^T (smem x smem -> TMEM), O_X += P_X V (TMEM x smem -> TMEM),
+//                                X in {A, B} ping-pong so the tensor pipe runs while the other tile is in softmax (a6, a8)
+//   warps 0-3 / 4-7 softmax A/B: tcgen05.ld S (one row per thread), mask, online softmax with lazy rescale of O,
+//                                P -> bf16 -> TMEM (aliasing S); epilogue O / l -> out, LSE                  (a7, a9)
 //
 // All hand-offs are mbarriers; generic-proxy smem writes are fenced with fence.proxy.async before the MMA reads.
 #include <cuda.h>
-#include <cstdio>
 
 #include "internal.h"
 
@@ -25,13 +29,16 @@ namespace minipic {
 namespace {
 
 constexpr int BM = 128, BN = 128, D = 128;
-constexpr int kTileBytes = BN * D * 2;       // 32 KB: one K / V / Q / P tile
-constexpr int kHalfBytes = kTileBytes / 2;   // [half of head_dim or keys][128 rows][128 B]
-constexpr int kThreads = 320;
+constexpr int kTileBytes = BN * D * 2;       // 32 KB: one K / V / Q tile
+constexpr int kHalfBytes = kTileBytes / 2;   // [half of head_dim][128 rows][128 B]
+constexpr int kKStages = 3, kVStages = 2, kRing = 4;
+constexpr int kThreads = 512;
 constexpr int kMaxBins = 4096;
+constexpr long long kWaitTimeoutCycles = 4000000000LL;
 
-struct TileDesc { int t0, ntok, r, idx0, lo, n_kv; };
-struct PlanHeader { int n_tiles; int next_item; int pad[62]; };
+struct TileDesc { int t0, ntok, r, idx0, lo, n_kv, kv_hi, kv_len; };
+struct PlanHeader { int n_tiles; int next_item; int err; int err_info[5]; int pad[56]; int hist[kMaxBins]; };
+struct ItemInfo { int t0, ntok, r, idx0, lo, kvh, n_kv, kv_hi, kv_len, pad[3]; };   // 48 B ring entry; t0 < 0 = stop
 
 // ------------------------------------------------------------------------------------------------ PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -44,23 +51,40 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
-  uint32_t done = 0;
-  unsigned long long spins = 0;
-  while (true) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
-        "selp.u32 %0, 1, 0, p;\n\t}"
-        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
-    if (done) break;
-    if (++spins > (1ull << 24)) {  // watchdog: a protocol bug must fault, not hang the GPU
-      printf("minipic prefill: mbarrier wait timed out (block %d thread %d bar %u parity %u)\n", blockIdx.x, threadIdx.x,
-             bar, parity);
-      __trap();
+__device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity) {
+  uint32_t done;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+  return done != 0;
+}
+// A protocol bug must neither hang the GPU nor kill the context: a wait that exceeds the timeout records
+// (barrier, parity, block, thread) in the plan header, and every thread that sees the flag stops waiting, so the
+// kernel drains and the host can read the error word (prefill_sm100_status()).
+struct Waiter {
+  int* err;
+  bool dead;
+  __device__ __forceinline__ void wait(uint32_t bar, uint32_t parity) {
+    if (dead) return;
+    if (mbar_try(bar, parity)) return;
+    const long long t0 = clock64();
+    unsigned spins = 0;
+    while (!mbar_try(bar, parity)) {
+      if ((++spins & 63u) == 0) {
+        if (*(volatile int*)err != 0) { dead = true; return; }
+        if (clock64() - t0 > kWaitTimeoutCycles) {
+          if (atomicCAS(err, 0, 1) == 0) {
+            err[1] = (int)bar; err[2] = (int)parity; err[3] = (int)blockIdx.x; err[4] = (int)threadIdx.x;
+          }
+          dead = true;
+          return;
+        }
+      }
     }
   }
-}
+};
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -72,11 +96,24 @@ __device__ __forceinline__ void tma_load_2d(uint32_t dst, const CUtensorMap* tma
       "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4}], [%2];"
       ::"r"(dst), "l"(tmap), "r"(bar), "r"(x), "r"(y) : "memory");
 }
-__device__ __forceinline__ void umma_bf16(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+__device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tmap, uint32_t bar, int x, int y, int z) {
+  asm volatile(
+      "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
+      ::"r"(dst), "l"(tmap), "r"(bar), "r"(x), "r"(y), "r"(z) : "memory");
+}
+// D[tmem] (+)= A[smem] * B[smem]
+__device__ __forceinline__ void umma_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
   asm volatile(
       "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
       "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
       ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+}
+// D[tmem] (+)= A[tmem] * B[smem]
+__device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+  asm volatile(
+      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
 }
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
   uint32_t* r = reinterpret_cast<uint32_t*>(v);
@@ -89,8 +126,7 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
         "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
       : "r"(taddr));
 }
-__device__ __forceinline__ void tmem_st32(uint32_t taddr, const float* v) {
-  const uint32_t* r = reinterpret_cast<const uint32_t*>(v);
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
   asm volatile(
       "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,"
       "%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
@@ -100,13 +136,46 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const float* v) {
         "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
       : "memory");
 }
+__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ float fast_exp2(float x) {
   float y;
   asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
   return y;
 }
-__device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
-__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+__device__ __forceinline__ float max3(float a, float b, float c) {
+  float d;
+  asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
+  return d;
+}
+// packed fp32 pairs (one 64-bit register = two lanes of an FFMA2)
+__device__ __forceinline__ uint64_t pk2(float a, float b) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+  return r;
+}
+__device__ __forceinline__ void upk2(uint64_t v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ uint32_t lds32(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared.b32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ void sts32(uint32_t addr, uint32_t v) { asm volatile("st.shared.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory"); }
+__device__ __forceinline__ void sts128z(uint32_t addr) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(addr), "r"(0) : "memory");
+}
+template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
+template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 
 // shared-memory matrix descriptor (SWIZZLE_128B, version 1): start address, leading / stride byte offsets
 __device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
@@ -118,40 +187,6 @@ __host__ __device__ constexpr uint32_t instr_desc(bool b_mn) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn ? 1u : 0u) << 16) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
 }
 
-// byte offset of 16-byte chunk `c` (0..15) of row `r` inside a [2][128 rows][128 B] SWIZZLE_128B tile
-__device__ __forceinline__ uint32_t tile_off(int r, int c) {
-  return (uint32_t)((c >> 3) * kHalfBytes + r * 128 + (((c & 7) ^ (r & 7)) << 4));
-}
-
-__device__ __forceinline__ void cs8(const RopeParams& rp, const unsigned long long* finc, int p, int i0, float (&c)[8],
-                                    float (&s)[8]) {
-  if (p < rp.table_len) {  // PAPER.md:113 "a cos/sin table lookup"
-    const float4* t = reinterpret_cast<const float4*>(rp.table + (size_t)p * rp.half + i0);
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
-      const float4 v = __ldg(t + e);
-      c[2 * e] = v.x; s[2 * e] = v.y; c[2 * e + 1] = v.z; s[2 * e + 1] = v.w;
-    }
-  } else {
-#pragma unroll
-    for (int e = 0; e < 8; ++e) {
-      const unsigned long long ph = (unsigned long long)(unsigned)p * finc[i0 + e];
-      const float a = (float)(int)(ph >> 32) * 1.4629180792671596e-9f;
-      c[e] = __cosf(a); s[e] = __sinf(a);
-    }
-  }
-}
-__device__ __forceinline__ void rotate16(uint4& lo, uint4& hi, const float (&c)[8], const float (&s)[8]) {
-  unsigned* l = reinterpret_cast<unsigned*>(&lo);
-  unsigned* h = reinterpret_cast<unsigned*>(&hi);
-#pragma unroll
-  for (int w = 0; w < 4; ++w) {
-    const float a0 = bf16lo(l[w]), a1 = bf16hi(l[w]), b0 = bf16lo(h[w]), b1 = bf16hi(h[w]);
-    l[w] = pack_bf16(a0 * c[2 * w] - b0 * s[2 * w], a1 * c[2 * w + 1] - b1 * s[2 * w + 1]);
-    h[w] = pack_bf16(b0 * c[2 * w] + a0 * s[2 * w], b1 * c[2 * w + 1] + a1 * s[2 * w + 1]);
-  }
-}
-
 // ------------------------------------------------------------------------------------------------ a2: plan
 __device__ __forceinline__ bool tile_starts(const PrefillArgs& a, int t, int r, int tok) {
   if (t == __ldg(a.cu_q_lens + r)) return true;
@@ -160,106 +195,171 @@ __device__ __forceinline__ bool tile_starts(const PrefillArgs& a, int t, int r, 
   return i1 != i0 + 1 || l1 != l0 || ((i1 - max(l1, 0)) % tok) == 0;
 }
 
-__global__ void __launch_bounds__(1024) prefill_plan_kernel(PrefillArgs a, int tok, PlanHeader* hdr, TileDesc* sorted,
-                                                            TileDesc* tmp) {
-  __shared__ int hist[kMaxBins];
-  __shared__ int n_tiles_s;
-  for (int i = threadIdx.x; i < kMaxBins; i += blockDim.x) hist[i] = 0;
-  if (threadIdx.x == 0) n_tiles_s = 0;
-  __syncthreads();
-  for (int t = threadIdx.x; t < a.num_q_tokens; t += blockDim.x) {
-    int lo_r = 0, hi_r = a.num_reqs;
-    while (hi_r - lo_r > 1) {
-      const int mid = (lo_r + hi_r) >> 1;
-      if (__ldg(a.cu_q_lens + mid) <= t) lo_r = mid; else hi_r = mid;
-    }
-    const int r = lo_r;
-    if (!tile_starts(a, t, r, tok)) continue;
-    const int t_end = __ldg(a.cu_q_lens + r + 1);
-    int n = 1;
-    while (n < tok && t + n < t_end && !tile_starts(a, t + n, r, tok)) ++n;
-    TileDesc td;
-    td.t0 = t; td.ntok = n; td.r = r; td.idx0 = __ldg(a.q_seq_idx + t); td.lo = max(__ldg(a.q_vis_lo + t), 0);
-    const int kv_lo = td.lo & ~(kBlock - 1), kv_hi = min(td.idx0 + n, __ldg(a.kv_lens + r));
-    td.n_kv = kv_hi > kv_lo ? (kv_hi - kv_lo + BN - 1) / BN : 0;
-    const int slot = atomicAdd(&n_tiles_s, 1);
-    tmp[slot] = td;
-    atomicAdd(&hist[min(td.n_kv, kMaxBins - 1)], 1);
+// one thread per query token: the tokens that start a super-tile emit its descriptor and count it in the cost histogram
+__global__ void __launch_bounds__(256) plan_mark_kernel(PrefillArgs a, int tok, PlanHeader* hdr, TileDesc* tmp) {
+  const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= a.num_q_tokens) return;
+  int lo_r = 0, hi_r = a.num_reqs;
+  while (hi_r - lo_r > 1) {
+    const int mid = (lo_r + hi_r) >> 1;
+    if (__ldg(a.cu_q_lens + mid) <= t) lo_r = mid; else hi_r = mid;
   }
-  __syncthreads();
-  // exclusive prefix over bins in DESCENDING cost order (longest-first), one warp
-  if (threadIdx.x < 32) {
-    int carry = 0;
-    for (int base = kMaxBins - 32; base >= 0; base -= 32) {
-      const int b = base + 31 - threadIdx.x;  // lane 0 takes the most expensive bin of the chunk
-      const int v = hist[b];
-      int incl = v;
+  const int r = lo_r;
+  if (!tile_starts(a, t, r, tok)) return;
+  const int t_end = __ldg(a.cu_q_lens + r + 1);
+  int n = 1;
+  while (n < tok && t + n < t_end && !tile_starts(a, t + n, r, tok)) ++n;
+  TileDesc td;
+  td.t0 = t; td.ntok = n; td.r = r; td.idx0 = __ldg(a.q_seq_idx + t); td.lo = max(__ldg(a.q_vis_lo + t), 0);
+  td.kv_len = __ldg(a.kv_lens + r);
+  const int kv_lo = td.lo & ~(kBlock - 1);
+  td.kv_hi = min(td.idx0 + n, td.kv_len);
+  td.n_kv = td.kv_hi > kv_lo ? (td.kv_hi - kv_lo + BN - 1) / BN : 0;
+  tmp[atomicAdd(&hdr->n_tiles, 1)] = td;
+  atomicAdd(&hdr->hist[min(td.n_kv, kMaxBins - 1)], 1);
+}
+// exclusive prefix over the cost bins in DESCENDING order (longest-first): thread t owns ranks [4t, 4t+4), rank = kMaxBins-1-bin
+__global__ void __launch_bounds__(1024) plan_scan_kernel(PlanHeader* hdr) {
+  __shared__ int wsum[32];
+  const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
+  int v[4], tot = 0;
 #pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const int n = __shfl_up_sync(0xffffffffu, incl, o);
-        if ((int)threadIdx.x >= o) incl += n;
-      }
-      hist[b] = carry + incl - v;
-      carry += __shfl_sync(0xffffffffu, incl, 31);
+  for (int e = 0; e < 4; ++e) { v[e] = hdr->hist[kMaxBins - 1 - (4 * t + e)]; tot += v[e]; }
+  int incl = tot;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const int n = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += n;
+  }
+  if (lane == 31) wsum[wid] = incl;
+  __syncthreads();
+  if (wid == 0) {
+    const int w = wsum[lane];
+    int wi = w;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const int n = __shfl_up_sync(0xffffffffu, wi, o);
+      if (lane >= o) wi += n;
     }
+    wsum[lane] = wi - w;
   }
   __syncthreads();
-  const int n_tiles = n_tiles_s;
-  for (int i = threadIdx.x; i < n_tiles; i += blockDim.x) {
-    const TileDesc td = tmp[i];
-    sorted[atomicAdd(&hist[min(td.n_kv, kMaxBins - 1)], 1)] = td;
-  }
-  if (threadIdx.x == 0) { hdr->n_tiles = n_tiles; hdr->next_item = 0; }
+  int base = wsum[wid] + incl - tot;
+#pragma unroll
+  for (int e = 0; e < 4; ++e) { hdr->hist[kMaxBins - 1 - (4 * t + e)] = base; base += v[e]; }
+}
+__global__ void __launch_bounds__(256) plan_scatter_kernel(PlanHeader* hdr, const TileDesc* tmp, TileDesc* sorted) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= hdr->n_tiles) return;
+  const TileDesc td = tmp[i];
+  sorted[atomicAdd(&hdr->hist[min(td.n_kv, kMaxBins - 1)], 1)] = td;
 }
 
 // ------------------------------------------------------------------------------------------------ main kernel
 struct Smem {
-  alignas(1024) unsigned char q[kTileBytes];
-  alignas(1024) unsigned char k[2][kTileBytes];
-  alignas(1024) unsigned char v[2][kTileBytes];
-  alignas(1024) unsigned char p[kTileBytes];
-  unsigned long long finc[64];
-  unsigned long long bars[32];
+  alignas(1024) unsigned char q[2][kTileBytes];
+  alignas(1024) unsigned char k[kKStages][kTileBytes];
+  alignas(1024) unsigned char v[kVStages][kTileBytes];
+  unsigned long long bars[40];
+  ItemInfo ring[kRing];
   uint32_t tmem_base;
 };
-enum Bar { Q_FULL = 0, Q_EMPTY, K_FULL, K_READY = K_FULL + 2, K_EMPTY = K_READY + 2, V_FULL = K_EMPTY + 2,
-           V_READY = V_FULL + 2, V_EMPTY = V_READY + 2, S_FULL = V_EMPTY + 2, S_EMPTY = S_FULL + 2, P_FULL = S_EMPTY + 2,
-           PV_DONE, O_FREE, NUM_BARS };
+enum Bar {
+  SCHED_FULL = 0, SCHED_EMPTY = SCHED_FULL + kRing,
+  Q_FULL = SCHED_EMPTY + kRing, Q_READY, Q_EMPTY,
+  K_FULL, K_READY = K_FULL + kKStages, K_EMPTY = K_READY + kKStages,
+  V_FULL = K_EMPTY + kKStages, V_EMPTY = V_FULL + kVStages, V_FIX = V_EMPTY + kVStages,
+  S_FULL, P_FULL = S_FULL + 2, O_FULL = P_FULL + 2, O_FREE = O_FULL + 2, NUM_BARS = O_FREE + 2
+};
+static_assert(NUM_BARS <= 40, "barrier array too small");
+static_assert(sizeof(Smem) <= 232448, "shared memory budget");
 
 struct Params {
   PrefillArgs a;
   int hq, hkv;
   float scale_log2;
   unsigned flags;
-  const PlanHeader* hdr;
+  PlanHeader* hdr;
   const TileDesc* tiles;
-  RopeParams rp;
+  int oob_row;                       // first row beyond the cache tensor map: TMA zero-fills
+  unsigned long long phase_inc[64];  // F_i (common.cuh)
+  float2 step[64];                   // (cos f_i, sin f_i): one-position RoPE step
+};
+
+struct Item {
+  int t0, ntok, r, idx0, lo, kvh, n_kv, kv_hi, kv_len;
+  int kv_lo, ntok_x[2], n_x[2];
+};
+template <int TOK>
+__device__ __forceinline__ Item load_item(const ItemInfo& ii) {
+  Item it;
+  it.t0 = ii.t0; it.ntok = ii.ntok; it.r = ii.r; it.idx0 = ii.idx0; it.lo = ii.lo; it.kvh = ii.kvh; it.n_kv = ii.n_kv;
+  it.kv_hi = ii.kv_hi; it.kv_len = ii.kv_len;
+  it.kv_lo = it.lo & ~(kBlock - 1);
+  it.ntok_x[0] = min(it.ntok, TOK); it.ntok_x[1] = it.ntok - it.ntok_x[0];
+  const int hi_a = min(it.idx0 + it.ntok_x[0], it.kv_len);
+  it.n_x[0] = hi_a > it.kv_lo ? (hi_a - it.kv_lo + BN - 1) / BN : 0;
+  it.n_x[1] = it.ntok_x[1] > 0 ? it.n_kv : 0;
+  return it;
+}
+
+// RoPE state of one lane: two adjacent frequencies (2*lane, 2*lane+1), cos / sin packed as f32x2
+struct Rot {
+  unsigned long long f0, f1;   // fixed-point phase increments
+  uint64_t c1, s1, ns1;        // one-position step (cos, sin, -sin)
+  uint64_t c, s;
+  __device__ __forceinline__ void restart(int p) {
+    const unsigned long long p0 = (unsigned long long)(unsigned)p * f0, p1 = (unsigned long long)(unsigned)p * f1;
+    const float a0 = (float)(int)(p0 >> 32) * 1.4629180792671596e-9f;   // * pi * 2^-31
+    const float a1 = (float)(int)(p1 >> 32) * 1.4629180792671596e-9f;
+    c = pk2(__cosf(a0), __cosf(a1));
+    s = pk2(__sinf(a0), __sinf(a1));
+  }
+  __device__ __forceinline__ void advance() {
+    const uint64_t cn = fma2(c, c1, mul2(s, ns1));
+    s = fma2(s, c1, mul2(c, s1));
+    c = cn;
+  }
+  // rotate the lane's 2+2 elements of one 128-dim row: lo word = dims (2l, 2l+1), hi word = dims (64+2l, 64+2l+1)
+  __device__ __forceinline__ void apply(uint32_t addr) const {
+    const uint32_t lo = lds32(addr), hi = lds32(addr + kHalfBytes);
+    const uint64_t a = pk2(bf16lo(lo), bf16hi(lo)), b = pk2(bf16lo(hi), bf16hi(hi));
+    const uint64_t ns = mul2(s, pk2(-1.f, -1.f));
+    const uint64_t an = fma2(a, c, mul2(b, ns));
+    const uint64_t bn = fma2(b, c, mul2(a, s));
+    float x0, x1, y0, y1;
+    upk2(an, x0, x1); upk2(bn, y0, y1);
+    sts32(addr, pack_bf16(x0, x1));
+    sts32(addr + kHalfBytes, pack_bf16(y0, y1));
+  }
 };
 
 template <int G>
 __global__ void __launch_bounds__(kThreads, 1)
-prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v,
-                     const __grid_constant__ Params prm) {
-  extern __shared__ unsigned char smem_raw[];
-  Smem& sm = *reinterpret_cast<Smem*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
+                     const __grid_constant__ CUtensorMap tmap_v, const __grid_constant__ Params prm) {
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
   constexpr int TOK = BM / G;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const PrefillArgs& a = prm.a;
   const uint32_t bar0 = smem_u32(sm.bars);
   auto bar = [&](int b) { return bar0 + 8u * (uint32_t)b; };
+  Waiter w{&prm.hdr->err, false};
 
-  if (threadIdx.x < 64) sm.finc[threadIdx.x] = prm.rp.phase_inc[threadIdx.x];
   if (threadIdx.x == 0) {
-    mbar_init(bar(Q_FULL), 128); mbar_init(bar(Q_EMPTY), 1);
-    for (int s = 0; s < 2; ++s) {
-      mbar_init(bar(K_FULL + s), 1); mbar_init(bar(K_READY + s), 128); mbar_init(bar(K_EMPTY + s), 1);
-      mbar_init(bar(V_FULL + s), 1); mbar_init(bar(V_READY + s), 128); mbar_init(bar(V_EMPTY + s), 1);
-      mbar_init(bar(S_FULL + s), 1); mbar_init(bar(S_EMPTY + s), 128);
+    if (smem_u32(smem_raw) & 1023u) atomicCAS(&prm.hdr->err, 0, 2);   // swizzled tiles need a 1024-byte aligned base
+    for (int s = 0; s < kRing; ++s) { mbar_init(bar(SCHED_FULL + s), 1); mbar_init(bar(SCHED_EMPTY + s), 13); }
+    mbar_init(bar(Q_FULL), 1); mbar_init(bar(Q_READY), 128); mbar_init(bar(Q_EMPTY), 1);
+    for (int s = 0; s < kKStages; ++s) { mbar_init(bar(K_FULL + s), 1); mbar_init(bar(K_READY + s), 128); mbar_init(bar(K_EMPTY + s), 1); }
+    for (int s = 0; s < kVStages; ++s) { mbar_init(bar(V_FULL + s), 1); mbar_init(bar(V_EMPTY + s), 1); }
+    mbar_init(bar(V_FIX), 128);
+    for (int x = 0; x < 2; ++x) {
+      mbar_init(bar(S_FULL + x), 1); mbar_init(bar(P_FULL + x), 128); mbar_init(bar(O_FULL + x), 1); mbar_init(bar(O_FREE + x), 128);
     }
-    mbar_init(bar(P_FULL), 128); mbar_init(bar(PV_DONE), 1); mbar_init(bar(O_FREE), 128);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 9) {  // TMEM: 512 columns (S0, S1, O at 0, 128, 256)
+  if (warp == 13) {  // TMEM: 512 columns = S_A | S_B | O_A | O_B, 128 each; P_X aliases the first 64 columns of S_X
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&sm.tmem_base)), "r"(512));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::);
   }
@@ -267,266 +367,342 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_co
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = sm.tmem_base;
+  const int n_items = prm.hdr->n_tiles * prm.hkv;
 
-  const int n_tiles = prm.hdr->n_tiles;
-  const int n_items = n_tiles * prm.hkv;
-  const int nctas = gridDim.x;
-  // static longest-first assignment in snake order: round k gives CTA b item k*nctas + (k odd ? nctas-1-b : b)
-  auto item_of = [&](int k) { return k * nctas + ((k & 1) ? nctas - 1 - (int)blockIdx.x : (int)blockIdx.x); };
-
-  if (warp == 8) {
-    // ============================================================ TMA producer (a4)
-    uint32_t kv_it = 0;
-    for (int k = 0;; ++k) {
-      const int item = item_of(k);
-      if (item >= n_items) break;
-      const TileDesc td = prm.tiles[item / prm.hkv];
-      const int kvh = item % prm.hkv;
-      const int kv_lo = td.lo & ~(kBlock - 1), kv_hi = min(td.idx0 + td.ntok, __ldg(a.kv_lens + td.r));
-      const int* bt = a.block_tables + (size_t)td.r * a.max_blocks;
-      for (int i = 0; i < td.n_kv; ++i, ++kv_it) {
-        const int st = kv_it & 1;
-        const uint32_t par = ((kv_it >> 1) & 1) ^ 1;
-        const int j0 = kv_lo + i * BN;
-        const int nblk = min(BN / kBlock, (kv_hi - j0 + kBlock - 1) / kBlock);
-        int y = 0;
-        if (lane < nblk) y = (__ldg(bt + j0 / kBlock + lane) * prm.hkv + kvh) * kBlock;
-        if (lane == 0) { mbar_wait(bar(K_EMPTY + st), par); mbar_expect_tx(bar(K_FULL + st), nblk * 4096); }
-        __syncwarp();
-        if (lane < nblk) {
-          const uint32_t dst = smem_u32(sm.k[st]) + lane * 2048;
-          tma_load_2d(dst, &tmap_k, bar(K_FULL + st), 0, y);
-          tma_load_2d(dst + kHalfBytes, &tmap_k, bar(K_FULL + st), 64, y);
+  if (warp >= 12) {
+    reg_dec<48>();
+    if (warp == 12) {
+      // ============================================================ scheduler + TMA producer (a4)
+      uint32_t kc = 0, vc = 0, qc = 0;
+      for (uint32_t it_n = 0;; ++it_n) {
+        const int slot = it_n & (kRing - 1);
+        int item = 0;
+        if (lane == 0) {
+          w.wait(bar(SCHED_EMPTY + slot), ((it_n / kRing) & 1) ^ 1);
+          item = w.dead ? n_items : atomicAdd(&prm.hdr->next_item, 1);
         }
-        if (lane == 0) { mbar_wait(bar(V_EMPTY + st), par); mbar_expect_tx(bar(V_FULL + st), nblk * 4096); }
-        __syncwarp();
-        if (lane < nblk) {
-          const uint32_t dst = smem_u32(sm.v[st]) + lane * 2048;
-          tma_load_2d(dst, &tmap_v, bar(V_FULL + st), 0, y);
-          tma_load_2d(dst + kHalfBytes, &tmap_v, bar(V_FULL + st), 64, y);
+        item = __shfl_sync(0xffffffffu, item, 0);
+        if (item >= n_items) {
+          if (lane == 0) { sm.ring[slot].t0 = -1; mbar_arrive(bar(SCHED_FULL + slot)); }
+          break;
+        }
+        const TileDesc td = prm.tiles[item / prm.hkv];
+        const int kvh = item % prm.hkv;
+        if (lane == 0) {
+          ItemInfo& ii = sm.ring[slot];
+          ii.t0 = td.t0; ii.ntok = td.ntok; ii.r = td.r; ii.idx0 = td.idx0; ii.lo = td.lo; ii.kvh = kvh; ii.n_kv = td.n_kv;
+          ii.kv_hi = td.kv_hi; ii.kv_len = td.kv_len;
+          mbar_arrive(bar(SCHED_FULL + slot));
+        }
+        if (td.n_kv == 0) continue;
+        const int kv_lo = td.lo & ~(kBlock - 1);
+        const int nblk_total = (td.kv_hi + kBlock - 1) / kBlock;   // blocks [0, nblk_total) of the request hold visible keys
+        const int* bt = a.block_tables + (size_t)td.r * a.max_blocks;
+        auto block_row = [&](int i) {   // cache-matrix row of this lane's block (lanes 0-7) of KV tile i
+          const int b = (kv_lo >> 4) + i * (BN / kBlock) + lane;
+          return (lane < BN / kBlock && b < nblk_total) ? (__ldg(bt + b) * prm.hkv + kvh) * kBlock : prm.oob_row;
+        };
+        int y = block_row(0);
+        for (int i = 0; i < td.n_kv; ++i) {
+          const int y_next = (i + 1 < td.n_kv) ? block_row(i + 1) : 0;
+          {  // K tile i
+            const int st = kc % kKStages;
+            if (lane == 0) { w.wait(bar(K_EMPTY + st), ((kc / kKStages) & 1) ^ 1); mbar_expect_tx(bar(K_FULL + st), kTileBytes); }
+            __syncwarp();
+            if (lane < BN / kBlock) {
+              const uint32_t dst = smem_u32(sm.k[st]) + lane * 2048;
+              tma_load_2d(dst, &tmap_k, bar(K_FULL + st), 0, y);
+              tma_load_2d(dst + kHalfBytes, &tmap_k, bar(K_FULL + st), 64, y);
+            }
+            ++kc;
+          }
+          if (i == 0) {  // Q super-tile: rows (token, head-in-group), tile A then tile B
+            const int ntile = td.ntok > TOK ? 2 : 1;
+            if (lane == 0) { w.wait(bar(Q_EMPTY), (qc & 1) ^ 1); mbar_expect_tx(bar(Q_FULL), ntile * kTileBytes); }
+            __syncwarp();
+            if (lane < 2 * ntile) {
+              const int x = lane >> 1, h = lane & 1;
+              tma_load_3d(smem_u32(sm.q[x]) + h * kHalfBytes, &tmap_q, bar(Q_FULL), 64 * h, kvh * G, td.t0 + x * TOK);
+            }
+            ++qc;
+          }
+          {  // V tile i
+            const int st = vc % kVStages;
+            if (lane == 0) { w.wait(bar(V_EMPTY + st), ((vc / kVStages) & 1) ^ 1); mbar_expect_tx(bar(V_FULL + st), kTileBytes); }
+            __syncwarp();
+            if (lane < BN / kBlock) {
+              const uint32_t dst = smem_u32(sm.v[st]) + lane * 2048;
+              tma_load_2d(dst, &tmap_v, bar(V_FULL + st), 0, y);
+              tma_load_2d(dst + kHalfBytes, &tmap_v, bar(V_FULL + st), 64, y);
+            }
+            ++vc;
+          }
+          y = y_next;
         }
       }
-    }
-  } else if (warp == 9) {
-    // ============================================================ MMA issuer (a6, a8)
-    const uint32_t idesc_qk = instr_desc(false), idesc_pv = instr_desc(true);
-    const uint32_t q_addr = smem_u32(sm.q), p_addr = smem_u32(sm.p);
-    uint32_t kv_it = 0, s_it = 0, pv_it = 0;
-    int n_used = 0;   // items with at least one KV tile (only those touch the Q / O barriers)
-    for (int k = 0;; ++k) {
-      const int item = item_of(k);
-      if (item >= n_items) break;
-      const TileDesc td = prm.tiles[item / prm.hkv];
-      if (td.n_kv == 0) continue;
-      auto issue_qk = [&](uint32_t kv_i, uint32_t s_i) {
-        const int st = kv_i & 1, sb = s_i & 1;
-        mbar_wait(bar(K_READY + st), (kv_i >> 1) & 1);
-        mbar_wait(bar(S_EMPTY + sb), ((s_i >> 1) & 1) ^ 1);
-        tc_fence_after();
-        if (lane == 0) {
-          const uint32_t k_addr = smem_u32(sm.k[st]);
+    } else if (warp == 13 && lane == 0) {
+      // ============================================================ MMA issuer (a6, a8): one thread
+      const uint32_t idesc_qk = instr_desc(false), idesc_pv = instr_desc(true);
+      uint32_t kc = 0, vc = 0, qc = 0, fixc = 0;
+      uint32_t pc[2] = {0, 0}, oc[2] = {0, 0};
+      for (uint32_t it_n = 0;; ++it_n) {
+        const int slot = it_n & (kRing - 1);
+        w.wait(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
+        if (w.dead || sm.ring[slot].t0 < 0) break;
+        const Item it = load_item<TOK>(sm.ring[slot]);
+        mbar_arrive(bar(SCHED_EMPTY + slot));
+        const int n = it.n_kv;
+        if (n == 0) continue;
+        const bool vfix = (it.kv_hi & (kBlock - 1)) != 0;
+        int k_upto = 0, v_upto = 0;
+        auto need_k = [&](int i) {
+          while (k_upto <= i) { const uint32_t c = kc + k_upto; w.wait(bar(K_READY + c % kKStages), (c / kKStages) & 1); ++k_upto; }
+        };
+        auto need_v = [&](int i) {
+          while (v_upto <= i) {
+            const uint32_t c = vc + v_upto;
+            w.wait(bar(V_FULL + c % kVStages), (c / kVStages) & 1);
+            if (v_upto == n - 1 && vfix) { w.wait(bar(V_FIX), fixc & 1); ++fixc; }
+            ++v_upto;
+          }
+        };
+        auto qk = [&](int x, int i) {
+          const uint32_t q_addr = smem_u32(sm.q[x]), k_addr = smem_u32(sm.k[(kc + i) % kKStages]);
 #pragma unroll
           for (int ks = 0; ks < D / 16; ++ks) {
             const uint32_t off = (ks >> 2) * kHalfBytes + (ks & 3) * 32;
-            umma_bf16(tmem + sb * BN, smem_desc(q_addr + off, 16, 1024), smem_desc(k_addr + off, 16, 1024), idesc_qk, ks > 0);
+            umma_ss(tmem + x * BN, smem_desc(q_addr + off, 16, 1024), smem_desc(k_addr + off, 16, 1024), idesc_qk, ks > 0);
           }
-          tc_commit(bar(S_FULL + sb));
-          tc_commit(bar(K_EMPTY + st));
-        }
-        __syncwarp();
-      };
-      mbar_wait(bar(Q_FULL), n_used & 1);
-      issue_qk(kv_it, s_it);
-      for (int i = 0; i < td.n_kv; ++i) {
-        if (i + 1 < td.n_kv) issue_qk(kv_it + i + 1, s_it + i + 1);
-        if (i == max(td.n_kv - 2, 0) && lane == 0) tc_commit(bar(Q_EMPTY));  // the item's last QK has been issued
-        const int st = (kv_it + i) & 1;
-        mbar_wait(bar(P_FULL), pv_it & 1);
-        mbar_wait(bar(V_READY + st), ((kv_it + i) >> 1) & 1);
-        if (i == 0) mbar_wait(bar(O_FREE), (n_used & 1) ^ 1);
+          tc_commit(bar(S_FULL + x));
+        };
+        auto pv = [&](int x, int i) {
+          const uint32_t v_addr = smem_u32(sm.v[(vc + i) % kVStages]);
+#pragma unroll
+          for (int ks = 0; ks < BN / 16; ++ks)
+            umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, smem_desc(v_addr + ks * 2048, kHalfBytes, 1024), idesc_pv,
+                    (i > 0 || ks > 0));
+        };
+        w.wait(bar(Q_READY), qc & 1);
+        need_k(0);
         tc_fence_after();
-        if (lane == 0) {
-          const uint32_t v_addr = smem_u32(sm.v[st]);
 #pragma unroll
-          for (int ks = 0; ks < BN / 16; ++ks) {
-            const uint32_t aoff = (ks >> 2) * kHalfBytes + (ks & 3) * 32;
-            umma_bf16(tmem + 2 * BN, smem_desc(p_addr + aoff, 16, 1024), smem_desc(v_addr + ks * 2048, kHalfBytes, 1024),
-                      idesc_pv, (i > 0 || ks > 0));
-          }
-          tc_commit(bar(PV_DONE));
-          tc_commit(bar(V_EMPTY + st));
-        }
-        __syncwarp();
-        ++pv_it;
-      }
-      kv_it += td.n_kv; s_it += td.n_kv;
-      ++n_used;
-    }
-  } else if (warp >= 4) {
-    // ============================================================ rotation warps: Q (a3) and K tiles (a5)
-    const int row = threadIdx.x - 128;
-    uint32_t kv_it = 0;
-    int n_used = 0;
-    for (int k = 0;; ++k) {
-      const int item = item_of(k);
-      if (item >= n_items) break;
-      const TileDesc td = prm.tiles[item / prm.hkv];
-      const int kvh = item % prm.hkv;
-      if (td.n_kv == 0) continue;
-      const int* pos = a.kv_positions + __ldg(a.cu_kv_lens + td.r);
-      const int kv_lo = td.lo & ~(kBlock - 1), kv_hi = min(td.idx0 + td.ntok, __ldg(a.kv_lens + td.r));
-      // ---- Q tile: row = token * G + head-in-group
-      mbar_wait(bar(Q_EMPTY), (n_used & 1) ^ 1);
-      {
-        const int tok = row / G, hg = row % G;
-        if (tok < td.ntok) {
-          const __nv_bfloat16* qrow = (const __nv_bfloat16*)a.q + ((size_t)(td.t0 + tok) * prm.hq + kvh * G + hg) * D;
-          const int qpos = __ldg(pos + td.idx0 + tok);
+        for (int x = 0; x < 2; ++x)
+          if (it.n_x[x] > 0) qk(x, 0);
+        tc_commit(bar(K_EMPTY + kc % kKStages));
+        if (n == 1) tc_commit(bar(Q_EMPTY));
+        for (int i = 0; i < n; ++i) {
 #pragma unroll
-          for (int c = 0; c < 8; ++c) {
-            uint4 lo = __ldg(reinterpret_cast<const uint4*>(qrow + 8 * c));
-            uint4 hi = __ldg(reinterpret_cast<const uint4*>(qrow + 64 + 8 * c));
-            if (!(prm.flags & MINIPIC_Q_PREROTATED)) {
-              float cs[8], sn[8];
-              cs8(prm.rp, sm.finc, qpos, 8 * c, cs, sn);
-              rotate16(lo, hi, cs, sn);
+          for (int x = 0; x < 2; ++x) {
+            if (i < it.n_x[x]) {
+              w.wait(bar(P_FULL + x), pc[x] & 1); ++pc[x];
+              need_v(i);
+              if (i == 0) w.wait(bar(O_FREE + x), (oc[x] & 1) ^ 1);
+              tc_fence_after();
+              pv(x, i);
+              if (i == it.n_x[x] - 1) tc_commit(bar(O_FULL + x));
             }
-            *reinterpret_cast<uint4*>(sm.q + tile_off(row, c)) = lo;
-            *reinterpret_cast<uint4*>(sm.q + tile_off(row, c + 8)) = hi;
+            if (x == 1) tc_commit(bar(V_EMPTY + (vc + i) % kVStages));
+            if (i + 1 < it.n_x[x]) {
+              need_k(i + 1);
+              tc_fence_after();
+              qk(x, i + 1);
+            }
           }
-        } else {
-#pragma unroll
-          for (int c = 0; c < 16; ++c) *reinterpret_cast<uint4*>(sm.q + tile_off(row, c)) = make_uint4(0, 0, 0, 0);
+          if (i + 1 < n) {
+            tc_commit(bar(K_EMPTY + (kc + i + 1) % kKStages));
+            if (i + 1 == n - 1) tc_commit(bar(Q_EMPTY));
+          }
         }
+        kc += n; vc += n; ++qc;
+        if (it.n_x[0] > 0) ++oc[0];
+        if (it.n_x[1] > 0) ++oc[1];
       }
-      fence_proxy_async();
-      mbar_arrive(bar(Q_FULL));
-      // ---- K tiles: one key per thread, rotated in place in the UMMA layout
-      for (int i = 0; i < td.n_kv; ++i, ++kv_it) {
-        const int st = kv_it & 1;
-        const uint32_t par = (kv_it >> 1) & 1;
-        const int j = kv_lo + i * BN + row;
-        mbar_wait(bar(K_FULL + st), par);
-        if (!(prm.flags & MINIPIC_K_PREROTATED) && j < kv_hi) {
-          const int p = __ldg(pos + j);
-          unsigned char* kt = sm.k[st];
+    }
+  } else if (warp >= 8) {
+    // ============================================================ rotation warps: Q (a3) and K tiles (a5)
+    reg_dec<80>();
+    const int rw = warp - 8, rot_tid = threadIdx.x - 256;
+    Rot rot;
+    rot.f0 = prm.phase_inc[2 * lane]; rot.f1 = prm.phase_inc[2 * lane + 1];
+    {
+      const float2 s0 = prm.step[2 * lane], s1 = prm.step[2 * lane + 1];
+      rot.c1 = pk2(s0.x, s1.x); rot.s1 = pk2(s0.y, s1.y); rot.ns1 = pk2(-s0.y, -s1.y);
+    }
+    rot.c = 0; rot.s = 0;
+    uint32_t off8[8];   // byte offset of the lane's word inside row (r & 7) of a swizzle atom
 #pragma unroll
-          for (int c = 0; c < 8; ++c) {
-            uint4 lo = *reinterpret_cast<uint4*>(kt + tile_off(row, c));
-            uint4 hi = *reinterpret_cast<uint4*>(kt + tile_off(row, c + 8));
-            float cs[8], sn[8];
-            cs8(prm.rp, sm.finc, p, 8 * c, cs, sn);
-            rotate16(lo, hi, cs, sn);
-            *reinterpret_cast<uint4*>(kt + tile_off(row, c)) = lo;
-            *reinterpret_cast<uint4*>(kt + tile_off(row, c + 8)) = hi;
+    for (int k = 0; k < 8; ++k) off8[k] = (uint32_t)(k * 128 + (((lane >> 2) ^ k) << 4) + ((lane & 3) << 2));
+    const bool k_prerot = (prm.flags & MINIPIC_K_PREROTATED) != 0, q_prerot = (prm.flags & MINIPIC_Q_PREROTATED) != 0;
+    uint32_t kc = 0, vc = 0, qc = 0;
+    for (uint32_t it_n = 0;; ++it_n) {
+      const int slot = it_n & (kRing - 1);
+      w.wait(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
+      if (w.dead || sm.ring[slot].t0 < 0) break;
+      const Item it = load_item<TOK>(sm.ring[slot]);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(SCHED_EMPTY + slot));
+      if (it.n_kv == 0) continue;
+      const int* pos = a.kv_positions + __ldg(a.cu_kv_lens + it.r);
+      for (int i = 0; i < it.n_kv; ++i) {
+        // ---- K tile i: every 16-key block restarts the trig recurrence from the exact fixed-point phase
+        const int st = kc % kKStages;
+        const int j0 = it.kv_lo + i * BN;
+        w.wait(bar(K_FULL + st), (kc / kKStages) & 1);
+        if (!k_prerot) {
+          const int nblk = min(BN / kBlock, (it.kv_hi - j0 + kBlock - 1) / kBlock);
+          const uint32_t kt = smem_u32(sm.k[st]);
+#pragma unroll 1
+          for (int b = 2 * rw; b < 2 * rw + 2; ++b) {
+            if (b >= nblk) break;
+            const int myp = __ldg(pos + min(j0 + b * kBlock + (lane & 15), it.kv_len - 1));
+            int prev = 0;
+#pragma unroll
+            for (int rr = 0; rr < kBlock; ++rr) {
+              const int p = __shfl_sync(0xffffffffu, myp, rr);
+              if (rr == 0 || p != prev + 1) rot.restart(p); else rot.advance();
+              prev = p;
+              rot.apply(kt + b * 2048 + (rr >> 3) * 1024 + off8[rr & 7]);
+            }
           }
         }
         fence_proxy_async();
         mbar_arrive(bar(K_READY + st));
-        // V: rows at or beyond the item's last visible key get P = 0; make sure 0 * (stale / uninitialised bits) != NaN
-        mbar_wait(bar(V_FULL + st), par);
-        if (j >= kv_hi) {
+        ++kc;
+        if (i == 0) {
+          // ---- Q super-tile: row = token * G + head-in-group; G rows share one position
+          w.wait(bar(Q_FULL), qc & 1);
+          if (!q_prerot) {
 #pragma unroll
-          for (int c = 0; c < 16; ++c) *reinterpret_cast<uint4*>(sm.v[st] + tile_off(row, c)) = make_uint4(0, 0, 0, 0);
+            for (int x = 0; x < 2; ++x) {
+              if (it.ntok_x[x] <= 0) continue;
+              constexpr int TPW = 32 / G;   // tokens per warp
+              const int tok0 = rw * TPW;
+              const int myp = (tok0 + (lane % TPW) < it.ntok_x[x])
+                                  ? __ldg(pos + min(it.idx0 + x * TOK + tok0 + (lane % TPW), it.kv_len - 1)) : 0;
+              const uint32_t qt = smem_u32(sm.q[x]);
+#pragma unroll
+              for (int t = 0; t < TPW; ++t) {
+                if (tok0 + t >= it.ntok_x[x]) break;
+                rot.restart(__shfl_sync(0xffffffffu, myp, t));
+#pragma unroll
+                for (int g = 0; g < G; ++g) {
+                  const int r = 32 * rw + t * G + g;
+                  rot.apply(qt + (r >> 3) * 1024 + off8[(t * G + g) & 7]);
+                }
+              }
+            }
+          }
+          fence_proxy_async();
+          mbar_arrive(bar(Q_READY));
+          ++qc;
         }
-        fence_proxy_async();
-        mbar_arrive(bar(V_READY + st));
+        // ---- V tile i: rows at or beyond kv_hi inside the last gathered block may hold anything (never written
+        //      cache slots); their P is 0, make sure 0 * (those bits) is not NaN
+        if (i == it.n_kv - 1 && (it.kv_hi & (kBlock - 1)) != 0) {
+          const int vs = (vc + i) % kVStages;
+          w.wait(bar(V_FULL + vs), ((vc + i) / kVStages) & 1);
+          const int first = it.kv_hi - j0, last = (first + kBlock - 1) & ~(kBlock - 1);
+          if (rot_tid >= first && rot_tid < last) {
+            const uint32_t vrow = smem_u32(sm.v[vs]) + rot_tid * 128;
+#pragma unroll
+            for (int c = 0; c < 8; ++c) { sts128z(vrow + c * 16); sts128z(vrow + kHalfBytes + c * 16); }
+          }
+          fence_proxy_async();
+          mbar_arrive(bar(V_FIX));
+        }
       }
-      ++n_used;
+      vc += it.n_kv;
     }
   } else {
     // ============================================================ softmax + epilogue warps (a7, a9): thread = row
-    const int row = threadIdx.x;
-    const uint32_t t_lane = tmem + ((uint32_t)(warp * 32) << 16);
-    uint32_t s_it = 0, pv_it = 0;
-    for (int k = 0;; ++k) {
-      const int item = item_of(k);
-      if (item >= n_items) break;
-      const TileDesc td = prm.tiles[item / prm.hkv];
-      const int kvh = item % prm.hkv;
-      const int tok = row / G, hg = row % G;
-      const bool row_ok = tok < td.ntok;
-      const int idx_row = td.idx0 + tok;
-      const int kv_lo = td.lo & ~(kBlock - 1);
+    reg_inc<192>();
+    const int x = warp >> 2;                 // 0: tile A, 1: tile B
+    const int row = threadIdx.x & 127;
+    const uint32_t t_lane = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+    const uint32_t t_s = t_lane + x * BN, t_o = t_lane + (2 + x) * BN;
+    const int tok_in = row / G, hg = row % G;
+    uint32_t sc = 0, oc = 0;
+    for (uint32_t it_n = 0;; ++it_n) {
+      const int slot = it_n & (kRing - 1);
+      w.wait(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
+      if (w.dead || sm.ring[slot].t0 < 0) break;
+      const Item it = load_item<TOK>(sm.ring[slot]);
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar(SCHED_EMPTY + slot));
+      const bool row_ok = tok_in < it.ntok_x[x];
+      const int tok = x * TOK + tok_in;
+      const int idx_first = it.idx0 + x * TOK;                       // lowest query index of this tile
+      const int idx_row = min(it.idx0 + tok, it.kv_len - 1);         // highest visible key of this row
+      const int n = it.n_x[x];
       float m_used = -INFINITY, l_run = 0.f;   // m in log2 units (score * scale * log2 e)
-      for (int i = 0; i < td.n_kv; ++i, ++s_it) {
-        const int sb = s_it & 1;
-        const int j0 = kv_lo + i * BN;
+      for (int i = 0; i < n; ++i, ++sc) {
+        const int j0 = it.kv_lo + i * BN;
         float s[BN];
-        mbar_wait(bar(S_FULL + sb), (s_it >> 1) & 1);
+        w.wait(bar(S_FULL + x), sc & 1);
         tc_fence_after();
 #pragma unroll
-        for (int c = 0; c < 4; ++c) tmem_ld32(t_lane + sb * BN + c * 32, s + c * 32);
+        for (int c = 0; c < 4; ++c) tmem_ld32(t_s + c * 32, s + c * 32);
         tmem_wait_ld();
-        tc_fence_before();
-        mbar_arrive(bar(S_EMPTY + sb));
-        const bool full = (j0 >= td.lo) && (j0 + BN - 1 <= td.idx0);
-        float mx = -INFINITY;
-        if (full) {
+        const bool full = (j0 >= it.lo) && (j0 + BN - 1 <= min(idx_first, it.kv_len - 1));
+        if (!full) {
+          const int c_lo = it.lo - j0, c_hi = row_ok ? idx_row - j0 : -1;
 #pragma unroll
-          for (int c = 0; c < BN; ++c) mx = fmaxf(mx, s[c]);
-        } else {
-#pragma unroll
-          for (int c = 0; c < BN; ++c) {
-            const int j = j0 + c;
-            s[c] = (j >= td.lo && j <= idx_row) ? s[c] : -INFINITY;
-            mx = fmaxf(mx, s[c]);
-          }
+          for (int c = 0; c < BN; ++c) s[c] = (c >= c_lo && c <= c_hi) ? s[c] : -INFINITY;
         }
-        const float m_new = fmaxf(m_used, mx * prm.scale_log2);
-        const bool grow = m_new > m_used + 8.f;   // lazy rescale: P may exceed 1 by up to 2^8 before O, l are rescaled
-        bool pv_waited = (i == 0);
+        float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+#pragma unroll
+        for (int c = 0; c < BN; c += 8) {
+          mx0 = max3(mx0, s[c], s[c + 1]); mx1 = max3(mx1, s[c + 2], s[c + 3]);
+          mx2 = max3(mx2, s[c + 4], s[c + 5]); mx3 = max3(mx3, s[c + 6], s[c + 7]);
+        }
+        const float m_new = fmaxf(m_used, fmaxf(max3(mx0, mx1, mx2), mx3) * prm.scale_log2);
         if (i == 0) {
           m_used = m_new;
-        } else if (__any_sync(0xffffffffu, grow)) {
-          mbar_wait(bar(PV_DONE), pv_it & 1);     // O is stable once PV(i-1) has completed
-          pv_waited = true;
-          const float corr = grow ? fast_exp2(m_used - m_new) : 1.f;
-          if (grow) { l_run *= corr; m_used = m_new; }
-          tc_fence_after();
+        } else {
+          const bool grow = m_new > m_used + 8.f;   // lazy rescale: P may exceed 1 by up to 2^8 before O, l are rescaled
+          if (__any_sync(0xffffffffu, grow)) {
+            // S_FULL(i) was committed after PV(i-1): O is stable until this thread publishes P(i)
+            const float corr = grow ? fast_exp2(m_used - m_new) : 1.f;
+            if (grow) { l_run *= corr; m_used = m_new; }
 #pragma unroll
-          for (int c = 0; c < 4; ++c) {
-            float o[32];
-            tmem_ld32(t_lane + 2 * BN + c * 32, o);
-            tmem_wait_ld();
+            for (int c = 0; c < 4; ++c) {
+              float o[32];
+              tmem_ld32(t_o + c * 32, o);
+              tmem_wait_ld();
 #pragma unroll
-            for (int e = 0; e < 32; ++e) o[e] *= corr;
-            tmem_st32(t_lane + 2 * BN + c * 32, o);
+              for (int e = 0; e < 32; ++e) o[e] *= corr;
+              tmem_st32(t_o + c * 32, reinterpret_cast<const uint32_t*>(o));
+            }
           }
-          tmem_wait_st();
-          tc_fence_before();
         }
         const float m_sub = (m_used == -INFINITY) ? 0.f : m_used;
-        float lsum = 0.f;
-        uint4 pk[16];
+        float lsum0 = 0.f, lsum1 = 0.f;
 #pragma unroll
-        for (int c = 0; c < 16; ++c) {
-          float pv[8];
+        for (int h = 0; h < 2; ++h) {
+          uint32_t pk[32];
 #pragma unroll
-          for (int e = 0; e < 8; ++e) { pv[e] = fast_exp2(fmaf(s[8 * c + e], prm.scale_log2, -m_sub)); lsum += pv[e]; }
-          pk[c].x = pack_bf16(pv[0], pv[1]); pk[c].y = pack_bf16(pv[2], pv[3]);
-          pk[c].z = pack_bf16(pv[4], pv[5]); pk[c].w = pack_bf16(pv[6], pv[7]);
+          for (int c = 0; c < 32; ++c) {
+            const float p0 = fast_exp2(fmaf(s[64 * h + 2 * c], prm.scale_log2, -m_sub));
+            const float p1 = fast_exp2(fmaf(s[64 * h + 2 * c + 1], prm.scale_log2, -m_sub));
+            lsum0 += p0; lsum1 += p1;
+            pk[c] = pack_bf16(p0, p1);
+          }
+          tmem_st32(t_s + 32 * h, pk);
         }
-        if (!pv_waited) mbar_wait(bar(PV_DONE), pv_it & 1);   // the single P buffer is free once PV(i-1) has read it
-        if (i > 0) ++pv_it;
-#pragma unroll
-        for (int c = 0; c < 16; ++c) *reinterpret_cast<uint4*>(sm.p + tile_off(row, c)) = pk[c];
-        l_run += lsum;
-        fence_proxy_async();
-        mbar_arrive(bar(P_FULL));
-      }
-      if (td.n_kv > 0) {
-        mbar_wait(bar(PV_DONE), pv_it & 1);
-        ++pv_it;
-        tc_fence_after();
+        l_run += lsum0 + lsum1;
+        tmem_wait_st();
+        tc_fence_before();
+        mbar_arrive(bar(P_FULL + x));
       }
       // ---- epilogue (a9): O / l -> out, LSE = ln sum exp of the scaled scores
+      if (it.ntok_x[x] <= 0) continue;
       const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
-      __nv_bfloat16* orow = (__nv_bfloat16*)a.out + ((size_t)(td.t0 + tok) * prm.hq + kvh * G + hg) * D;
+      __nv_bfloat16* orow = (__nv_bfloat16*)a.out + ((size_t)(it.t0 + tok) * prm.hq + it.kvh * G + hg) * D;
+      if (n > 0) { w.wait(bar(O_FULL + x), oc & 1); ++oc; tc_fence_after(); }
 #pragma unroll
       for (int c = 0; c < 4; ++c) {
         float o[32];
-        if (td.n_kv > 0) { tmem_ld32(t_lane + 2 * BN + c * 32, o); tmem_wait_ld(); }
+        if (n > 0) { tmem_ld32(t_o + c * 32, o); tmem_wait_ld(); }
         else {
 #pragma unroll
           for (int e = 0; e < 32; ++e) o[e] = 0.f;
@@ -534,22 +710,22 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_co
         if (row_ok) {
 #pragma unroll
           for (int e = 0; e < 4; ++e) {
-            uint4 w;
-            w.x = pack_bf16(o[8 * e] * inv, o[8 * e + 1] * inv); w.y = pack_bf16(o[8 * e + 2] * inv, o[8 * e + 3] * inv);
-            w.z = pack_bf16(o[8 * e + 4] * inv, o[8 * e + 5] * inv); w.w = pack_bf16(o[8 * e + 6] * inv, o[8 * e + 7] * inv);
-            *reinterpret_cast<uint4*>(orow + c * 32 + e * 8) = w;
+            uint4 v;
+            v.x = pack_bf16(o[8 * e] * inv, o[8 * e + 1] * inv); v.y = pack_bf16(o[8 * e + 2] * inv, o[8 * e + 3] * inv);
+            v.z = pack_bf16(o[8 * e + 4] * inv, o[8 * e + 5] * inv); v.w = pack_bf16(o[8 * e + 6] * inv, o[8 * e + 7] * inv);
+            *reinterpret_cast<uint4*>(orow + c * 32 + e * 8) = v;
           }
         }
       }
+      if (n > 0) { tc_fence_before(); mbar_arrive(bar(O_FREE + x)); }
       if (row_ok)
-        a.lse[(size_t)(td.t0 + tok) * prm.hq + kvh * G + hg] =
+        a.lse[(size_t)(it.t0 + tok) * prm.hq + it.kvh * G + hg] =
             l_run > 0.f ? (m_used + log2f(l_run)) * 0.6931471805599453f : -INFINITY;
-      if (td.n_kv > 0) { tc_fence_before(); mbar_arrive(bar(O_FREE)); }
     }
   }
   tc_fence_before();
   __syncthreads();
-  if (warp == 9) {
+  if (warp == 13) {
     tc_fence_after();
     asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512));
   }
@@ -582,17 +758,29 @@ bool make_cache_map(CUtensorMap* m, const void* cache, int num_blocks, int hkv) 
              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
+// q viewed as [Tq][Hq][128]; box = (128/G tokens) x (G heads) x 64 columns: one half of an MMA tile, rows (token, head)
+bool make_q_map(CUtensorMap* m, const void* q, int num_q_tokens, int hq, int group) {
+  EncodeTiledFn enc = get_encode();
+  if (!enc) return false;
+  cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)hq, (cuuint64_t)num_q_tokens};
+  cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)hq * D * 2};
+  cuuint32_t box[3] = {64, (cuuint32_t)group, (cuuint32_t)(BM / group)};
+  cuuint32_t estr[3] = {1, 1, 1};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, const_cast<void*>(q), dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
 
 template <int G>
-bool launch_g(const Ctx& c, const PrefillArgs& a, const CUtensorMap& mk, const CUtensorMap& mv, const Params& prm, int sms) {
-  const size_t smem = sizeof(Smem) + 1024;
+bool launch_g(const Ctx& c, const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const Params& prm, int sms) {
+  const size_t smem = sizeof(Smem);
   static bool attr_done = false;
   if (!attr_done) {
     if (cudaFuncSetAttribute(prefill_sm100_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
       return false;
     attr_done = true;
   }
-  prefill_sm100_kernel<G><<<sms, kThreads, smem, c.stream>>>(mk, mv, prm);
+  prefill_sm100_kernel<G><<<sms, kThreads, smem, c.stream>>>(mq, mk, mv, prm);
   note_launch();
   return true;
 }
@@ -608,24 +796,35 @@ size_t prefill_sm100_workspace_bytes(const Ctx&, int, int num_q_tokens) {
 }
 
 bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
-  CUtensorMap mk, mv;
-  if (!make_cache_map(&mk, a.k_cache, c.num_blocks, c.hkv) || !make_cache_map(&mv, a.v_cache, c.num_blocks, c.hkv)) return false;
+  CUtensorMap mq, mk, mv;
+  if (!make_cache_map(&mk, a.k_cache, c.num_blocks, c.hkv) || !make_cache_map(&mv, a.v_cache, c.num_blocks, c.hkv) ||
+      !make_q_map(&mq, a.q, a.num_q_tokens, c.hq, c.group))
+    return false;
   PlanHeader* hdr = (PlanHeader*)a.workspace;
   TileDesc* sorted = (TileDesc*)((char*)a.workspace + sizeof(PlanHeader));
   TileDesc* tmp = sorted + (a.num_q_tokens + 1);
-  prefill_plan_kernel<<<1, 1024, 0, c.stream>>>(a, BM / c.group, hdr, sorted, tmp);
-  note_launch();
+  const int tok2 = 2 * BM / c.group;
+  if (cudaMemsetAsync(hdr, 0, sizeof(PlanHeader), c.stream) != cudaSuccess) return false;
+  plan_mark_kernel<<<(a.num_q_tokens + 255) / 256, 256, 0, c.stream>>>(a, tok2, hdr, tmp);
+  plan_scan_kernel<<<1, 1024, 0, c.stream>>>(hdr);
+  plan_scatter_kernel<<<(a.num_q_tokens + 255) / 256, 256, 0, c.stream>>>(hdr, tmp, sorted);
+  note_launch(3);
   Params prm;
   prm.a = a; prm.hq = c.hq; prm.hkv = c.hkv; prm.scale_log2 = c.scale_log2; prm.flags = c.flags;
-  prm.hdr = hdr; prm.tiles = sorted; prm.rp = c.rope;
+  prm.hdr = hdr; prm.tiles = sorted;
+  prm.oob_row = c.num_blocks * c.hkv * kBlock;
+  for (int i = 0; i < 64; ++i) {
+    prm.phase_inc[i] = c.rope.phase_inc[i];
+    prm.step[i] = make_float2((float)c.rope_step_cos[i], (float)c.rope_step_sin[i]);
+  }
   int dev = 0, sms = 148;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   switch (c.group) {
-    case 1: return launch_g<1>(c, a, mk, mv, prm, sms);
-    case 2: return launch_g<2>(c, a, mk, mv, prm, sms);
-    case 4: return launch_g<4>(c, a, mk, mv, prm, sms);
-    case 8: return launch_g<8>(c, a, mk, mv, prm, sms);
+    case 1: return launch_g<1>(c, mq, mk, mv, prm, sms);
+    case 2: return launch_g<2>(c, mq, mk, mv, prm, sms);
+    case 4: return launch_g<4>(c, mq, mk, mv, prm, sms);
+    case 8: return launch_g<8>(c, mq, mk, mv, prm, sms);
   }
   return false;
 }
