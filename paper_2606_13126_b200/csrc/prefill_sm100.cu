@@ -101,19 +101,25 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tma
       "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
       ::"r"(dst), "l"(tmap), "r"(bar), "r"(x), "r"(y), "r"(z) : "memory");
 }
+// Shared-memory matrix descriptors (SWIZZLE_128B): the low word carries the start address (>> 4) and the leading byte
+// offset (>> 4, bits 16-29); the high word is the same for every operand of this kernel: stride byte offset 1024
+// (8 rows x 128 B), descriptor version 1 (bit 46), swizzle mode 128B (2 << 61).
+constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);
 // D[tmem] (+)= A[smem] * B[smem]
-__device__ __forceinline__ void umma_ss(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+__device__ __forceinline__ void umma_ss(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, uint32_t acc) {
   asm volatile(
-      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-      ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+      "{\n\t.reg .pred p;\n\t.reg .b64 da, db;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "mov.b64 da, {%1, %5};\n\tmov.b64 db, {%2, %5};\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(idesc), "r"(acc), "r"(kDescHi) : "memory");
 }
 // D[tmem] (+)= A[tmem] * B[smem]
-__device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t bdesc, uint32_t idesc, uint32_t acc) {
+__device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_lo, uint32_t idesc, uint32_t acc) {
   asm volatile(
-      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
-      ::"r"(d_tmem), "r"(a_tmem), "l"(bdesc), "r"(idesc), "r"(acc) : "memory");
+      "{\n\t.reg .pred p;\n\t.reg .b64 db;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+      "mov.b64 db, {%2, %5};\n\t"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], db, %3, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_tmem), "r"(b_lo), "r"(idesc), "r"(acc), "r"(kDescHi) : "memory");
 }
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
   uint32_t* r = reinterpret_cast<uint32_t*>(v);
@@ -177,11 +183,6 @@ __device__ __forceinline__ void sts128z(uint32_t addr) {
 template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 
-// shared-memory matrix descriptor (SWIZZLE_128B, version 1): start address, leading / stride byte offsets
-__device__ __forceinline__ uint64_t smem_desc(uint32_t addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
-  return (uint64_t)((addr >> 4) & 0x3FFF) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFF) << 16) |
-         ((uint64_t)((sbo_bytes >> 4) & 0x3FFF) << 32) | (1ull << 46) | (2ull << 61);
-}
 // instruction descriptor: D fp32, A/B bf16, M=128, N=128; b_mn = B operand is MN-major (V tile)
 __host__ __device__ constexpr uint32_t instr_desc(bool b_mn) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn ? 1u : 0u) << 16) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
@@ -442,80 +443,76 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       }
     } else if (warp == 13 && lane == 0) {
       // ============================================================ MMA issuer (a6, a8): one thread
-      const uint32_t idesc_qk = instr_desc(false), idesc_pv = instr_desc(true);
-      uint32_t kc = 0, vc = 0, qc = 0, fixc = 0;
-      uint32_t pc[2] = {0, 0}, oc[2] = {0, 0};
+      // Kept lean on purpose (this role lives in 48 registers): 32-bit descriptor words, the high word is a
+      // compile-time constant, pipeline stages / phases are running counters, no per-stage tables.
+      constexpr uint32_t idesc_qk = instr_desc(false), idesc_pv = instr_desc(true);
+      const uint32_t q_lo = ((smem_u32(sm.q[0]) >> 4) & 0x3FFF) | (1u << 16);          // + x * 2048
+      const uint32_t k_lo = ((smem_u32(sm.k[0]) >> 4) & 0x3FFF) | (1u << 16);          // + stage * 2048
+      const uint32_t v_lo = ((smem_u32(sm.v[0]) >> 4) & 0x3FFF) | ((uint32_t)(kHalfBytes >> 4) << 16);
+      uint32_t k_st = 0, k_ph = 0, v_st = 0, v_ph = 0;   // next K / V stage to consume and its full-barrier parity
+      uint32_t ph = 0;   // bit 0,1: P_FULL parity of tile A,B; bit 2,3: O_FREE; bit 4: Q_READY; bit 5: V_FIX
       for (uint32_t it_n = 0;; ++it_n) {
         const int slot = it_n & (kRing - 1);
         w.wait(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
         if (w.dead || sm.ring[slot].t0 < 0) break;
-        const Item it = load_item<TOK>(sm.ring[slot]);
+        int n, nx0, nx1;
+        bool vfix;
+        {
+          const Item it = load_item<TOK>(sm.ring[slot]);
+          n = it.n_kv; nx0 = it.n_x[0]; nx1 = it.n_x[1];
+          vfix = (it.kv_hi & (kBlock - 1)) != 0;
+        }
         mbar_arrive(bar(SCHED_EMPTY + slot));
-        const int n = it.n_kv;
         if (n == 0) continue;
-        const bool vfix = (it.kv_hi & (kBlock - 1)) != 0;
-        int k_upto = 0, v_upto = 0;
-        auto need_k = [&](int i) {
-          while (k_upto <= i) { const uint32_t c = kc + k_upto; w.wait(bar(K_READY + c % kKStages), (c / kKStages) & 1); ++k_upto; }
-        };
-        auto need_v = [&](int i) {
-          while (v_upto <= i) {
-            const uint32_t c = vc + v_upto;
-            w.wait(bar(V_FULL + c % kVStages), (c / kVStages) & 1);
-            if (v_upto == n - 1 && vfix) { w.wait(bar(V_FIX), fixc & 1); ++fixc; }
-            ++v_upto;
-          }
-        };
-        auto qk = [&](int x, int i) {
-          const uint32_t q_addr = smem_u32(sm.q[x]), k_addr = smem_u32(sm.k[(kc + i) % kKStages]);
+        // QK^T of tile x against K stage st: S_x = Q_x K'^T
+        auto qk = [&](int x, uint32_t st) {
+          const uint32_t a_lo = q_lo + (uint32_t)x * (kTileBytes >> 4), b_lo = k_lo + st * (kTileBytes >> 4);
 #pragma unroll
           for (int ks = 0; ks < D / 16; ++ks) {
-            const uint32_t off = (ks >> 2) * kHalfBytes + (ks & 3) * 32;
-            umma_ss(tmem + x * BN, smem_desc(q_addr + off, 16, 1024), smem_desc(k_addr + off, 16, 1024), idesc_qk, ks > 0);
+            const uint32_t off = (ks >> 2) * (kHalfBytes >> 4) + (ks & 3) * 2;
+            umma_ss(tmem + x * BN, a_lo + off, b_lo + off, idesc_qk, ks > 0);
           }
           tc_commit(bar(S_FULL + x));
         };
-        auto pv = [&](int x, int i) {
-          const uint32_t v_addr = smem_u32(sm.v[(vc + i) % kVStages]);
-#pragma unroll
-          for (int ks = 0; ks < BN / 16; ++ks)
-            umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, smem_desc(v_addr + ks * 2048, kHalfBytes, 1024), idesc_pv,
-                    (i > 0 || ks > 0));
-        };
-        w.wait(bar(Q_READY), qc & 1);
-        need_k(0);
+        w.wait(bar(Q_READY), (ph >> 4) & 1); ph ^= 16u;
+        w.wait(bar(K_READY + k_st), k_ph);
         tc_fence_after();
-#pragma unroll
-        for (int x = 0; x < 2; ++x)
-          if (it.n_x[x] > 0) qk(x, 0);
-        tc_commit(bar(K_EMPTY + kc % kKStages));
+        if (nx0 > 0) qk(0, k_st);
+        if (nx1 > 0) qk(1, k_st);
+        tc_commit(bar(K_EMPTY + k_st));
+        if (++k_st == kKStages) { k_st = 0; k_ph ^= 1; }
         if (n == 1) tc_commit(bar(Q_EMPTY));
+#pragma unroll 1
         for (int i = 0; i < n; ++i) {
-#pragma unroll
+          w.wait(bar(V_FULL + v_st), v_ph);
+          if (i == n - 1 && vfix) { w.wait(bar(V_FIX), (ph >> 5) & 1); ph ^= 32u; }
+          bool k_waited = false;
+#pragma unroll 1
           for (int x = 0; x < 2; ++x) {
-            if (i < it.n_x[x]) {
-              w.wait(bar(P_FULL + x), pc[x] & 1); ++pc[x];
-              need_v(i);
-              if (i == 0) w.wait(bar(O_FREE + x), (oc[x] & 1) ^ 1);
+            const int nx = x ? nx1 : nx0;
+            if (i < nx) {
+              w.wait(bar(P_FULL + x), (ph >> x) & 1); ph ^= 1u << x;
+              if (i == 0) { w.wait(bar(O_FREE + x), ((ph >> (2 + x)) & 1) ^ 1); ph ^= 4u << x; }
               tc_fence_after();
-              pv(x, i);
-              if (i == it.n_x[x] - 1) tc_commit(bar(O_FULL + x));
+              const uint32_t b_lo = v_lo + v_st * (kTileBytes >> 4);
+#pragma unroll
+              for (int ks = 0; ks < BN / 16; ++ks)
+                umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, b_lo + ks * (2048 >> 4), idesc_pv, (i > 0 || ks > 0));
+              if (i == nx - 1) tc_commit(bar(O_FULL + x));
             }
-            if (x == 1) tc_commit(bar(V_EMPTY + (vc + i) % kVStages));
-            if (i + 1 < it.n_x[x]) {
-              need_k(i + 1);
-              tc_fence_after();
-              qk(x, i + 1);
+            if (x == 1) tc_commit(bar(V_EMPTY + v_st));
+            if (i + 1 < nx) {
+              if (!k_waited) { w.wait(bar(K_READY + k_st), k_ph); k_waited = true; tc_fence_after(); }
+              qk(x, k_st);
             }
           }
+          if (++v_st == kVStages) { v_st = 0; v_ph ^= 1; }
           if (i + 1 < n) {
-            tc_commit(bar(K_EMPTY + (kc + i + 1) % kKStages));
+            tc_commit(bar(K_EMPTY + k_st));
+            if (++k_st == kKStages) { k_st = 0; k_ph ^= 1; }
             if (i + 1 == n - 1) tc_commit(bar(Q_EMPTY));
           }
         }
-        kc += n; vc += n; ++qc;
-        if (it.n_x[0] > 0) ++oc[0];
-        if (it.n_x[1] > 0) ++oc[1];
       }
     }
   } else if (warp >= 8) {
