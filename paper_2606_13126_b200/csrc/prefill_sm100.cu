@@ -180,6 +180,11 @@ __device__ __forceinline__ void sts32(uint32_t addr, uint32_t v) { asm volatile(
 __device__ __forceinline__ void sts128z(uint32_t addr) {
   asm volatile("st.shared.v4.b32 [%0], {%1, %1, %1, %1};" ::"r"(addr), "r"(0) : "memory");
 }
+__device__ __forceinline__ bool elect_one() {   // one lane of a converged warp (the same lane every time)
+  uint32_t pred;
+  asm volatile("{\n\t.reg .pred p;\n\telect.sync _|p, 0xffffffff;\n\tselp.u32 %0, 1, 0, p;\n\t}" : "=r"(pred));
+  return pred != 0;
+}
 template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 
@@ -441,10 +446,12 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           y = y_next;
         }
       }
-    } else if (warp == 13 && lane == 0) {
-      // ============================================================ MMA issuer (a6, a8): one thread
-      // Kept lean on purpose (this role lives in 48 registers): 32-bit descriptor words, the high word is a
-      // compile-time constant, pipeline stages / phases are running counters, no per-stage tables.
+    } else if (warp == 13) {
+      // ============================================================ MMA issuer (a6, a8)
+      // The whole warp runs the control flow converged on warp-uniform values (item fields are broadcast from
+      // lane 0, so descriptors, stages and phases live in uniform registers); one elected lane issues every
+      // tcgen05.mma / tcgen05.commit.  This role lives in 48 registers: 32-bit descriptor words, running
+      // stage / phase counters, no per-stage tables.
       constexpr uint32_t idesc_qk = instr_desc(false), idesc_pv = instr_desc(true);
       const uint32_t q_lo = ((smem_u32(sm.q[0]) >> 4) & 0x3FFF) | (1u << 16);          // + x * 2048
       const uint32_t k_lo = ((smem_u32(sm.k[0]) >> 4) & 0x3FFF) | (1u << 16);          // + stage * 2048
@@ -454,17 +461,18 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       for (uint32_t it_n = 0;; ++it_n) {
         const int slot = it_n & (kRing - 1);
         w.wait(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
-        if (w.dead || sm.ring[slot].t0 < 0) break;
-        int n, nx0, nx1;
-        bool vfix;
+        if (__any_sync(0xffffffffu, w.dead) || sm.ring[slot].t0 < 0) break;
+        int n, nx0, nx1, kv_hi;
         {
           const Item it = load_item<TOK>(sm.ring[slot]);
-          n = it.n_kv; nx0 = it.n_x[0]; nx1 = it.n_x[1];
-          vfix = (it.kv_hi & (kBlock - 1)) != 0;
+          n = __shfl_sync(0xffffffffu, it.n_kv, 0); nx0 = __shfl_sync(0xffffffffu, it.n_x[0], 0);
+          nx1 = __shfl_sync(0xffffffffu, it.n_x[1], 0); kv_hi = __shfl_sync(0xffffffffu, it.kv_hi, 0);
         }
-        mbar_arrive(bar(SCHED_EMPTY + slot));
+        const bool vfix = (kv_hi & (kBlock - 1)) != 0;
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(SCHED_EMPTY + slot));
         if (n == 0) continue;
-        // QK^T of tile x against K stage st: S_x = Q_x K'^T
+        // QK^T of tile x against K stage st: S_x = Q_x K'^T (elected lane only)
         auto qk = [&](int x, uint32_t st) {
           const uint32_t a_lo = q_lo + (uint32_t)x * (kTileBytes >> 4), b_lo = k_lo + st * (kTileBytes >> 4);
 #pragma unroll
@@ -477,11 +485,14 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         w.wait(bar(Q_READY), (ph >> 4) & 1); ph ^= 16u;
         w.wait(bar(K_READY + k_st), k_ph);
         tc_fence_after();
-        if (nx0 > 0) qk(0, k_st);
-        if (nx1 > 0) qk(1, k_st);
-        tc_commit(bar(K_EMPTY + k_st));
+        if (elect_one()) {
+          if (nx0 > 0) qk(0, k_st);
+          if (nx1 > 0) qk(1, k_st);
+          tc_commit(bar(K_EMPTY + k_st));
+          if (n == 1) tc_commit(bar(Q_EMPTY));
+        }
+        __syncwarp();
         if (++k_st == kKStages) { k_st = 0; k_ph ^= 1; }
-        if (n == 1) tc_commit(bar(Q_EMPTY));
 #pragma unroll 1
         for (int i = 0; i < n; ++i) {
           w.wait(bar(V_FULL + v_st), v_ph);
@@ -490,28 +501,32 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
 #pragma unroll 1
           for (int x = 0; x < 2; ++x) {
             const int nx = x ? nx1 : nx0;
-            if (i < nx) {
+            const bool do_pv = i < nx, do_qk = i + 1 < nx;
+            if (do_pv) {
               w.wait(bar(P_FULL + x), (ph >> x) & 1); ph ^= 1u << x;
               if (i == 0) { w.wait(bar(O_FREE + x), ((ph >> (2 + x)) & 1) ^ 1); ph ^= 4u << x; }
-              tc_fence_after();
-              const uint32_t b_lo = v_lo + v_st * (kTileBytes >> 4);
+            }
+            if (do_qk && !k_waited) { w.wait(bar(K_READY + k_st), k_ph); k_waited = true; }
+            tc_fence_after();
+            if (elect_one()) {
+              if (do_pv) {
+                const uint32_t b_lo = v_lo + v_st * (kTileBytes >> 4);
 #pragma unroll
-              for (int ks = 0; ks < BN / 16; ++ks)
-                umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, b_lo + ks * (2048 >> 4), idesc_pv, (i > 0 || ks > 0));
-              if (i == nx - 1) tc_commit(bar(O_FULL + x));
+                for (int ks = 0; ks < BN / 16; ++ks)
+                  umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, b_lo + ks * (2048 >> 4), idesc_pv, (i > 0 || ks > 0));
+                if (i == nx - 1) tc_commit(bar(O_FULL + x));
+              }
+              if (x == 1) tc_commit(bar(V_EMPTY + v_st));
+              if (do_qk) qk(x, k_st);
+              if (x == 1 && i + 1 < n) {
+                tc_commit(bar(K_EMPTY + k_st));
+                if (i + 1 == n - 1) tc_commit(bar(Q_EMPTY));
+              }
             }
-            if (x == 1) tc_commit(bar(V_EMPTY + v_st));
-            if (i + 1 < nx) {
-              if (!k_waited) { w.wait(bar(K_READY + k_st), k_ph); k_waited = true; tc_fence_after(); }
-              qk(x, k_st);
-            }
+            __syncwarp();
           }
           if (++v_st == kVStages) { v_st = 0; v_ph ^= 1; }
-          if (i + 1 < n) {
-            tc_commit(bar(K_EMPTY + k_st));
-            if (++k_st == kKStages) { k_st = 0; k_ph ^= 1; }
-            if (i + 1 == n - 1) tc_commit(bar(Q_EMPTY));
-          }
+          if (i + 1 < n) { if (++k_st == kKStages) { k_st = 0; k_ph ^= 1; } }
         }
       }
     }
