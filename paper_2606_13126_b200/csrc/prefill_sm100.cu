@@ -32,7 +32,12 @@ constexpr int BM = 128, BN = 128, D = 128;
 constexpr int kTileBytes = BN * D * 2;       // 32 KB: one K / V / Q tile
 constexpr int kHalfBytes = kTileBytes / 2;   // [half of head_dim][128 rows][128 B]
 constexpr int kKStages = 3, kVStages = 2, kRing = 4;
+// 16 warps = 4 warpgroups: softmax A, softmax B (184 registers each after setmaxnreg), rotation (96), control (TMA, MMA and
+// two idle warps, 48).  setmaxnreg is a WARPGROUP-wide instruction (all four warps, same count), and the split must fit the
+// launch pool of 512 * 128 registers or setmaxnreg.inc blocks forever: 256*184 + 128*96 + 128*48 = 65536.
 constexpr int kThreads = 512;
+constexpr int kRegsSoftmax = 184, kRegsRot = 96, kRegsCtl = 48;
+static_assert(256 * kRegsSoftmax + 128 * kRegsRot + 128 * kRegsCtl <= 65536, "setmaxnreg split exceeds the CTA register pool");
 constexpr int kMaxBins = 4096;
 constexpr long long kWaitTimeoutCycles = 4000000000LL;
 
@@ -142,6 +147,21 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t* r) {
         "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
       : "memory");
 }
+__device__ __forceinline__ void tmem_ld16(uint32_t taddr, float* v) {
+  uint32_t* r = reinterpret_cast<uint32_t*>(v);
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]),
+        "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15])
+      : "r"(taddr));
+}
+__device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t* r) {
+  asm volatile(
+      "tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};"
+      ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]), "r"(r[8]),
+        "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15])
+      : "memory");
+}
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ float fast_exp2(float x) {
@@ -170,6 +190,19 @@ __device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) {
   uint64_t d;
   asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
   return d;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ void sts128(uint32_t addr, uint4 v) {
+  asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w) : "memory");
 }
 __device__ __forceinline__ uint32_t lds32(uint32_t addr) {
   uint32_t v;
@@ -268,6 +301,7 @@ struct Smem {
   alignas(1024) unsigned char v[kVStages][kTileBytes];
   unsigned long long bars[40];
   ItemInfo ring[kRing];
+  alignas(16) unsigned long long finc[64];   // F_i (common.cuh), read by the rotation lanes at every exact restart
   uint32_t tmem_base;
 };
 enum Bar {
@@ -289,12 +323,14 @@ struct Params {
   const TileDesc* tiles;
   int oob_row;                       // first row beyond the cache tensor map: TMA zero-fills
   unsigned long long phase_inc[64];  // F_i (common.cuh)
-  float2 step[64];                   // (cos f_i, sin f_i): one-position RoPE step
+  float2 step4[64];                  // (cos 4 f_i, sin 4 f_i): the four-position RoPE step of the rotation lanes
 };
 
 struct Item {
   int t0, ntok, r, idx0, lo, kvh, n_kv, kv_hi, kv_len;
-  int kv_lo, ntok_x[2], n_x[2];
+  int kv_lo, ntok_a, ntok_b, n_a, n_b;
+  __device__ __forceinline__ int ntok_x(int x) const { return x ? ntok_b : ntok_a; }
+  __device__ __forceinline__ int n_x(int x) const { return x ? n_b : n_a; }
 };
 template <int TOK>
 __device__ __forceinline__ Item load_item(const ItemInfo& ii) {
@@ -302,41 +338,58 @@ __device__ __forceinline__ Item load_item(const ItemInfo& ii) {
   it.t0 = ii.t0; it.ntok = ii.ntok; it.r = ii.r; it.idx0 = ii.idx0; it.lo = ii.lo; it.kvh = ii.kvh; it.n_kv = ii.n_kv;
   it.kv_hi = ii.kv_hi; it.kv_len = ii.kv_len;
   it.kv_lo = it.lo & ~(kBlock - 1);
-  it.ntok_x[0] = min(it.ntok, TOK); it.ntok_x[1] = it.ntok - it.ntok_x[0];
-  const int hi_a = min(it.idx0 + it.ntok_x[0], it.kv_len);
-  it.n_x[0] = hi_a > it.kv_lo ? (hi_a - it.kv_lo + BN - 1) / BN : 0;
-  it.n_x[1] = it.ntok_x[1] > 0 ? it.n_kv : 0;
+  it.ntok_a = min(it.ntok, TOK); it.ntok_b = it.ntok - it.ntok_a;
+  const int hi_a = min(it.idx0 + it.ntok_a, it.kv_len);
+  it.n_a = hi_a > it.kv_lo ? (hi_a - it.kv_lo + BN - 1) / BN : 0;
+  it.n_b = it.ntok_b > 0 ? it.n_kv : 0;
   return it;
 }
 
-// RoPE state of one lane: two adjacent frequencies (2*lane, 2*lane+1), cos / sin packed as f32x2
-struct Rot {
-  unsigned long long f0, f1;   // fixed-point phase increments
-  uint64_t c1, s1, ns1;        // one-position step (cos, sin, -sin)
-  uint64_t c, s;
-  __device__ __forceinline__ void restart(int p) {
-    const unsigned long long p0 = (unsigned long long)(unsigned)p * f0, p1 = (unsigned long long)(unsigned)p * f1;
-    const float a0 = (float)(int)(p0 >> 32) * 1.4629180792671596e-9f;   // * pi * 2^-31
-    const float a1 = (float)(int)(p1 >> 32) * 1.4629180792671596e-9f;
-    c = pk2(__cosf(a0), __cosf(a1));
-    s = pk2(__sinf(a0), __sinf(a1));
+// RoPE state of one rotation lane.  A warp covers 4 tile rows per step: lane = (row-in-step = lane >> 3, 16-byte
+// chunk = lane & 7); the lane owns dims [8*chunk, 8*chunk + 8) of both halves of its row, i.e. 8 RoPE pairs (i, i + 64)
+// and 8 frequencies, kept as four packed f32x2 (cos, sin) registers.  One 128-bit shared load / store per half.
+struct Rot8 {
+  uint64_t c[4], s[4];
+  // exact restart at position p: 64-bit fixed-point phase (common.cuh) + MUFU on the reduced angle
+  __device__ __forceinline__ void restart(int p, uint32_t finc_addr) {
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const uint4 f = lds128(finc_addr + 16 * e);   // F of frequencies 2e, 2e + 1 of this lane
+      const unsigned long long f0 = ((unsigned long long)f.y << 32) | f.x, f1 = ((unsigned long long)f.w << 32) | f.z;
+      const unsigned long long p0 = (unsigned long long)(unsigned)p * f0, p1 = (unsigned long long)(unsigned)p * f1;
+      const float a0 = (float)(int)(p0 >> 32) * 1.4629180792671596e-9f;   // * pi * 2^-31
+      const float a1 = (float)(int)(p1 >> 32) * 1.4629180792671596e-9f;
+      c[e] = pk2(__cosf(a0), __cosf(a1));
+      s[e] = pk2(__sinf(a0), __sinf(a1));
+    }
   }
-  __device__ __forceinline__ void advance() {
-    const uint64_t cn = fma2(c, c1, mul2(s, ns1));
-    s = fma2(s, c1, mul2(c, s1));
-    c = cn;
+  // angle-addition step by a fixed position stride: (c, s) <- (c, s) * (cd, sd)
+  __device__ __forceinline__ void advance(const uint64_t (&cd)[4], const uint64_t (&sd)[4], const uint64_t (&nsd)[4]) {
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const uint64_t cn = fma2(c[e], cd[e], mul2(s[e], nsd[e]));
+      s[e] = fma2(s[e], cd[e], mul2(c[e], sd[e]));
+      c[e] = cn;
+    }
   }
-  // rotate the lane's 2+2 elements of one 128-dim row: lo word = dims (2l, 2l+1), hi word = dims (64+2l, 64+2l+1)
+  // rotate the lane's 8 + 8 elements of one 128-dim row in place; addr = the lane's chunk in the low half
   __device__ __forceinline__ void apply(uint32_t addr) const {
-    const uint32_t lo = lds32(addr), hi = lds32(addr + kHalfBytes);
-    const uint64_t a = pk2(bf16lo(lo), bf16hi(lo)), b = pk2(bf16lo(hi), bf16hi(hi));
-    const uint64_t ns = mul2(s, pk2(-1.f, -1.f));
-    const uint64_t an = fma2(a, c, mul2(b, ns));
-    const uint64_t bn = fma2(b, c, mul2(a, s));
-    float x0, x1, y0, y1;
-    upk2(an, x0, x1); upk2(bn, y0, y1);
-    sts32(addr, pack_bf16(x0, x1));
-    sts32(addr + kHalfBytes, pack_bf16(y0, y1));
+    const uint4 lo = lds128(addr), hi = lds128(addr + kHalfBytes);
+    const uint32_t wl[4] = {lo.x, lo.y, lo.z, lo.w}, wh[4] = {hi.x, hi.y, hi.z, hi.w};
+    uint32_t ol[4], oh[4];
+    const uint64_t neg1 = pk2(-1.f, -1.f);
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const uint64_t a = pk2(bf16lo(wl[e]), bf16hi(wl[e])), b = pk2(bf16lo(wh[e]), bf16hi(wh[e]));
+      const uint64_t ns = mul2(s[e], neg1);
+      const uint64_t an = fma2(a, c[e], mul2(b, ns));
+      const uint64_t bn = fma2(b, c[e], mul2(a, s[e]));
+      float x0, x1, y0, y1;
+      upk2(an, x0, x1); upk2(bn, y0, y1);
+      ol[e] = pack_bf16(x0, x1); oh[e] = pack_bf16(y0, y1);
+    }
+    sts128(addr, make_uint4(ol[0], ol[1], ol[2], ol[3]));
+    sts128(addr + kHalfBytes, make_uint4(oh[0], oh[1], oh[2], oh[3]));
   }
 };
 
@@ -353,6 +406,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
   auto bar = [&](int b) { return bar0 + 8u * (uint32_t)b; };
   Waiter w{&prm.hdr->err, false};
 
+  if (threadIdx.x >= 64 && threadIdx.x < 128) sm.finc[threadIdx.x - 64] = prm.phase_inc[threadIdx.x - 64];
   if (threadIdx.x == 0) {
     if (smem_u32(smem_raw) & 1023u) atomicCAS(&prm.hdr->err, 0, 2);   // swizzled tiles need a 1024-byte aligned base
     for (int s = 0; s < kRing; ++s) { mbar_init(bar(SCHED_FULL + s), 1); mbar_init(bar(SCHED_EMPTY + s), 13); }
@@ -376,7 +430,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
   const int n_items = prm.hdr->n_tiles * prm.hkv;
 
   if (warp >= 12) {
-    reg_dec<48>();
+    reg_dec<kRegsCtl>();
     if (warp == 12) {
       // ============================================================ scheduler + TMA producer (a4)
       uint32_t kc = 0, vc = 0, qc = 0;
@@ -465,8 +519,8 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         int n, nx0, nx1, kv_hi;
         {
           const Item it = load_item<TOK>(sm.ring[slot]);
-          n = __shfl_sync(0xffffffffu, it.n_kv, 0); nx0 = __shfl_sync(0xffffffffu, it.n_x[0], 0);
-          nx1 = __shfl_sync(0xffffffffu, it.n_x[1], 0); kv_hi = __shfl_sync(0xffffffffu, it.kv_hi, 0);
+          n = __shfl_sync(0xffffffffu, it.n_kv, 0); nx0 = __shfl_sync(0xffffffffu, it.n_a, 0);
+          nx1 = __shfl_sync(0xffffffffu, it.n_b, 0); kv_hi = __shfl_sync(0xffffffffu, it.kv_hi, 0);
         }
         const bool vfix = (kv_hi & (kBlock - 1)) != 0;
         __syncwarp();
@@ -532,18 +586,20 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
     }
   } else if (warp >= 8) {
     // ============================================================ rotation warps: Q (a3) and K tiles (a5)
-    reg_dec<80>();
+    reg_dec<kRegsRot>();
     const int rw = warp - 8, rot_tid = threadIdx.x - 256;
-    Rot rot;
-    rot.f0 = prm.phase_inc[2 * lane]; rot.f1 = prm.phase_inc[2 * lane + 1];
-    {
-      const float2 s0 = prm.step[2 * lane], s1 = prm.step[2 * lane + 1];
-      rot.c1 = pk2(s0.x, s1.x); rot.s1 = pk2(s0.y, s1.y); rot.ns1 = pk2(-s0.y, -s1.y);
-    }
-    rot.c = 0; rot.s = 0;
-    uint32_t off8[8];   // byte offset of the lane's word inside row (r & 7) of a swizzle atom
+    const int rsub = lane >> 3, ch = lane & 7;
+    Rot8 rot;
+    uint64_t c4[4], s4[4], ns4[4];
 #pragma unroll
-    for (int k = 0; k < 8; ++k) off8[k] = (uint32_t)(k * 128 + (((lane >> 2) ^ k) << 4) + ((lane & 3) << 2));
+    for (int e = 0; e < 4; ++e) {
+      const float2 u0 = prm.step4[8 * ch + 2 * e], u1 = prm.step4[8 * ch + 2 * e + 1];
+      c4[e] = pk2(u0.x, u1.x); s4[e] = pk2(u0.y, u1.y); ns4[e] = pk2(-u0.y, -u1.y);
+    }
+    const uint32_t finc_addr = smem_u32(sm.finc) + 64 * ch;
+    // byte offset of the lane's 16-byte chunk in row (4k + rsub) of a 16-row block: even k / odd k (SWIZZLE_128B)
+    const uint32_t off_e = (uint32_t)(rsub * 128 + ((ch ^ rsub) << 4));
+    const uint32_t off_o = (uint32_t)((4 + rsub) * 128 + ((ch ^ (4 + rsub)) << 4));
     const bool k_prerot = (prm.flags & MINIPIC_K_PREROTATED) != 0, q_prerot = (prm.flags & MINIPIC_Q_PREROTATED) != 0;
     uint32_t kc = 0, vc = 0, qc = 0;
     for (uint32_t it_n = 0;; ++it_n) {
@@ -555,52 +611,58 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       if (lane == 0) mbar_arrive(bar(SCHED_EMPTY + slot));
       if (it.n_kv == 0) continue;
       const int* pos = a.kv_positions + __ldg(a.cu_kv_lens + it.r);
+      // this warp rotates keys [32 rw, 32 rw + 32) of every tile; lane l holds the position of key 32 rw + l
+      int myp = __ldg(pos + min(it.kv_lo + 32 * rw + lane, it.kv_len - 1));
       for (int i = 0; i < it.n_kv; ++i) {
-        // ---- K tile i: every 16-key block restarts the trig recurrence from the exact fixed-point phase
         const int st = kc % kKStages;
-        const int j0 = it.kv_lo + i * BN;
+        const int j0 = it.kv_lo + i * BN + 32 * rw;
+        const int myp_next = (i + 1 < it.n_kv) ? __ldg(pos + min(j0 + BN + lane, it.kv_len - 1)) : 0;
         w.wait(bar(K_FULL + st), (kc / kKStages) & 1);
-        if (!k_prerot) {
-          const int nblk = min(BN / kBlock, (it.kv_hi - j0 + kBlock - 1) / kBlock);
-          const uint32_t kt = smem_u32(sm.k[st]);
-#pragma unroll 1
-          for (int b = 2 * rw; b < 2 * rw + 2; ++b) {
-            if (b >= nblk) break;
-            const int myp = __ldg(pos + min(j0 + b * kBlock + (lane & 15), it.kv_len - 1));
-            int prev = 0;
+        if (!k_prerot && j0 < it.kv_hi) {
+          const uint32_t kt = smem_u32(sm.k[st]) + (uint32_t)rw * 4096;
+          const int nrow = it.kv_hi - j0;                 // rows of this warp's chunk that hold visible keys
+          const int p0 = __shfl_sync(0xffffffffu, myp, 0);
+          if (__all_sync(0xffffffffu, lane >= nrow || myp == p0 + lane)) {
+            // consecutive positions (every workload the paper describes): one exact restart, then 4-position steps
+            rot.restart(p0 + rsub, finc_addr);
 #pragma unroll
-            for (int rr = 0; rr < kBlock; ++rr) {
-              const int p = __shfl_sync(0xffffffffu, myp, rr);
-              if (rr == 0 || p != prev + 1) rot.restart(p); else rot.advance();
-              prev = p;
-              rot.apply(kt + b * 2048 + (rr >> 3) * 1024 + off8[rr & 7]);
+            for (int k = 0; k < 8; ++k) {
+              if (k == 4 && nrow <= 16) break;
+              rot.apply(kt + (k >> 1) * 1024 + ((k & 1) ? off_o : off_e));
+              if (k < 7) rot.advance(c4, s4, ns4);
+            }
+          } else {
+#pragma unroll 1
+            for (int k = 0; k < 8; ++k) {
+              if (4 * k >= nrow) break;
+              rot.restart(__shfl_sync(0xffffffffu, myp, 4 * k + rsub), finc_addr);
+              rot.apply(kt + (k >> 1) * 1024 + ((k & 1) ? off_o : off_e));
             }
           }
         }
         fence_proxy_async();
         mbar_arrive(bar(K_READY + st));
         ++kc;
+        myp = myp_next;
         if (i == 0) {
-          // ---- Q super-tile: row = token * G + head-in-group; G rows share one position
+          // ---- Q super-tile: row = token * G + head-in-group; the G rows of a token share one position
           w.wait(bar(Q_FULL), qc & 1);
           if (!q_prerot) {
-#pragma unroll
+#pragma unroll 1
             for (int x = 0; x < 2; ++x) {
-              if (it.ntok_x[x] <= 0) continue;
-              constexpr int TPW = 32 / G;   // tokens per warp
-              const int tok0 = rw * TPW;
-              const int myp = (tok0 + (lane % TPW) < it.ntok_x[x])
-                                  ? __ldg(pos + min(it.idx0 + x * TOK + tok0 + (lane % TPW), it.kv_len - 1)) : 0;
-              const uint32_t qt = smem_u32(sm.q[x]);
+              if (it.ntok_x(x) <= 0) continue;
+              const uint32_t qt = smem_u32(sm.q[x]) + (uint32_t)rw * 4096;
+              int qp[8];
 #pragma unroll
-              for (int t = 0; t < TPW; ++t) {
-                if (tok0 + t >= it.ntok_x[x]) break;
-                rot.restart(__shfl_sync(0xffffffffu, myp, t));
+              for (int k = 0; k < 8; ++k) {
+                const int tok = (32 * rw + 4 * k + rsub) / G;
+                qp[k] = __ldg(pos + min(it.idx0 + x * TOK + min(tok, it.ntok_x(x) - 1), it.kv_len - 1));
+              }
 #pragma unroll
-                for (int g = 0; g < G; ++g) {
-                  const int r = 32 * rw + t * G + g;
-                  rot.apply(qt + (r >> 3) * 1024 + off8[(t * G + g) & 7]);
-                }
+              for (int k = 0; k < 8; ++k) {
+                if ((32 * rw + 4 * k) / G >= it.ntok_x(x)) break;
+                if (k == 0 || (4 * k) / G != (4 * k - 4) / G || G < 4) rot.restart(qp[k], finc_addr);
+                rot.apply(qt + (k >> 1) * 1024 + ((k & 1) ? off_o : off_e));
               }
             }
           }
@@ -613,7 +675,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         if (i == it.n_kv - 1 && (it.kv_hi & (kBlock - 1)) != 0) {
           const int vs = (vc + i) % kVStages;
           w.wait(bar(V_FULL + vs), ((vc + i) / kVStages) & 1);
-          const int first = it.kv_hi - j0, last = (first + kBlock - 1) & ~(kBlock - 1);
+          const int first = it.kv_hi - (it.kv_lo + i * BN), last = (first + kBlock - 1) & ~(kBlock - 1);
           if (rot_tid >= first && rot_tid < last) {
             const uint32_t vrow = smem_u32(sm.v[vs]) + rot_tid * 128;
 #pragma unroll
@@ -627,7 +689,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
     }
   } else {
     // ============================================================ softmax + epilogue warps (a7, a9): thread = row
-    reg_inc<192>();
+    reg_inc<kRegsSoftmax>();
     const int x = warp >> 2;                 // 0: tile A, 1: tile B
     const int row = threadIdx.x & 127;
     const uint32_t t_lane = tmem + ((uint32_t)((warp & 3) * 32) << 16);
@@ -641,11 +703,11 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       const Item it = load_item<TOK>(sm.ring[slot]);
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(SCHED_EMPTY + slot));
-      const bool row_ok = tok_in < it.ntok_x[x];
+      const bool row_ok = tok_in < it.ntok_x(x);
       const int tok = x * TOK + tok_in;
       const int idx_first = it.idx0 + x * TOK;                       // lowest query index of this tile
       const int idx_row = min(it.idx0 + tok, it.kv_len - 1);         // highest visible key of this row
-      const int n = it.n_x[x];
+      const int n = it.n_x(x);
       float m_used = -INFINITY, l_run = 0.f;   // m in log2 units (score * scale * log2 e)
       for (int i = 0; i < n; ++i, ++sc) {
         const int j0 = it.kv_lo + i * BN;
@@ -676,38 +738,44 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
             // S_FULL(i) was committed after PV(i-1): O is stable until this thread publishes P(i)
             const float corr = grow ? fast_exp2(m_used - m_new) : 1.f;
             if (grow) { l_run *= corr; m_used = m_new; }
-#pragma unroll
-            for (int c = 0; c < 4; ++c) {
-              float o[32];
-              tmem_ld32(t_o + c * 32, o);
+#pragma unroll 1
+            for (int c = 0; c < 8; ++c) {
+              float o[16];
+              tmem_ld16(t_o + c * 16, o);
               tmem_wait_ld();
 #pragma unroll
-              for (int e = 0; e < 32; ++e) o[e] *= corr;
-              tmem_st32(t_o + c * 32, reinterpret_cast<const uint32_t*>(o));
+              for (int e = 0; e < 16; ++e) o[e] *= corr;
+              tmem_st16(t_o + c * 16, reinterpret_cast<const uint32_t*>(o));
             }
           }
         }
         const float m_sub = (m_used == -INFINITY) ? 0.f : m_used;
-        float lsum0 = 0.f, lsum1 = 0.f;
+        const uint64_t sc2 = pk2(prm.scale_log2, prm.scale_log2), nm2 = pk2(-m_sub, -m_sub);
+        uint64_t lsum0 = pk2(0.f, 0.f), lsum1 = lsum0;
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
-          uint32_t pk[32];
+        for (int h = 0; h < 4; ++h) {
+          uint32_t pk[16];
 #pragma unroll
-          for (int c = 0; c < 32; ++c) {
-            const float p0 = fast_exp2(fmaf(s[64 * h + 2 * c], prm.scale_log2, -m_sub));
-            const float p1 = fast_exp2(fmaf(s[64 * h + 2 * c + 1], prm.scale_log2, -m_sub));
-            lsum0 += p0; lsum1 += p1;
+          for (int c = 0; c < 16; ++c) {
+            float x0, x1;
+            upk2(fma2(pk2(s[32 * h + 2 * c], s[32 * h + 2 * c + 1]), sc2, nm2), x0, x1);
+            const float p0 = fast_exp2(x0), p1 = fast_exp2(x1);
+            if (c & 1) lsum1 = add2(lsum1, pk2(p0, p1)); else lsum0 = add2(lsum0, pk2(p0, p1));
             pk[c] = pack_bf16(p0, p1);
           }
-          tmem_st32(t_s + 32 * h, pk);
+          tmem_st16(t_s + 16 * h, pk);
         }
-        l_run += lsum0 + lsum1;
+        {
+          float a0, a1;
+          upk2(add2(lsum0, lsum1), a0, a1);
+          l_run += a0 + a1;
+        }
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(bar(P_FULL + x));
       }
       // ---- epilogue (a9): O / l -> out, LSE = ln sum exp of the scaled scores
-      if (it.ntok_x[x] <= 0) continue;
+      if (it.ntok_x(x) <= 0) continue;
       const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
       __nv_bfloat16* orow = (__nv_bfloat16*)a.out + ((size_t)(it.t0 + tok) * prm.hq + it.kvh * G + hg) * D;
       if (n > 0) { w.wait(bar(O_FULL + x), oc & 1); ++oc; tc_fence_after(); }
@@ -827,7 +895,9 @@ bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
   prm.oob_row = c.num_blocks * c.hkv * kBlock;
   for (int i = 0; i < 64; ++i) {
     prm.phase_inc[i] = c.rope.phase_inc[i];
-    prm.step[i] = make_float2((float)c.rope_step_cos[i], (float)c.rope_step_sin[i]);
+    const double c1 = c.rope_step_cos[i], s1 = c.rope_step_sin[i];
+    const double c2 = c1 * c1 - s1 * s1, s2 = 2.0 * s1 * c1;
+    prm.step4[i] = make_float2((float)(c2 * c2 - s2 * s2), (float)(2.0 * s2 * c2));
   }
   int dev = 0, sms = 148;
   cudaGetDevice(&dev);
