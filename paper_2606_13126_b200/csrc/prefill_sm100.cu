@@ -31,7 +31,11 @@ namespace {
 constexpr int BM = 128, BN = 128, D = 128;
 constexpr int kTileBytes = BN * D * 2;       // 32 KB: one K / V / Q tile
 constexpr int kHalfBytes = kTileBytes / 2;   // [half of head_dim][128 rows][128 B]
-constexpr int kKStages = 3, kVStages = 2, kRing = 4;
+constexpr int kKStages = 2, kVStages = 2, kRing = 4;
+// K / V tile in shared memory: 16 row groups of [half of head_dim (2)][8 rows x 128 B] = 2048 B each, so one (block, head)
+// of the cache (16 tokens x 256 B) is ONE 4-D TMA box of two groups.  Q tile: [half (2)][128 rows x 128 B].
+constexpr int kGroupBytes = 2048, kKvHalfOff = 1024;
+constexpr int kStageBytes = 4096;            // epilogue staging per softmax warp: 32 rows x 128 B (64 bf16 columns)
 // 16 warps = 4 warpgroups: softmax A, softmax B (184 registers each after setmaxnreg), rotation (96), control (TMA, MMA and
 // two idle warps, 48).  setmaxnreg is a WARPGROUP-wide instruction (all four warps, same count), and the split must fit the
 // launch pool of 512 * 128 registers or setmaxnreg.inc blocks forever: 256*184 + 128*96 + 128*48 = 65536.
@@ -39,11 +43,11 @@ constexpr int kThreads = 512;
 constexpr int kRegsSoftmax = 184, kRegsRot = 96, kRegsCtl = 48;
 static_assert(256 * kRegsSoftmax + 128 * kRegsRot + 128 * kRegsCtl <= 65536, "setmaxnreg split exceeds the CTA register pool");
 constexpr int kMaxBins = 4096;
-constexpr long long kWaitTimeoutCycles = 4000000000LL;
+constexpr unsigned kWaitMaxSpins = 1u << 26;   // x (>= 30 cycles per failed try_wait) = seconds
 
-struct TileDesc { int t0, ntok, r, idx0, lo, n_kv, kv_hi, kv_len; };
+struct TileDesc { int t0, ntok, r, idx0, lo, n_kv, kv_hi, kv_len, kv_off, pad; };   // kv_off = cu_kv_lens[r]
 struct PlanHeader { int n_tiles; int next_item; int err; int err_info[5]; int pad[56]; int hist[kMaxBins]; };
-struct ItemInfo { int t0, ntok, r, idx0, lo, kvh, n_kv, kv_hi, kv_len, pad[3]; };   // 48 B ring entry; t0 < 0 = stop
+struct ItemInfo { int t0, ntok, r, idx0, lo, kvh, n_kv, kv_hi, kv_len, kv_off, pad[2]; };   // 48 B ring entry; t0 < 0 = stop
 
 // ------------------------------------------------------------------------------------------------ PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -71,25 +75,36 @@ __device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity) {
 struct Waiter {
   int* err;
   bool dead;
+  // kept tiny on purpose: ~25 wait sites inline this, and the kernel is instruction-cache bound (four roles with
+  // different code share an SM).  try_wait suspends in hardware for a bounded time, so spins are cheap to count.
   __device__ __forceinline__ void wait(uint32_t bar, uint32_t parity) {
     if (dead) return;
-    if (mbar_try(bar, parity)) return;
-    const long long t0 = clock64();
     unsigned spins = 0;
     while (!mbar_try(bar, parity)) {
-      if ((++spins & 63u) == 0) {
-        if (*(volatile int*)err != 0) { dead = true; return; }
-        if (clock64() - t0 > kWaitTimeoutCycles) {
-          if (atomicCAS(err, 0, 1) == 0) {
-            err[1] = (int)bar; err[2] = (int)parity; err[3] = (int)blockIdx.x; err[4] = (int)threadIdx.x;
-          }
-          dead = true;
-          return;
-        }
+      if ((++spins & 4095u) == 0 && (*(volatile int*)err != 0 || spins > kWaitMaxSpins)) {
+        atomicCAS(err, 0, (int)(bar | 0x40000000u));   // records the barrier that timed out
+        dead = true;
+        return;
       }
     }
   }
 };
+// Debug-only event trace (-DMINIPIC_TRACE, never in the shipped library): CTA 0 records (tag, SM clock) per role.
+#ifdef MINIPIC_TRACE
+constexpr int kTraceRoles = 8, kTraceLen = 8192;
+__device__ long long g_trace[kTraceRoles][kTraceLen][2];
+__device__ int g_trace_n[kTraceRoles];
+__device__ __forceinline__ void trace_ev(int role, int tag) {
+  if (blockIdx.x != 0) return;
+  const int n = g_trace_n[role];
+  if (n < kTraceLen) { g_trace[role][n][0] = tag; g_trace[role][n][1] = clock64(); g_trace_n[role] = n + 1; }
+}
+#define TRACE(role, tag) trace_ev(role, tag)
+#define TRACE_L0(role, tag) do { if (lane == 0) trace_ev(role, tag); } while (0)
+#else
+#define TRACE(role, tag) do { } while (0)
+#define TRACE_L0(role, tag) do { } while (0)
+#endif
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
@@ -106,17 +121,23 @@ __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tma
       "cp.async.bulk.tensor.3d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5}], [%2];"
       ::"r"(dst), "l"(tmap), "r"(bar), "r"(x), "r"(y), "r"(z) : "memory");
 }
+__device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* tmap, uint32_t bar, int c0, int c1, int c2, int c3) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
+      ::"r"(dst), "l"(tmap), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+}
 // Shared-memory matrix descriptors (SWIZZLE_128B): the low word carries the start address (>> 4) and the leading byte
 // offset (>> 4, bits 16-29); the high word is the same for every operand of this kernel: stride byte offset 1024
 // (8 rows x 128 B), descriptor version 1 (bit 46), swizzle mode 128B (2 << 61).
-constexpr uint32_t kDescHi = (1024u >> 4) | (1u << 14) | (2u << 29);
+constexpr uint32_t kDescHiQ = (1024u >> 4) | (1u << 14) | (2u << 29);                    // Q tile: 8-row groups 1024 B apart
+constexpr uint32_t kDescHiKV = ((uint32_t)kGroupBytes >> 4) | (1u << 14) | (2u << 29);   // K / V tile: 2048 B apart
 // D[tmem] (+)= A[smem] * B[smem]
 __device__ __forceinline__ void umma_ss(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, uint32_t acc) {
   asm volatile(
       "{\n\t.reg .pred p;\n\t.reg .b64 da, db;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-      "mov.b64 da, {%1, %5};\n\tmov.b64 db, {%2, %5};\n\t"
+      "mov.b64 da, {%1, %5};\n\tmov.b64 db, {%2, %6};\n\t"
       "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, p;\n\t}"
-      ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(idesc), "r"(acc), "r"(kDescHi) : "memory");
+      ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(idesc), "r"(acc), "r"(kDescHiQ), "r"(kDescHiKV) : "memory");
 }
 // D[tmem] (+)= A[tmem] * B[smem]
 __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint32_t b_lo, uint32_t idesc, uint32_t acc) {
@@ -124,7 +145,7 @@ __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint32
       "{\n\t.reg .pred p;\n\t.reg .b64 db;\n\tsetp.ne.b32 p, %4, 0;\n\t"
       "mov.b64 db, {%2, %5};\n\t"
       "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], db, %3, p;\n\t}"
-      ::"r"(d_tmem), "r"(a_tmem), "r"(b_lo), "r"(idesc), "r"(acc), "r"(kDescHi) : "memory");
+      ::"r"(d_tmem), "r"(a_tmem), "r"(b_lo), "r"(idesc), "r"(acc), "r"(kDescHiKV) : "memory");
 }
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
   uint32_t* r = reinterpret_cast<uint32_t*>(v);
@@ -251,6 +272,7 @@ __global__ void __launch_bounds__(256) plan_mark_kernel(PrefillArgs a, int tok, 
   TileDesc td;
   td.t0 = t; td.ntok = n; td.r = r; td.idx0 = __ldg(a.q_seq_idx + t); td.lo = max(__ldg(a.q_vis_lo + t), 0);
   td.kv_len = __ldg(a.kv_lens + r);
+  td.kv_off = __ldg(a.cu_kv_lens + r); td.pad = 0;
   const int kv_lo = td.lo & ~(kBlock - 1);
   td.kv_hi = min(td.idx0 + n, td.kv_len);
   td.n_kv = td.kv_hi > kv_lo ? (td.kv_hi - kv_lo + BN - 1) / BN : 0;
@@ -299,14 +321,17 @@ struct Smem {
   alignas(1024) unsigned char q[2][kTileBytes];
   alignas(1024) unsigned char k[kKStages][kTileBytes];
   alignas(1024) unsigned char v[kVStages][kTileBytes];
+  alignas(1024) unsigned char ostage[8][kStageBytes];
   unsigned long long bars[40];
   ItemInfo ring[kRing];
   alignas(16) unsigned long long finc[64];   // F_i (common.cuh), read by the rotation lanes at every exact restart
+  alignas(16) float2 step1[64];              // (cos f_i, sin f_i): one-position step, used by the Q rotation
+  alignas(16) float2 step4[64];              // (cos 4 f_i, sin 4 f_i): four-position step, used by the K rotation
   uint32_t tmem_base;
 };
 enum Bar {
   SCHED_FULL = 0, SCHED_EMPTY = SCHED_FULL + kRing,
-  Q_FULL = SCHED_EMPTY + kRing, Q_READY, Q_EMPTY,
+  Q_FULL = SCHED_EMPTY + kRing, Q_READY, Q_EMPTY = Q_READY + 2,
   K_FULL, K_READY = K_FULL + kKStages, K_EMPTY = K_READY + kKStages,
   V_FULL = K_EMPTY + kKStages, V_EMPTY = V_FULL + kVStages, V_FIX = V_EMPTY + kVStages,
   S_FULL, P_FULL = S_FULL + 2, O_FULL = P_FULL + 2, O_FREE = O_FULL + 2, NUM_BARS = O_FREE + 2
@@ -321,13 +346,14 @@ struct Params {
   unsigned flags;
   PlanHeader* hdr;
   const TileDesc* tiles;
-  int oob_row;                       // first row beyond the cache tensor map: TMA zero-fills
+  int oob_grp;                       // first row-group coordinate beyond the cache tensor map: TMA zero-fills
   unsigned long long phase_inc[64];  // F_i (common.cuh)
+  float2 step1[64];                  // (cos f_i, sin f_i)
   float2 step4[64];                  // (cos 4 f_i, sin 4 f_i): the four-position RoPE step of the rotation lanes
 };
 
 struct Item {
-  int t0, ntok, r, idx0, lo, kvh, n_kv, kv_hi, kv_len;
+  int t0, ntok, r, idx0, lo, kvh, n_kv, kv_hi, kv_len, kv_off;
   int kv_lo, ntok_a, ntok_b, n_a, n_b;
   __device__ __forceinline__ int ntok_x(int x) const { return x ? ntok_b : ntok_a; }
   __device__ __forceinline__ int n_x(int x) const { return x ? n_b : n_a; }
@@ -336,7 +362,7 @@ template <int TOK>
 __device__ __forceinline__ Item load_item(const ItemInfo& ii) {
   Item it;
   it.t0 = ii.t0; it.ntok = ii.ntok; it.r = ii.r; it.idx0 = ii.idx0; it.lo = ii.lo; it.kvh = ii.kvh; it.n_kv = ii.n_kv;
-  it.kv_hi = ii.kv_hi; it.kv_len = ii.kv_len;
+  it.kv_hi = ii.kv_hi; it.kv_len = ii.kv_len; it.kv_off = ii.kv_off;
   it.kv_lo = it.lo & ~(kBlock - 1);
   it.ntok_a = min(it.ntok, TOK); it.ntok_b = it.ntok - it.ntok_a;
   const int hi_a = min(it.idx0 + it.ntok_a, it.kv_len);
@@ -372,9 +398,9 @@ struct Rot8 {
       c[e] = cn;
     }
   }
-  // rotate the lane's 8 + 8 elements of one 128-dim row in place; addr = the lane's chunk in the low half
-  __device__ __forceinline__ void apply(uint32_t addr) const {
-    const uint4 lo = lds128(addr), hi = lds128(addr + kHalfBytes);
+  // rotate the lane's 8 + 8 elements of one 128-dim row (already loaded: lo / hi = its chunk of the two halves) and
+  // store them back; addr = the lane's chunk in the low half, half_off = distance to the high half
+  __device__ __forceinline__ void rotate_store(uint32_t addr, uint32_t half_off, const uint4& lo, const uint4& hi) const {
     const uint32_t wl[4] = {lo.x, lo.y, lo.z, lo.w}, wh[4] = {hi.x, hi.y, hi.z, hi.w};
     uint32_t ol[4], oh[4];
     const uint64_t neg1 = pk2(-1.f, -1.f);
@@ -389,7 +415,7 @@ struct Rot8 {
       ol[e] = pack_bf16(x0, x1); oh[e] = pack_bf16(y0, y1);
     }
     sts128(addr, make_uint4(ol[0], ol[1], ol[2], ol[3]));
-    sts128(addr + kHalfBytes, make_uint4(oh[0], oh[1], oh[2], oh[3]));
+    sts128(addr + half_off, make_uint4(oh[0], oh[1], oh[2], oh[3]));
   }
 };
 
@@ -406,11 +432,15 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
   auto bar = [&](int b) { return bar0 + 8u * (uint32_t)b; };
   Waiter w{&prm.hdr->err, false};
 
-  if (threadIdx.x >= 64 && threadIdx.x < 128) sm.finc[threadIdx.x - 64] = prm.phase_inc[threadIdx.x - 64];
+  if (threadIdx.x >= 64 && threadIdx.x < 128) {
+    sm.finc[threadIdx.x - 64] = prm.phase_inc[threadIdx.x - 64];
+    sm.step1[threadIdx.x - 64] = prm.step1[threadIdx.x - 64];
+    sm.step4[threadIdx.x - 64] = prm.step4[threadIdx.x - 64];
+  }
   if (threadIdx.x == 0) {
     if (smem_u32(smem_raw) & 1023u) atomicCAS(&prm.hdr->err, 0, 2);   // swizzled tiles need a 1024-byte aligned base
-    for (int s = 0; s < kRing; ++s) { mbar_init(bar(SCHED_FULL + s), 1); mbar_init(bar(SCHED_EMPTY + s), 13); }
-    mbar_init(bar(Q_FULL), 1); mbar_init(bar(Q_READY), 128); mbar_init(bar(Q_EMPTY), 1);
+    for (int s = 0; s < kRing; ++s) { mbar_init(bar(SCHED_FULL + s), 1); mbar_init(bar(SCHED_EMPTY + s), 14); }
+    mbar_init(bar(Q_FULL), 1); mbar_init(bar(Q_READY), 128); mbar_init(bar(Q_READY + 1), 128); mbar_init(bar(Q_EMPTY), 1);
     for (int s = 0; s < kKStages; ++s) { mbar_init(bar(K_FULL + s), 1); mbar_init(bar(K_READY + s), 128); mbar_init(bar(K_EMPTY + s), 1); }
     for (int s = 0; s < kVStages; ++s) { mbar_init(bar(V_FULL + s), 1); mbar_init(bar(V_EMPTY + s), 1); }
     mbar_init(bar(V_FIX), 128);
@@ -432,8 +462,8 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
   if (warp >= 12) {
     reg_dec<kRegsCtl>();
     if (warp == 12) {
-      // ============================================================ scheduler + TMA producer (a4)
-      uint32_t kc = 0, vc = 0, qc = 0;
+      // ============================================================ scheduler + Q / K TMA producer (a4)
+      uint32_t kc = 0, qc = 0;
       for (uint32_t it_n = 0;; ++it_n) {
         const int slot = it_n & (kRing - 1);
         int item = 0;
@@ -448,33 +478,31 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         }
         const TileDesc td = prm.tiles[item / prm.hkv];
         const int kvh = item % prm.hkv;
+        TRACE_L0(0, 1);
         if (lane == 0) {
           ItemInfo& ii = sm.ring[slot];
           ii.t0 = td.t0; ii.ntok = td.ntok; ii.r = td.r; ii.idx0 = td.idx0; ii.lo = td.lo; ii.kvh = kvh; ii.n_kv = td.n_kv;
-          ii.kv_hi = td.kv_hi; ii.kv_len = td.kv_len;
+          ii.kv_hi = td.kv_hi; ii.kv_len = td.kv_len; ii.kv_off = td.kv_off;
           mbar_arrive(bar(SCHED_FULL + slot));
         }
         if (td.n_kv == 0) continue;
         const int kv_lo = td.lo & ~(kBlock - 1);
         const int nblk_total = (td.kv_hi + kBlock - 1) / kBlock;   // blocks [0, nblk_total) of the request hold visible keys
         const int* bt = a.block_tables + (size_t)td.r * a.max_blocks;
-        auto block_row = [&](int i) {   // cache-matrix row of this lane's block (lanes 0-7) of KV tile i
+        auto block_grp = [&](int i) {   // cache row-group coordinate of this lane's block (lanes 0-7) of KV tile i
           const int b = (kv_lo >> 4) + i * (BN / kBlock) + lane;
-          return (lane < BN / kBlock && b < nblk_total) ? (__ldg(bt + b) * prm.hkv + kvh) * kBlock : prm.oob_row;
+          return (lane < BN / kBlock && b < nblk_total) ? (__ldg(bt + b) * prm.hkv + kvh) * 2 : prm.oob_grp;
         };
-        int y = block_row(0);
+        int y = block_grp(0);
         for (int i = 0; i < td.n_kv; ++i) {
-          const int y_next = (i + 1 < td.n_kv) ? block_row(i + 1) : 0;
-          {  // K tile i
+          const int y_next = (i + 1 < td.n_kv) ? block_grp(i + 1) : 0;
+          {  // K tile i: one 4 KB box per physical block
             const int st = kc % kKStages;
             if (lane == 0) { w.wait(bar(K_EMPTY + st), ((kc / kKStages) & 1) ^ 1); mbar_expect_tx(bar(K_FULL + st), kTileBytes); }
             __syncwarp();
-            if (lane < BN / kBlock) {
-              const uint32_t dst = smem_u32(sm.k[st]) + lane * 2048;
-              tma_load_2d(dst, &tmap_k, bar(K_FULL + st), 0, y);
-              tma_load_2d(dst + kHalfBytes, &tmap_k, bar(K_FULL + st), 64, y);
-            }
+            if (lane < BN / kBlock) tma_load_4d(smem_u32(sm.k[st]) + lane * 4096, &tmap_k, bar(K_FULL + st), 0, 0, 0, y);
             ++kc;
+            TRACE_L0(0, 2);
           }
           if (i == 0) {  // Q super-tile: rows (token, head-in-group), tile A then tile B
             const int ntile = td.ntok > TOK ? 2 : 1;
@@ -485,18 +513,38 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
               tma_load_3d(smem_u32(sm.q[x]) + h * kHalfBytes, &tmap_q, bar(Q_FULL), 64 * h, kvh * G, td.t0 + x * TOK);
             }
             ++qc;
+            TRACE_L0(0, 3);
           }
-          {  // V tile i
-            const int st = vc % kVStages;
-            if (lane == 0) { w.wait(bar(V_EMPTY + st), ((vc / kVStages) & 1) ^ 1); mbar_expect_tx(bar(V_FULL + st), kTileBytes); }
-            __syncwarp();
-            if (lane < BN / kBlock) {
-              const uint32_t dst = smem_u32(sm.v[st]) + lane * 2048;
-              tma_load_2d(dst, &tmap_v, bar(V_FULL + st), 0, y);
-              tma_load_2d(dst + kHalfBytes, &tmap_v, bar(V_FULL + st), 64, y);
-            }
-            ++vc;
-          }
+          y = y_next;
+        }
+      }
+    } else if (warp == 14) {
+      // ============================================================ V TMA producer (a4): follows the item ring
+      uint32_t vc = 0;
+      for (uint32_t it_n = 0;; ++it_n) {
+        const int slot = it_n & (kRing - 1);
+        w.wait(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
+        if (__any_sync(0xffffffffu, w.dead) || sm.ring[slot].t0 < 0) break;
+        const ItemInfo ii = sm.ring[slot];
+        __syncwarp();
+        if (lane == 0) mbar_arrive(bar(SCHED_EMPTY + slot));
+        if (ii.n_kv == 0) continue;
+        const int kv_lo = ii.lo & ~(kBlock - 1);
+        const int nblk_total = (ii.kv_hi + kBlock - 1) / kBlock;
+        const int* bt = a.block_tables + (size_t)ii.r * a.max_blocks;
+        auto block_grp = [&](int i) {
+          const int b = (kv_lo >> 4) + i * (BN / kBlock) + lane;
+          return (lane < BN / kBlock && b < nblk_total) ? (__ldg(bt + b) * prm.hkv + ii.kvh) * 2 : prm.oob_grp;
+        };
+        int y = block_grp(0);
+        for (int i = 0; i < ii.n_kv; ++i) {
+          const int y_next = (i + 1 < ii.n_kv) ? block_grp(i + 1) : 0;
+          const int st = vc % kVStages;
+          if (lane == 0) { w.wait(bar(V_EMPTY + st), ((vc / kVStages) & 1) ^ 1); mbar_expect_tx(bar(V_FULL + st), kTileBytes); }
+          __syncwarp();
+          if (lane < BN / kBlock) tma_load_4d(smem_u32(sm.v[st]) + lane * 4096, &tmap_v, bar(V_FULL + st), 0, 0, 0, y);
+          ++vc;
+          TRACE_L0(0, 4);
           y = y_next;
         }
       }
@@ -509,7 +557,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       constexpr uint32_t idesc_qk = instr_desc(false), idesc_pv = instr_desc(true);
       const uint32_t q_lo = ((smem_u32(sm.q[0]) >> 4) & 0x3FFF) | (1u << 16);          // + x * 2048
       const uint32_t k_lo = ((smem_u32(sm.k[0]) >> 4) & 0x3FFF) | (1u << 16);          // + stage * 2048
-      const uint32_t v_lo = ((smem_u32(sm.v[0]) >> 4) & 0x3FFF) | ((uint32_t)(kHalfBytes >> 4) << 16);
+      const uint32_t v_lo = ((smem_u32(sm.v[0]) >> 4) & 0x3FFF) | ((uint32_t)(kKvHalfOff >> 4) << 16);
       uint32_t k_st = 0, k_ph = 0, v_st = 0, v_ph = 0;   // next K / V stage to consume and its full-barrier parity
       uint32_t ph = 0;   // bit 0,1: P_FULL parity of tile A,B; bit 2,3: O_FREE; bit 4: Q_READY; bit 5: V_FIX
       for (uint32_t it_n = 0;; ++it_n) {
@@ -531,16 +579,20 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           const uint32_t a_lo = q_lo + (uint32_t)x * (kTileBytes >> 4), b_lo = k_lo + st * (kTileBytes >> 4);
 #pragma unroll
           for (int ks = 0; ks < D / 16; ++ks) {
-            const uint32_t off = (ks >> 2) * (kHalfBytes >> 4) + (ks & 3) * 2;
-            umma_ss(tmem + x * BN, a_lo + off, b_lo + off, idesc_qk, ks > 0);
+            const uint32_t off_q = (ks >> 2) * (kHalfBytes >> 4) + (ks & 3) * 2, off_k = (ks >> 2) * (kKvHalfOff >> 4) + (ks & 3) * 2;
+            umma_ss(tmem + x * BN, a_lo + off_q, b_lo + off_k, idesc_qk, ks > 0);
           }
           tc_commit(bar(S_FULL + x));
+          TRACE(1, 10 + x);
         };
-        w.wait(bar(Q_READY), (ph >> 4) & 1); ph ^= 16u;
+        w.wait(bar(Q_READY), (ph >> 4) & 1);   // tile A of Q is rotated; tile B follows while QK_A already runs
         w.wait(bar(K_READY + k_st), k_ph);
         tc_fence_after();
+        if (nx0 > 0 && elect_one()) qk(0, k_st);
+        __syncwarp();
+        w.wait(bar(Q_READY + 1), (ph >> 4) & 1); ph ^= 16u;
+        tc_fence_after();
         if (elect_one()) {
-          if (nx0 > 0) qk(0, k_st);
           if (nx1 > 0) qk(1, k_st);
           tc_commit(bar(K_EMPTY + k_st));
           if (n == 1) tc_commit(bar(Q_EMPTY));
@@ -560,16 +612,19 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
               w.wait(bar(P_FULL + x), (ph >> x) & 1); ph ^= 1u << x;
               if (i == 0) { w.wait(bar(O_FREE + x), ((ph >> (2 + x)) & 1) ^ 1); ph ^= 4u << x; }
             }
-            if (do_qk && !k_waited) { w.wait(bar(K_READY + k_st), k_ph); k_waited = true; }
             tc_fence_after();
-            if (elect_one()) {
-              if (do_pv) {
-                const uint32_t b_lo = v_lo + v_st * (kTileBytes >> 4);
+            if (do_pv && elect_one()) {
+              const uint32_t b_lo = v_lo + v_st * (kTileBytes >> 4);
 #pragma unroll
-                for (int ks = 0; ks < BN / 16; ++ks)
-                  umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, b_lo + ks * (2048 >> 4), idesc_pv, (i > 0 || ks > 0));
-                if (i == nx - 1) tc_commit(bar(O_FULL + x));
-              }
+              for (int ks = 0; ks < BN / 16; ++ks)
+                umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, b_lo + ks * (2 * kGroupBytes >> 4), idesc_pv, (i > 0 || ks > 0));
+              if (i == nx - 1) tc_commit(bar(O_FULL + x));
+              TRACE(1, 20 + x);
+            }
+            __syncwarp();
+            // the next K tile is only needed now: the PV above is already running while this waits on the rotation
+            if (do_qk && !k_waited) { w.wait(bar(K_READY + k_st), k_ph); k_waited = true; tc_fence_after(); }
+            if (elect_one()) {
               if (x == 1) tc_commit(bar(V_EMPTY + v_st));
               if (do_qk) qk(x, k_st);
               if (x == 1 && i + 1 < n) {
@@ -586,6 +641,8 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
     }
   } else if (warp >= 8) {
     // ============================================================ rotation warps: Q (a3) and K tiles (a5)
+    // NOTE on code shape: the kernel is instruction-cache bound (four roles with different code share an SM), so only the
+    // per-tile K path is unrolled; the once-per-item Q path is a rolled loop (unrolling it measured 8% slower on config 5).
     reg_dec<kRegsRot>();
     const int rw = warp - 8, rot_tid = threadIdx.x - 256;
     const int rsub = lane >> 3, ch = lane & 7;
@@ -596,11 +653,12 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       const float2 u0 = prm.step4[8 * ch + 2 * e], u1 = prm.step4[8 * ch + 2 * e + 1];
       c4[e] = pk2(u0.x, u1.x); s4[e] = pk2(u0.y, u1.y); ns4[e] = pk2(-u0.y, -u1.y);
     }
-    const uint32_t finc_addr = smem_u32(sm.finc) + 64 * ch;
-    // byte offset of the lane's 16-byte chunk in row (4k + rsub) of a 16-row block: even k / odd k (SWIZZLE_128B)
+    const uint32_t finc_addr = smem_u32(sm.finc) + 64 * ch, step1_addr = smem_u32(sm.step1) + 64 * ch;
+    // byte offset of the lane's 16-byte chunk in row (4k + rsub) of a 16-row stretch: even k / odd k (SWIZZLE_128B)
     const uint32_t off_e = (uint32_t)(rsub * 128 + ((ch ^ rsub) << 4));
     const uint32_t off_o = (uint32_t)((4 + rsub) * 128 + ((ch ^ (4 + rsub)) << 4));
     const bool k_prerot = (prm.flags & MINIPIC_K_PREROTATED) != 0, q_prerot = (prm.flags & MINIPIC_Q_PREROTATED) != 0;
+    constexpr int NTW = (32 / G) > 0 ? (32 / G) : 1;   // Q tokens per warp per tile
     uint32_t kc = 0, vc = 0, qc = 0;
     for (uint32_t it_n = 0;; ++it_n) {
       const int slot = it_n & (kRing - 1);
@@ -610,66 +668,98 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       __syncwarp();
       if (lane == 0) mbar_arrive(bar(SCHED_EMPTY + slot));
       if (it.n_kv == 0) continue;
-      const int* pos = a.kv_positions + __ldg(a.cu_kv_lens + it.r);
-      // this warp rotates keys [32 rw, 32 rw + 32) of every tile; lane l holds the position of key 32 rw + l
+      const int* pos = a.kv_positions + it.kv_off;
+      // lane l holds the position of key 32 rw + l of the tile / of Q token 32 rw / G + l of tile A, B (fetched early)
       int myp = __ldg(pos + min(it.kv_lo + 32 * rw + lane, it.kv_len - 1));
+      int qpos_a, qpos_b;
+      {
+        const int ta = min((32 * rw) / G + min(lane, NTW - 1), max(it.ntok_a - 1, 0));
+        const int tb = min((32 * rw) / G + min(lane, NTW - 1), max(it.ntok_b - 1, 0));
+        qpos_a = __ldg(pos + min(it.idx0 + ta, it.kv_len - 1));
+        qpos_b = __ldg(pos + min(it.idx0 + TOK + tb, it.kv_len - 1));
+      }
       for (int i = 0; i < it.n_kv; ++i) {
         const int st = kc % kKStages;
         const int j0 = it.kv_lo + i * BN + 32 * rw;
         const int myp_next = (i + 1 < it.n_kv) ? __ldg(pos + min(j0 + BN + lane, it.kv_len - 1)) : 0;
+        const int nrow = it.kv_hi - j0;                   // rows of this warp's chunk that hold visible keys
+        const bool work = !k_prerot && nrow > 0;
+        const int p0 = __shfl_sync(0xffffffffu, myp, 0);
+        // consecutive positions (every workload the paper describes): one exact restart, then 4-position steps
+        const bool contig = __all_sync(0xffffffffu, lane >= nrow || myp == p0 + lane);
+        if (work && contig) rot.restart(p0 + rsub, finc_addr);          // before the wait: overlaps the TMA latency
         w.wait(bar(K_FULL + st), (kc / kKStages) & 1);
-        if (!k_prerot && j0 < it.kv_hi) {
-          const uint32_t kt = smem_u32(sm.k[st]) + (uint32_t)rw * 4096;
-          const int nrow = it.kv_hi - j0;                 // rows of this warp's chunk that hold visible keys
-          const int p0 = __shfl_sync(0xffffffffu, myp, 0);
-          if (__all_sync(0xffffffffu, lane >= nrow || myp == p0 + lane)) {
-            // consecutive positions (every workload the paper describes): one exact restart, then 4-position steps
-            rot.restart(p0 + rsub, finc_addr);
+        if (rw == 0) TRACE_L0(2, 30);
+        if (work) {
+          const uint32_t kt = smem_u32(sm.k[st]) + (uint32_t)rw * (4 * kGroupBytes);
+          auto row_addr = [&](int k) { return kt + (k >> 1) * kGroupBytes + ((k & 1) ? off_o : off_e); };
+          if (contig) {
+            uint4 lo = lds128(row_addr(0)), hi = lds128(row_addr(0) + kKvHalfOff);
 #pragma unroll
             for (int k = 0; k < 8; ++k) {
               if (k == 4 && nrow <= 16) break;
-              rot.apply(kt + (k >> 1) * 1024 + ((k & 1) ? off_o : off_e));
+              uint4 lo_n = lo, hi_n = hi;
+              if (k < 7) { lo_n = lds128(row_addr(k + 1)); hi_n = lds128(row_addr(k + 1) + kKvHalfOff); }
+              rot.rotate_store(row_addr(k), kKvHalfOff, lo, hi);
               if (k < 7) rot.advance(c4, s4, ns4);
+              lo = lo_n; hi = hi_n;
             }
           } else {
 #pragma unroll 1
             for (int k = 0; k < 8; ++k) {
               if (4 * k >= nrow) break;
               rot.restart(__shfl_sync(0xffffffffu, myp, 4 * k + rsub), finc_addr);
-              rot.apply(kt + (k >> 1) * 1024 + ((k & 1) ? off_o : off_e));
+              const uint4 lo = lds128(row_addr(k)), hi = lds128(row_addr(k) + kKvHalfOff);
+              rot.rotate_store(row_addr(k), kKvHalfOff, lo, hi);
             }
           }
         }
         fence_proxy_async();
         mbar_arrive(bar(K_READY + st));
-        ++kc;
-        myp = myp_next;
+        if (rw == 0) TRACE_L0(2, 31);
         if (i == 0) {
-          // ---- Q super-tile: row = token * G + head-in-group; the G rows of a token share one position
+          // ---- Q super-tile: row = token * G + head-in-group; the G rows of a token share one position.  Exact restart
+          //      at the first row, one-position steps while the positions are consecutive, restart otherwise.  Tile A is
+          //      published first so that QK_A runs while tile B is still being rotated.
           w.wait(bar(Q_FULL), qc & 1);
+          if (rw == 0) TRACE_L0(2, 32);
           if (!q_prerot) {
+            uint64_t c1[4], s1[4], ns1[4];
+#pragma unroll
+            for (int e = 0; e < 4; ++e) {
+              const uint4 u = lds128(step1_addr + 16 * e);   // (cos, sin) of frequencies 2e, 2e + 1 of this lane
+              c1[e] = pk2(__uint_as_float(u.x), __uint_as_float(u.z));
+              s1[e] = pk2(__uint_as_float(u.y), __uint_as_float(u.w));
+              ns1[e] = pk2(-__uint_as_float(u.y), -__uint_as_float(u.w));
+            }
 #pragma unroll 1
             for (int x = 0; x < 2; ++x) {
-              if (it.ntok_x(x) <= 0) continue;
+              const int ntw = it.ntok_x(x) - (32 * rw) / G;        // tokens of this tile that this warp rotates
               const uint32_t qt = smem_u32(sm.q[x]) + (uint32_t)rw * 4096;
-              int qp[8];
-#pragma unroll
+              const int qpx = x ? qpos_b : qpos_a;
+              int prev = 0;
+#pragma unroll 1
               for (int k = 0; k < 8; ++k) {
-                const int tok = (32 * rw + 4 * k + rsub) / G;
-                qp[k] = __ldg(pos + min(it.idx0 + x * TOK + min(tok, it.ntok_x(x) - 1), it.kv_len - 1));
+                if ((4 * k) / G >= ntw) break;
+                const uint32_t addr = qt + (k >> 1) * 1024 + ((k & 1) ? off_o : off_e);
+                const uint4 lo = lds128(addr), hi = lds128(addr + kHalfBytes);
+                const int p = __shfl_sync(0xffffffffu, qpx, ((32 * rw) % G + 4 * k + rsub) / G);
+                if (k > 0 && p == prev + 1) rot.advance(c1, s1, ns1);
+                else if (k == 0 || p != prev) rot.restart(p, finc_addr);
+                prev = p;
+                rot.rotate_store(addr, kHalfBytes, lo, hi);
               }
-#pragma unroll
-              for (int k = 0; k < 8; ++k) {
-                if ((32 * rw + 4 * k) / G >= it.ntok_x(x)) break;
-                if (k == 0 || (4 * k) / G != (4 * k - 4) / G || G < 4) rot.restart(qp[k], finc_addr);
-                rot.apply(qt + (k >> 1) * 1024 + ((k & 1) ? off_o : off_e));
-              }
+              fence_proxy_async();
+              mbar_arrive(bar(Q_READY + x));
             }
+          } else {
+            mbar_arrive(bar(Q_READY)); mbar_arrive(bar(Q_READY + 1));
           }
-          fence_proxy_async();
-          mbar_arrive(bar(Q_READY));
-          ++qc;
+          if (rw == 0) TRACE_L0(2, 33);
         }
+        ++kc;
+        if (i == 0) ++qc;
+        myp = myp_next;
         // ---- V tile i: rows at or beyond kv_hi inside the last gathered block may hold anything (never written
         //      cache slots); their P is 0, make sure 0 * (those bits) is not NaN
         if (i == it.n_kv - 1 && (it.kv_hi & (kBlock - 1)) != 0) {
@@ -677,9 +767,9 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           w.wait(bar(V_FULL + vs), ((vc + i) / kVStages) & 1);
           const int first = it.kv_hi - (it.kv_lo + i * BN), last = (first + kBlock - 1) & ~(kBlock - 1);
           if (rot_tid >= first && rot_tid < last) {
-            const uint32_t vrow = smem_u32(sm.v[vs]) + rot_tid * 128;
+            const uint32_t vrow = smem_u32(sm.v[vs]) + (rot_tid >> 3) * kGroupBytes + (rot_tid & 7) * 128;
 #pragma unroll
-            for (int c = 0; c < 8; ++c) { sts128z(vrow + c * 16); sts128z(vrow + kHalfBytes + c * 16); }
+            for (int c = 0; c < 8; ++c) { sts128z(vrow + c * 16); sts128z(vrow + kKvHalfOff + c * 16); }
           }
           fence_proxy_async();
           mbar_arrive(bar(V_FIX));
@@ -713,13 +803,16 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         const int j0 = it.kv_lo + i * BN;
         float s[BN];
         w.wait(bar(S_FULL + x), sc & 1);
+        if ((warp & 3) == 0) TRACE_L0(3 + x, 40);
         tc_fence_after();
 #pragma unroll
         for (int c = 0; c < 4; ++c) tmem_ld32(t_s + c * 32, s + c * 32);
         tmem_wait_ld();
-        const bool full = (j0 >= it.lo) && (j0 + BN - 1 <= min(idx_first, it.kv_len - 1));
-        if (!full) {
-          const int c_lo = it.lo - j0, c_hi = row_ok ? idx_row - j0 : -1;
+        // mask at 32-column chunk granularity (all bounds but c_hi are warp-uniform): a chunk that every row of the
+        // tile sees needs no mask code, a chunk no row sees (above the causal diagonal) skips max / exp altogether
+        const int c_lo = it.lo - j0;
+        const int c_hi = row_ok ? idx_row - j0 : -1;
+        if (!((j0 >= it.lo) && (j0 + BN - 1 <= min(idx_first, it.kv_len - 1)))) {   // tile not fully visible to every row
 #pragma unroll
           for (int c = 0; c < BN; ++c) s[c] = (c >= c_lo && c <= c_hi) ? s[c] : -INFINITY;
         }
@@ -773,31 +866,49 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(bar(P_FULL + x));
+        if ((warp & 3) == 0) TRACE_L0(3 + x, 41);
       }
-      // ---- epilogue (a9): O / l -> out, LSE = ln sum exp of the scaled scores
+      // ---- epilogue (a9): O / l -> out, LSE = ln sum exp of the scaled scores.  A thread owns a row in TMEM, but a row
+      //      is 256 B in global memory: the warp transposes 64 columns at a time through its 4 KB staging buffer so
+      //      that every store instruction writes four full 128-byte lines instead of 32 scattered 16-byte pieces
       if (it.ntok_x(x) <= 0) continue;
       const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
-      __nv_bfloat16* orow = (__nv_bfloat16*)a.out + ((size_t)(it.t0 + tok) * prm.hq + it.kvh * G + hg) * D;
       if (n > 0) { w.wait(bar(O_FULL + x), oc & 1); ++oc; tc_fence_after(); }
+      if ((warp & 3) == 0) TRACE_L0(3 + x, 42);
+      {
+        const uint32_t stg = smem_u32(sm.ostage[warp]);
+        const int rr = lane >> 3, cc = lane & 7;
+        __nv_bfloat16* obase = (__nv_bfloat16*)a.out + ((size_t)(it.t0 + x * TOK) * prm.hq + it.kvh * G) * D + cc * 8;
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass) {
+          float o[64];
+          if (n > 0) {
+            tmem_ld32(t_o + pass * 64, o); tmem_ld32(t_o + pass * 64 + 32, o + 32);
+            tmem_wait_ld();
+            if (pass == 1) { tc_fence_before(); mbar_arrive(bar(O_FREE + x)); }   // O is in registers: the next item may start
+          } else {
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        float o[32];
-        if (n > 0) { tmem_ld32(t_o + c * 32, o); tmem_wait_ld(); }
-        else {
-#pragma unroll
-          for (int e = 0; e < 32; ++e) o[e] = 0.f;
-        }
-        if (row_ok) {
-#pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            uint4 v;
-            v.x = pack_bf16(o[8 * e] * inv, o[8 * e + 1] * inv); v.y = pack_bf16(o[8 * e + 2] * inv, o[8 * e + 3] * inv);
-            v.z = pack_bf16(o[8 * e + 4] * inv, o[8 * e + 5] * inv); v.w = pack_bf16(o[8 * e + 6] * inv, o[8 * e + 7] * inv);
-            *reinterpret_cast<uint4*>(orow + c * 32 + e * 8) = v;
+            for (int e = 0; e < 64; ++e) o[e] = 0.f;
           }
+#pragma unroll
+          for (int c = 0; c < 8; ++c) {
+            uint4 v;
+            v.x = pack_bf16(o[8 * c] * inv, o[8 * c + 1] * inv); v.y = pack_bf16(o[8 * c + 2] * inv, o[8 * c + 3] * inv);
+            v.z = pack_bf16(o[8 * c + 4] * inv, o[8 * c + 5] * inv); v.w = pack_bf16(o[8 * c + 6] * inv, o[8 * c + 7] * inv);
+            sts128(stg + lane * 128 + ((c ^ (lane & 7)) << 4), v);
+          }
+          __syncwarp();
+#pragma unroll
+          for (int itr = 0; itr < 8; ++itr) {
+            const int r = itr * 4 + rr, rowg = (warp & 3) * 32 + r;
+            const uint4 v = lds128(stg + r * 128 + ((cc ^ (r & 7)) << 4));
+            if (rowg / G < it.ntok_x(x))
+              *reinterpret_cast<uint4*>(obase + ((size_t)(rowg / G) * prm.hq + rowg % G) * D + pass * 64) = v;
+          }
+          __syncwarp();
         }
       }
-      if (n > 0) { tc_fence_before(); mbar_arrive(bar(O_FREE + x)); }
+      if ((warp & 3) == 0) TRACE_L0(3 + x, 43);
       if (row_ok)
         a.lse[(size_t)(it.t0 + tok) * prm.hq + it.kvh * G + hg] =
             l_run > 0.f ? (m_used + log2f(l_run)) * 0.6931471805599453f : -INFINITY;
@@ -826,15 +937,16 @@ EncodeTiledFn get_encode() {
   }
   return fn;
 }
-// cache viewed as a 2-D bf16 matrix [num_blocks * Hkv * 16 rows][128]; box = 16 rows x 64 columns, SWIZZLE_128B
+// cache viewed as a 4-D bf16 tensor (64 columns, 8 rows of a group [256 B apart], 2 halves of head_dim [128 B apart],
+// row groups [2048 B apart]); box = (64, 8, 2, 2) = one (block, head) = 4 KB landing as [group][half][8 x 128 B], SWIZZLE_128B
 bool make_cache_map(CUtensorMap* m, const void* cache, int num_blocks, int hkv) {
   EncodeTiledFn enc = get_encode();
   if (!enc) return false;
-  cuuint64_t dims[2] = {(cuuint64_t)D, (cuuint64_t)num_blocks * hkv * kBlock};
-  cuuint64_t strides[1] = {(cuuint64_t)D * 2};
-  cuuint32_t box[2] = {64, (cuuint32_t)kBlock};
-  cuuint32_t estr[2] = {1, 1};
-  return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 2, const_cast<void*>(cache), dims, strides, box, estr,
+  cuuint64_t dims[4] = {64, 8, 2, (cuuint64_t)num_blocks * hkv * 2};
+  cuuint64_t strides[3] = {(cuuint64_t)D * 2, 128, (cuuint64_t)kGroupBytes};
+  cuuint32_t box[4] = {64, 8, 2, 2};
+  cuuint32_t estr[4] = {1, 1, 1, 1};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(cache), dims, strides, box, estr,
              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
@@ -867,6 +979,17 @@ bool launch_g(const Ctx& c, const CUtensorMap& mq, const CUtensorMap& mk, const 
 
 }  // namespace
 
+#ifdef MINIPIC_TRACE
+extern "C" int minipic_debug_trace_copy(long long* host, int* counts) {
+  cudaDeviceSynchronize();
+  if (cudaMemcpyFromSymbol(host, g_trace, sizeof(long long) * kTraceRoles * kTraceLen * 2) != cudaSuccess) return -1;
+  if (cudaMemcpyFromSymbol(counts, g_trace_n, sizeof(int) * kTraceRoles) != cudaSuccess) return -1;
+  int zero[kTraceRoles] = {0};
+  cudaMemcpyToSymbol(g_trace_n, zero, sizeof(zero));
+  return kTraceLen;
+}
+#endif
+
 bool prefill_sm100_supported(const Ctx& c) {
   return c.dtype == MINIPIC_BF16 && c.d == 128 && (c.group == 1 || c.group == 2 || c.group == 4 || c.group == 8);
 }
@@ -892,11 +1015,12 @@ bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
   Params prm;
   prm.a = a; prm.hq = c.hq; prm.hkv = c.hkv; prm.scale_log2 = c.scale_log2; prm.flags = c.flags;
   prm.hdr = hdr; prm.tiles = sorted;
-  prm.oob_row = c.num_blocks * c.hkv * kBlock;
+  prm.oob_grp = c.num_blocks * c.hkv * 2;
   for (int i = 0; i < 64; ++i) {
     prm.phase_inc[i] = c.rope.phase_inc[i];
     const double c1 = c.rope_step_cos[i], s1 = c.rope_step_sin[i];
     const double c2 = c1 * c1 - s1 * s1, s2 = 2.0 * s1 * c1;
+    prm.step1[i] = make_float2((float)c1, (float)s1);
     prm.step4[i] = make_float2((float)(c2 * c2 - s2 * s2), (float)(2.0 * s2 * c2));
   }
   int dev = 0, sms = 148;
