@@ -262,7 +262,7 @@ def run_ours(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": {"workload": WORKLOAD, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
                        "l2": "inputs larger than L2: each step touches ~3.5 GB (Q/O 2.2 GB) between repeats of any kernel",
-                       "rope": "cos/sin table lookup (PAPER.md:113), in-kernel K and Q rotation",
+                       "rope": "in-kernel K and Q rotation; cos/sin from an exact 64-bit fixed-point phase + MUFU (prefill adds an angle-addition recurrence); table built but unused by the bf16 kernels",
                        "tokens_per_step": tokens_per_step},
             "roofline": roofline, "roofline_decode": roofline_decode, "roofline_cache_write": roofline_cache_write,
             "kernels_ms": {"c5_cache_write": seg_mean[0], "c5_prefill": seg_mean[1], "c4_cache_write": seg_mean[2],
