@@ -32,6 +32,12 @@ constexpr int BM = 128, BN = 128, D = 128;
 constexpr int kTileBytes = BN * D * 2;       // 32 KB: one K / V / Q tile
 constexpr int kHalfBytes = kTileBytes / 2;   // [half of head_dim][128 rows][128 B]
 constexpr int kKStages = 2, kVStages = 2, kRing = 4;
+// Two restructurings of the softmax were measured on config 5 (2.38 ms with this version) and dropped:
+//  * every 2nd / 3rd / 4th exp2 pair on the FMA pipe (Cody-Waite + cubic minimax) instead of MUFU: 2.59 / 2.56 / 2.45 ms -
+//    the softmax warps are issue / latency bound, not MUFU bound, at this tile period;
+//  * the two 64-column halves of S as a double buffer (QK of the next half issued right after the PV that frees it, softmax
+//    in 64-column steps): 2.61 ms - the P -> PV -> QK -> S round trip (~1000 cycles) is as long as a 64-column softmax
+//    step, so the softmax warps still wait (49 % of their samples) and A / B no longer alternate on the MUFU unit.
 // K / V tile in shared memory: 16 row groups of [half of head_dim (2)][8 rows x 128 B] = 2048 B each, so one (block, head)
 // of the cache (16 tokens x 256 B) is ONE 4-D TMA box of two groups.  Q tile: [half (2)][128 rows x 128 B].
 constexpr int kGroupBytes = 2048, kKvHalfOff = 1024;
@@ -808,6 +814,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
 #pragma unroll
         for (int c = 0; c < 4; ++c) tmem_ld32(t_s + c * 32, s + c * 32);
         tmem_wait_ld();
+        if ((warp & 3) == 0) TRACE_L0(3 + x, 44);
         // mask at 32-column chunk granularity (all bounds but c_hi are warp-uniform): a chunk that every row of the
         // tile sees needs no mask code, a chunk no row sees (above the causal diagonal) skips max / exp altogether
         const int c_lo = it.lo - j0;
@@ -823,6 +830,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           mx2 = max3(mx2, s[c + 4], s[c + 5]); mx3 = max3(mx3, s[c + 6], s[c + 7]);
         }
         const float m_new = fmaxf(m_used, fmaxf(max3(mx0, mx1, mx2), mx3) * prm.scale_log2);
+        if ((warp & 3) == 0) TRACE_L0(3 + x, 45);
         if (i == 0) {
           m_used = m_new;
         } else {
@@ -850,9 +858,9 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           uint32_t pk[16];
 #pragma unroll
           for (int c = 0; c < 16; ++c) {
-            float x0, x1;
+            float x0, x1, p0, p1;
             upk2(fma2(pk2(s[32 * h + 2 * c], s[32 * h + 2 * c + 1]), sc2, nm2), x0, x1);
-            const float p0 = fast_exp2(x0), p1 = fast_exp2(x1);
+            p0 = fast_exp2(x0); p1 = fast_exp2(x1);
             if (c & 1) lsum1 = add2(lsum1, pk2(p0, p1)); else lsum0 = add2(lsum0, pk2(p0, p1));
             pk[c] = pack_bf16(p0, p1);
           }
@@ -863,6 +871,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           upk2(add2(lsum0, lsum1), a0, a1);
           l_run += a0 + a1;
         }
+        if ((warp & 3) == 0) TRACE_L0(3 + x, 46);
         tmem_wait_st();
         tc_fence_before();
         mbar_arrive(bar(P_FULL + x));
