@@ -316,7 +316,11 @@ def run_ours(args):
                 only = time_calls(g, 20, 3, torch)[0]
                 warm = time_calls(dw.attention, 50, 5, torch)
                 fl = w.attention_flops()
+                dw.set_flags(mp.MINIPIC_K_PREROTATED)
+                warm_pre = time_calls(dw.attention, 50, 5, torch)
+                dw.set_flags(0)
                 extras[name] = {"ms_cold_l2": max(both - only, 1e-6), "ms_warm_l2": warm[0], "ms_best": warm[1],
+                                "ms_warm_prerotated": warm_pre[0], "rope_overhead": warm[0] / warm_pre[0] - 1.0,
                                 "tokens_per_s_warm": w.num_q_tokens / (warm[0] * 1e-3),
                                 "tflops_warm": fl / (warm[0] * 1e-3) / 1e12, "variant": mp.minipic_last_variant()}
                 del dw
@@ -325,8 +329,12 @@ def run_ours(args):
             dp.step(); torch.cuda.synchronize()
             tp = time_calls(dp.attention, 20, 3, torch)
             gb = wp.logical_kv_bytes() / (tp[0] * 1e-3) / 1e9
+            dp.set_flags(mp.MINIPIC_K_PREROTATED)
+            tpp = time_calls(dp.attention, 20, 3, torch)
+            dp.set_flags(0)
             extras["c4_private_pool"] = {"ms": tp[0], "ms_best": tp[1], "kv_gbs": gb, "frac_hbm_measured": gb / peaks["hbm_gbs"],
-                                         "resident_kv_bytes": wp.logical_kv_bytes()}
+                                         "resident_kv_bytes": wp.logical_kv_bytes(), "ms_prerotated": tpp[0],
+                                         "rope_overhead": tp[0] / tpp[0] - 1.0}
             del dp, flush
         except Exception as e:  # extras never break the contract line
             extras["error"] = repr(e)

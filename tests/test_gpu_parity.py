@@ -150,6 +150,34 @@ def test_position_shift_invariance_and_large_positions_on_gpu():
         compare(dw, oracle_cache=(kc, vc))
 
 
+@pytest.mark.parametrize("group", [1, 2, 4, 8])
+def test_non_consecutive_positions_all_group_sizes(group):
+    """Logical positions need not equal the sequence index nor be consecutive (reading A3; Prompt-Cache style layouts,
+    PAPER.md:149): gaps at random places, inside 16-token blocks and inside 32-key rotation chunks.  This drives the
+    per-row exact-restart paths of the K and Q rotation (the fast path assumes consecutive positions) for every GQA
+    group size the tcgen05 kernel instantiates, and the decode kernel on the same tables."""
+    hkv = 2
+    w = W.single_request_prefill(name=f"gaps_g{group}", hq=hkv * group, hkv=hkv, d=128, theta=5e5, dtype="bf16", sigma=1.0,
+                                 span_lens=[176, 80, 144], suffix_len=40, num_blocks=64, seed=17 + group)
+    rng = np.random.default_rng(99 + group)
+    gaps = rng.choice([1, 1, 1, 1, 1, 1, 2, 7, 300], size=w.kv_positions.shape[0])
+    w.kv_positions = (np.cumsum(gaps) - gaps[0] + 3).astype(np.int32)
+    dw = DeviceWorkload(w); dw.step(); torch.cuda.synchronize()
+    st = compare(dw, expect_variant="prefill_sm100_tcgen05")
+    # positions consecutive except for ONE jump in the middle of a 16-token block
+    w2 = W.single_request_prefill(name=f"jump_g{group}", hq=hkv * group, hkv=hkv, d=128, theta=5e5, dtype="bf16", sigma=1.0,
+                                  span_lens=[176, 80, 144], suffix_len=40, num_blocks=64, seed=17 + group)
+    pos = np.arange(w2.kv_positions.shape[0], dtype=np.int32)
+    pos[213:] += 1000
+    w2.kv_positions = pos
+    dw2 = DeviceWorkload(w2); dw2.step(); torch.cuda.synchronize()
+    compare(dw2, expect_variant="prefill_sm100_tcgen05")
+    wd = W.decode_from_prefill(w, seed=3)
+    dd = DeviceWorkload(wd); dd.step(); torch.cuda.synchronize()
+    compare(dd)
+    assert st["out_max"] > 0.0
+
+
 def test_k_prerotated_control_matches():
     """MINIPIC_K_PREROTATED control: a cache holding oracle-rotated keys (rounded to bf16) with the in-kernel
     K RoPE switched off gives the same attention within the same tolerances."""
