@@ -819,9 +819,14 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         // tile sees needs no mask code, a chunk no row sees (above the causal diagonal) skips max / exp altogether
         const int c_lo = it.lo - j0;
         const int c_hi = row_ok ? idx_row - j0 : -1;
-        if (!((j0 >= it.lo) && (j0 + BN - 1 <= min(idx_first, it.kv_len - 1)))) {   // tile not fully visible to every row
+        const int c_hi_max = min(idx_first + TOK - 1, it.kv_len - 1) - j0;   // highest row of the tile (warp-uniform)
+        if (j0 + BN - 1 > min(idx_first, it.kv_len - 1)) {   // tile reaches past the lowest row's last visible key
 #pragma unroll
-          for (int c = 0; c < BN; ++c) s[c] = (c >= c_lo && c <= c_hi) ? s[c] : -INFINITY;
+          for (int c = 0; c < BN; ++c) s[c] = (c <= c_hi) ? s[c] : -INFINITY;
+        }
+        if (c_lo > 0) {   // vis_lo inside the first gathered 16-token block (kv_lo = floor16(vis_lo)): c_lo < 16
+#pragma unroll
+          for (int c = 0; c < kBlock; ++c) s[c] = (c >= c_lo) ? s[c] : -INFINITY;
         }
         float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
 #pragma unroll
@@ -856,6 +861,12 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
 #pragma unroll
         for (int h = 0; h < 4; ++h) {
           uint32_t pk[16];
+          if (32 * h > c_hi_max) {   // keys above the causal diagonal for every row of the tile: P = 0, no exp
+#pragma unroll
+            for (int c = 0; c < 16; ++c) pk[c] = 0u;
+            tmem_st16(t_s + 16 * h, pk);
+            continue;
+          }
 #pragma unroll
           for (int c = 0; c < 16; ++c) {
             float x0, x1, p0, p1;
