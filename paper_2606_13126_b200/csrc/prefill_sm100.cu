@@ -132,6 +132,13 @@ __device__ __forceinline__ void tma_load_4d(uint32_t dst, const CUtensorMap* tma
       "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %4, %5, %6}], [%2];"
       ::"r"(dst), "l"(tmap), "r"(bar), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
 }
+__device__ __forceinline__ void tma_store_3d(const CUtensorMap* tmap, uint32_t src, int x, int y, int z) {
+  asm volatile("cp.async.bulk.tensor.3d.global.shared::cta.bulk_group [%0, {%2, %3, %4}], [%1];"
+               ::"l"(tmap), "r"(src), "r"(x), "r"(y), "r"(z) : "memory");
+}
+__device__ __forceinline__ void tma_store_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void tma_store_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 // Shared-memory matrix descriptors (SWIZZLE_128B): the low word carries the start address (>> 4) and the leading byte
 // offset (>> 4, bits 16-29); the high word is the same for every operand of this kernel: stride byte offset 1024
 // (8 rows x 128 B), descriptor version 1 (bit 46), swizzle mode 128B (2 << 61).
@@ -428,7 +435,8 @@ struct Rot8 {
 template <int G>
 __global__ void __launch_bounds__(kThreads, 1)
 prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
-                     const __grid_constant__ CUtensorMap tmap_v, const __grid_constant__ Params prm) {
+                     const __grid_constant__ CUtensorMap tmap_v, const __grid_constant__ CUtensorMap tmap_o,
+                     const __grid_constant__ Params prm) {
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
   constexpr int TOK = BM / G;
@@ -898,6 +906,8 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       {
         const uint32_t stg = smem_u32(sm.ostage[warp]);
         const int rr = lane >> 3, cc = lane & 7;
+        const bool whole = it.ntok_x(x) == TOK;   // every row of the tile is a real query row: the warp's 32 rows go out
+                                                  // as one TMA tensor store per pass (box = 64 columns x G heads x 32/G tokens)
         __nv_bfloat16* obase = (__nv_bfloat16*)a.out + ((size_t)(it.t0 + x * TOK) * prm.hq + it.kvh * G) * D + cc * 8;
 #pragma unroll 1
         for (int pass = 0; pass < 2; ++pass) {
@@ -910,6 +920,8 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
 #pragma unroll
             for (int e = 0; e < 64; ++e) o[e] = 0.f;
           }
+          if (lane == 0) tma_store_wait_read();   // the previous store out of this staging buffer has been read
+          __syncwarp();
 #pragma unroll
           for (int c = 0; c < 8; ++c) {
             uint4 v;
@@ -917,15 +929,24 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
             v.z = pack_bf16(o[8 * c + 4] * inv, o[8 * c + 5] * inv); v.w = pack_bf16(o[8 * c + 6] * inv, o[8 * c + 7] * inv);
             sts128(stg + lane * 128 + ((c ^ (lane & 7)) << 4), v);
           }
-          __syncwarp();
+          if (whole) {
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) {
+              tma_store_3d(&tmap_o, stg, pass * 64, it.kvh * G, it.t0 + x * TOK + ((warp & 3) * 32) / G);
+              tma_store_commit();
+            }
+          } else {
+            __syncwarp();
 #pragma unroll
-          for (int itr = 0; itr < 8; ++itr) {
-            const int r = itr * 4 + rr, rowg = (warp & 3) * 32 + r;
-            const uint4 v = lds128(stg + r * 128 + ((cc ^ (r & 7)) << 4));
-            if (rowg / G < it.ntok_x(x))
-              *reinterpret_cast<uint4*>(obase + ((size_t)(rowg / G) * prm.hq + rowg % G) * D + pass * 64) = v;
+            for (int itr = 0; itr < 8; ++itr) {
+              const int r = itr * 4 + rr, rowg = (warp & 3) * 32 + r;
+              const uint4 v = lds128(stg + r * 128 + ((cc ^ (r & 7)) << 4));
+              if (rowg / G < it.ntok_x(x))
+                *reinterpret_cast<uint4*>(obase + ((size_t)(rowg / G) * prm.hq + rowg % G) * D + pass * 64) = v;
+            }
+            __syncwarp();
           }
-          __syncwarp();
         }
       }
       if ((warp & 3) == 0) TRACE_L0(3 + x, 43);
@@ -933,6 +954,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         a.lse[(size_t)(it.t0 + tok) * prm.hq + it.kvh * G + hg] =
             l_run > 0.f ? (m_used + log2f(l_run)) * 0.6931471805599453f : -INFINITY;
     }
+    if (lane == 0) tma_store_wait_all();   // the staging buffers must outlive the last tensor stores
   }
   tc_fence_before();
   __syncthreads();
@@ -983,8 +1005,21 @@ bool make_q_map(CUtensorMap* m, const void* q, int num_q_tokens, int hq, int gro
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// out viewed as [Tq][Hq][128]; box = 64 columns x G heads x 32/G tokens = the 32 rows of one softmax warp, SWIZZLE_128B
+bool make_out_map(CUtensorMap* m, void* out, int num_q_tokens, int hq, int group) {
+  EncodeTiledFn enc = get_encode();
+  if (!enc) return false;
+  cuuint64_t dims[3] = {(cuuint64_t)D, (cuuint64_t)hq, (cuuint64_t)num_q_tokens};
+  cuuint64_t strides[2] = {(cuuint64_t)D * 2, (cuuint64_t)hq * D * 2};
+  cuuint32_t box[3] = {64, (cuuint32_t)group, (cuuint32_t)(32 / group > 0 ? 32 / group : 1)};
+  cuuint32_t estr[3] = {1, 1, 1};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 3, out, dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+             CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
 template <int G>
-bool launch_g(const Ctx& c, const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const Params& prm, int sms) {
+bool launch_g(const Ctx& c, const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mo,
+              const Params& prm, int sms) {
   const size_t smem = sizeof(Smem);
   static bool attr_done = false;
   if (!attr_done) {
@@ -992,7 +1027,7 @@ bool launch_g(const Ctx& c, const CUtensorMap& mq, const CUtensorMap& mk, const 
       return false;
     attr_done = true;
   }
-  prefill_sm100_kernel<G><<<sms, kThreads, smem, c.stream>>>(mq, mk, mv, prm);
+  prefill_sm100_kernel<G><<<sms, kThreads, smem, c.stream>>>(mq, mk, mv, mo, prm);
   note_launch();
   return true;
 }
@@ -1019,9 +1054,9 @@ size_t prefill_sm100_workspace_bytes(const Ctx&, int, int num_q_tokens) {
 }
 
 bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
-  CUtensorMap mq, mk, mv;
+  CUtensorMap mq, mk, mv, mo;
   if (!make_cache_map(&mk, a.k_cache, c.num_blocks, c.hkv) || !make_cache_map(&mv, a.v_cache, c.num_blocks, c.hkv) ||
-      !make_q_map(&mq, a.q, a.num_q_tokens, c.hq, c.group))
+      !make_q_map(&mq, a.q, a.num_q_tokens, c.hq, c.group) || !make_out_map(&mo, a.out, a.num_q_tokens, c.hq, c.group))
     return false;
   PlanHeader* hdr = (PlanHeader*)a.workspace;
   TileDesc* sorted = (TileDesc*)((char*)a.workspace + sizeof(PlanHeader));
@@ -1047,10 +1082,10 @@ bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   switch (c.group) {
-    case 1: return launch_g<1>(c, mq, mk, mv, prm, sms);
-    case 2: return launch_g<2>(c, mq, mk, mv, prm, sms);
-    case 4: return launch_g<4>(c, mq, mk, mv, prm, sms);
-    case 8: return launch_g<8>(c, mq, mk, mv, prm, sms);
+    case 1: return launch_g<1>(c, mq, mk, mv, mo, prm, sms);
+    case 2: return launch_g<2>(c, mq, mk, mv, mo, prm, sms);
+    case 4: return launch_g<4>(c, mq, mk, mv, mo, prm, sms);
+    case 8: return launch_g<8>(c, mq, mk, mv, mo, prm, sms);
   }
   return false;
 }
