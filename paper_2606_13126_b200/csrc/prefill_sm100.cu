@@ -32,7 +32,14 @@ constexpr int BM = 128, BN = 128, D = 128;
 constexpr int kTileBytes = BN * D * 2;       // 32 KB: one K / V / Q tile
 constexpr int kHalfBytes = kTileBytes / 2;   // [half of head_dim][128 rows][128 B]
 constexpr int kKStages = 2, kVStages = 2, kRing = 4;
-// Two restructurings of the softmax were measured on config 5 (2.38 ms with this version) and dropped:
+// Measured and dropped (config 5, in-kernel RoPE; the kept version runs 2.24 ms):
+//  * a ring of three Q tile slots (next item's tile A loaded + rotated during the current item, epilogue staged in the
+//    finishing item's tile-B slot): parity-green, dense +3 %, but span items -7 % (2.30 ms): the four rotation warps are
+//    saturated at item boundaries (K0', Q_A', Q_B', K1' = 4.5 tile rotations per ~3-tile item) and starting Q earlier only
+//    takes issue slots from the current item's softmax;  a single V stage (needed for a full Q double buffer) costs 7 %;
+//  * Q rotation unrolled like the K path, or two rows per iteration: 8 % / 7 % slower (instruction cache);
+//  * L2 prefetch of the next item's Q tiles: no change.
+// Two restructurings of the softmax were measured on config 5 (2.38 ms at the time) and dropped:
 //  * every 2nd / 3rd / 4th exp2 pair on the FMA pipe (Cody-Waite + cubic minimax) instead of MUFU: 2.59 / 2.56 / 2.45 ms -
 //    the softmax warps are issue / latency bound, not MUFU bound, at this tile period;
 //  * the two 64-column halves of S as a double buffer (QK of the next half issued right after the PV that frees it, softmax
