@@ -10,14 +10,15 @@
 //
 //   warp 12      TMA producer  : scheduler ring; Q super-tile (3-D box) and the KV tile's 8 physical blocks through
 //                                the block table with cp.async.bulk.tensor (SWIZZLE_128B boxes) into smem       (a4)
-//   warps 8-11   rotation      : in-place RoPE of the Q tiles (a3) and of every K tile (a5): smem -> registers ->
-//                                smem; a lane owns two frequencies and walks the keys of a 16-token block, cos/sin
-//                                restarted exactly (64-bit fixed-point phase + MUFU) at every block / position jump
-//                                and advanced by the angle-addition recurrence in between (packed f32x2 FMAs)
+//   warps 8-11   rotation      : in-place RoPE of every K tile (a5): smem -> registers -> smem; a lane owns 8 frequencies
+//                                (one 16-byte chunk of both halves of a row), cos/sin restarted exactly (64-bit fixed-point
+//                                phase + MUFU) once per 32-key chunk / at every position jump and advanced by the
+//                                angle-addition recurrence in between (packed f32x2 FMAs)
 //   warp 13      MMA issuer    : tcgen05.mma S_X = Q_X K'^T (smem x smem -> TMEM), O_X += P_X V (TMEM x smem -> TMEM),
 //                                X in {A, B} ping-pong so the tensor pipe runs while the other tile is in softmax (a6, a8)
-//   warps 0-3 / 4-7 softmax A/B: tcgen05.ld S (one row per thread), mask, online softmax with lazy rescale of O,
-//                                P -> bf16 -> TMEM (aliasing S); epilogue O / l -> out, LSE                  (a7, a9)
+//   warps 0-3 / 4-7 softmax A/B: in-place RoPE of their own Q tile at the start of an item (a3); tcgen05.ld S (one row per
+//                                thread), mask, online softmax with lazy rescale of O, P -> bf16 -> TMEM (aliasing S);
+//                                epilogue O / l -> out, LSE, deferred until the next item's Q is rotated       (a7, a9)
 //
 // All hand-offs are mbarriers; generic-proxy smem writes are fenced with fence.proxy.async before the MMA reads.
 #include <cuda.h>
@@ -661,9 +662,9 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       }
     }
   } else if (warp >= 8) {
-    // ============================================================ rotation warps: Q (a3) and K tiles (a5)
+    // ============================================================ rotation warps: K tiles (a5)
     // NOTE on code shape: the kernel is instruction-cache bound (four roles with different code share an SM), so only the
-    // per-tile K path is unrolled; the once-per-item Q path is a rolled loop (unrolling it measured 8% slower on config 5).
+    // per-tile K path is unrolled.  The once-per-item Q rotation (a3) lives in the softmax warps as a rolled loop.
     reg_dec<kRegsRot>();
     const int rw = warp - 8, rot_tid = threadIdx.x - 256;
     const int rsub = lane >> 3, ch = lane & 7;
@@ -680,7 +681,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
     const uint32_t off_o = (uint32_t)((4 + rsub) * 128 + ((ch ^ (4 + rsub)) << 4));
     const bool k_prerot = (prm.flags & MINIPIC_K_PREROTATED) != 0, q_prerot = (prm.flags & MINIPIC_Q_PREROTATED) != 0;
     constexpr int NTW = (32 / G) > 0 ? (32 / G) : 1;   // Q tokens per warp per tile
-    uint32_t kc = 0, vc = 0, qc = 0;
+    uint32_t kc = 0, vc = 0;
     for (uint32_t it_n = 0;; ++it_n) {
       const int slot = it_n & (kRing - 1);
       w.wait(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
@@ -692,13 +693,6 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       const int* pos = a.kv_positions + it.kv_off;
       // lane l holds the position of key 32 rw + l of the tile / of Q token 32 rw / G + l of tile A, B (fetched early)
       int myp = __ldg(pos + min(it.kv_lo + 32 * rw + lane, it.kv_len - 1));
-      int qpos_a, qpos_b;
-      {
-        const int ta = min((32 * rw) / G + min(lane, NTW - 1), max(it.ntok_a - 1, 0));
-        const int tb = min((32 * rw) / G + min(lane, NTW - 1), max(it.ntok_b - 1, 0));
-        qpos_a = __ldg(pos + min(it.idx0 + ta, it.kv_len - 1));
-        qpos_b = __ldg(pos + min(it.idx0 + TOK + tb, it.kv_len - 1));
-      }
       for (int i = 0; i < it.n_kv; ++i) {
         const int st = kc % kKStages;
         const int j0 = it.kv_lo + i * BN + 32 * rw;
@@ -738,48 +732,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         fence_proxy_async();
         mbar_arrive(bar(K_READY + st));
         if (rw == 0) TRACE_L0(2, 31);
-        if (i == 0) {
-          // ---- Q super-tile: row = token * G + head-in-group; the G rows of a token share one position.  Exact restart
-          //      at the first row, one-position steps while the positions are consecutive, restart otherwise.  Tile A is
-          //      published first so that QK_A runs while tile B is still being rotated.
-          w.wait(bar(Q_FULL), qc & 1);
-          if (rw == 0) TRACE_L0(2, 32);
-          if (!q_prerot) {
-            uint64_t c1[4], s1[4], ns1[4];
-#pragma unroll
-            for (int e = 0; e < 4; ++e) {
-              const uint4 u = lds128(step1_addr + 16 * e);   // (cos, sin) of frequencies 2e, 2e + 1 of this lane
-              c1[e] = pk2(__uint_as_float(u.x), __uint_as_float(u.z));
-              s1[e] = pk2(__uint_as_float(u.y), __uint_as_float(u.w));
-              ns1[e] = pk2(-__uint_as_float(u.y), -__uint_as_float(u.w));
-            }
-#pragma unroll 1
-            for (int x = 0; x < 2; ++x) {
-              const int ntw = it.ntok_x(x) - (32 * rw) / G;        // tokens of this tile that this warp rotates
-              const uint32_t qt = smem_u32(sm.q[x]) + (uint32_t)rw * 4096;
-              const int qpx = x ? qpos_b : qpos_a;
-              int prev = 0;
-#pragma unroll 1
-              for (int k = 0; k < 8; ++k) {
-                if ((4 * k) / G >= ntw) break;
-                const uint32_t addr = qt + (k >> 1) * 1024 + ((k & 1) ? off_o : off_e);
-                const uint4 lo = lds128(addr), hi = lds128(addr + kHalfBytes);
-                const int p = __shfl_sync(0xffffffffu, qpx, ((32 * rw) % G + 4 * k + rsub) / G);
-                if (k > 0 && p == prev + 1) rot.advance(c1, s1, ns1);
-                else if (k == 0 || p != prev) rot.restart(p, finc_addr);
-                prev = p;
-                rot.rotate_store(addr, kHalfBytes, lo, hi);
-              }
-              fence_proxy_async();
-              mbar_arrive(bar(Q_READY + x));
-            }
-          } else {
-            mbar_arrive(bar(Q_READY)); mbar_arrive(bar(Q_READY + 1));
-          }
-          if (rw == 0) TRACE_L0(2, 33);
-        }
         ++kc;
-        if (i == 0) ++qc;
         myp = myp_next;
         // ---- V tile i: rows at or beyond kv_hi inside the last gathered block may hold anything (never written
         //      cache slots); their P is 0, make sure 0 * (those bits) is not NaN
@@ -806,14 +759,122 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
     const uint32_t t_lane = tmem + ((uint32_t)((warp & 3) * 32) << 16);
     const uint32_t t_s = t_lane + x * BN, t_o = t_lane + (2 + x) * BN;
     const int tok_in = row / G, hg = row % G;
-    uint32_t sc = 0, oc = 0;
+    uint32_t sc = 0, oc = 0, qc = 0;
+    struct { bool valid; int t0, kvh, ntok_x, n; float l, m; } pe;
+    pe.valid = false;
+    auto epilogue = [&]() {
+      // ---- epilogue (a9): O / l -> out, LSE = ln sum exp of the scaled scores.  A thread owns a row in TMEM, but a row
+      //      is 256 B in global memory: the warp transposes 64 columns at a time through its 4 KB staging buffer so
+      //      that every store instruction writes four full 128-byte lines instead of 32 scattered 16-byte pieces
+      const float inv = pe.l > 0.f ? 1.f / pe.l : 0.f;
+      if (pe.n > 0) { w.wait(bar(O_FULL + x), oc & 1); ++oc; tc_fence_after(); }
+      if ((warp & 3) == 0) TRACE_L0(3 + x, 42);
+      {
+        const uint32_t stg = smem_u32(sm.ostage[warp]);
+        const int rr = lane >> 3, cc = lane & 7;
+        const bool whole = pe.ntok_x == TOK;   // every row of the tile is a real query row: the warp's 32 rows go out
+                                                  // as one TMA tensor store per pass (box = 64 columns x G heads x 32/G tokens)
+        __nv_bfloat16* obase = (__nv_bfloat16*)a.out + ((size_t)(pe.t0 + x * TOK) * prm.hq + pe.kvh * G) * D + cc * 8;
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass) {
+          float o[64];
+          if (pe.n > 0) {
+            tmem_ld32(t_o + pass * 64, o); tmem_ld32(t_o + pass * 64 + 32, o + 32);
+            tmem_wait_ld();
+            if (pass == 1) { tc_fence_before(); mbar_arrive(bar(O_FREE + x)); }   // O is in registers: the next item may start
+          } else {
+#pragma unroll
+            for (int e = 0; e < 64; ++e) o[e] = 0.f;
+          }
+          if (lane == 0) tma_store_wait_read();   // the previous store out of this staging buffer has been read
+          __syncwarp();
+#pragma unroll
+          for (int c = 0; c < 8; ++c) {
+            uint4 v;
+            v.x = pack_bf16(o[8 * c] * inv, o[8 * c + 1] * inv); v.y = pack_bf16(o[8 * c + 2] * inv, o[8 * c + 3] * inv);
+            v.z = pack_bf16(o[8 * c + 4] * inv, o[8 * c + 5] * inv); v.w = pack_bf16(o[8 * c + 6] * inv, o[8 * c + 7] * inv);
+            sts128(stg + lane * 128 + ((c ^ (lane & 7)) << 4), v);
+          }
+          if (whole) {
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) {
+              tma_store_3d(&tmap_o, stg, pass * 64, pe.kvh * G, pe.t0 + x * TOK + ((warp & 3) * 32) / G);
+              tma_store_commit();
+            }
+          } else {
+            __syncwarp();
+#pragma unroll
+            for (int itr = 0; itr < 8; ++itr) {
+              const int r = itr * 4 + rr, rowg = (warp & 3) * 32 + r;
+              const uint4 v = lds128(stg + r * 128 + ((cc ^ (r & 7)) << 4));
+              if (rowg / G < pe.ntok_x)
+                *reinterpret_cast<uint4*>(obase + ((size_t)(rowg / G) * prm.hq + rowg % G) * D + pass * 64) = v;
+            }
+            __syncwarp();
+          }
+        }
+      }
+      if ((warp & 3) == 0) TRACE_L0(3 + x, 43);
+      if ((tok_in < pe.ntok_x))
+        a.lse[(size_t)(pe.t0 + x * TOK + tok_in) * prm.hq + pe.kvh * G + hg] =
+            pe.l > 0.f ? (pe.m + log2f(pe.l)) * 0.6931471805599453f : -INFINITY;
+        };
+    // Q rotation (a3) state of this lane: same row / chunk mapping as the K rotation lanes
+    const int rw = warp & 3, rsub = lane >> 3, ch = lane & 7;
+    const uint32_t finc_addr = smem_u32(sm.finc) + 64 * ch, step1_addr = smem_u32(sm.step1) + 64 * ch;
+    const uint32_t off_e = (uint32_t)(rsub * 128 + ((ch ^ rsub) << 4));
+    const uint32_t off_o = (uint32_t)((4 + rsub) * 128 + ((ch ^ (4 + rsub)) << 4));
+    const bool q_prerot = (prm.flags & MINIPIC_Q_PREROTATED) != 0;
+    constexpr int NTW = (32 / G) > 0 ? (32 / G) : 1;   // Q tokens per warp per tile
     for (uint32_t it_n = 0;; ++it_n) {
       const int slot = it_n & (kRing - 1);
       w.wait(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
-      if (w.dead || sm.ring[slot].t0 < 0) break;
+      const bool stop = w.dead || sm.ring[slot].t0 < 0;   // one more trip for the deferred epilogue, then out
       const Item it = load_item<TOK>(sm.ring[slot]);
       __syncwarp();
-      if (lane == 0) mbar_arrive(bar(SCHED_EMPTY + slot));
+      if (!stop && lane == 0) mbar_arrive(bar(SCHED_EMPTY + slot));
+      if (!stop && it.n_kv > 0) {
+        // ---- a3: rotate this warp's 32 rows of Q tile x in place: row = token * G + head-in-group, the G rows of a token
+        //      share one position.  Exact restart at the first row, one-position steps while the positions are consecutive.
+        //      The eight softmax warps do this (not the four K rotation warps): they would otherwise idle at the item
+        //      boundary while K0, Q_A, Q_B queue up on the rotation warps.  Rolled loop: see the note on code size there.
+        const int ntw = it.ntok_x(x) - (32 * rw) / G;   // tokens of this tile that this warp rotates
+        int qpx = 0;
+        if (!q_prerot && ntw > 0) {
+          const int tk = min((32 * rw) / G + min(lane, NTW - 1), it.ntok_x(x) - 1);
+          qpx = __ldg(a.kv_positions + it.kv_off + min(it.idx0 + x * TOK + tk, it.kv_len - 1));
+        }
+        w.wait(bar(Q_FULL), qc & 1); ++qc;
+        if (!q_prerot && ntw > 0) {
+          Rot8 rot;
+          uint64_t c1[4], s1[4], ns1[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const uint4 u = lds128(step1_addr + 16 * e);   // (cos, sin) of frequencies 2e, 2e + 1 of this lane
+            c1[e] = pk2(__uint_as_float(u.x), __uint_as_float(u.z));
+            s1[e] = pk2(__uint_as_float(u.y), __uint_as_float(u.w));
+            ns1[e] = pk2(-__uint_as_float(u.y), -__uint_as_float(u.w));
+          }
+          const uint32_t qt = smem_u32(sm.q[x]) + (uint32_t)rw * 4096;
+          int prev = 0;
+#pragma unroll 1
+          for (int k = 0; k < 8; ++k) {
+            if ((4 * k) / G >= ntw) break;
+            const uint32_t addr = qt + (k >> 1) * 1024 + ((k & 1) ? off_o : off_e);
+            const uint4 lo = lds128(addr), hi = lds128(addr + kHalfBytes);
+            const int p = __shfl_sync(0xffffffffu, qpx, ((32 * rw) % G + 4 * k + rsub) / G);
+            if (k > 0 && p == prev + 1) rot.advance(c1, s1, ns1);
+            else if (k == 0 || p != prev) rot.restart(p, finc_addr);
+            prev = p;
+            rot.rotate_store(addr, kHalfBytes, lo, hi);
+          }
+        }
+        fence_proxy_async();
+        mbar_arrive(bar(Q_READY + x));
+      }
+      if (pe.valid) epilogue();   // previous item of this tile
+      if (stop) break;
       const bool row_ok = tok_in < it.ntok_x(x);
       const int tok = x * TOK + tok_in;
       const int idx_first = it.idx0 + x * TOK;                       // lowest query index of this tile
@@ -903,63 +964,9 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         mbar_arrive(bar(P_FULL + x));
         if ((warp & 3) == 0) TRACE_L0(3 + x, 41);
       }
-      // ---- epilogue (a9): O / l -> out, LSE = ln sum exp of the scaled scores.  A thread owns a row in TMEM, but a row
-      //      is 256 B in global memory: the warp transposes 64 columns at a time through its 4 KB staging buffer so
-      //      that every store instruction writes four full 128-byte lines instead of 32 scattered 16-byte pieces
-      if (it.ntok_x(x) <= 0) continue;
-      const float inv = l_run > 0.f ? 1.f / l_run : 0.f;
-      if (n > 0) { w.wait(bar(O_FULL + x), oc & 1); ++oc; tc_fence_after(); }
-      if ((warp & 3) == 0) TRACE_L0(3 + x, 42);
-      {
-        const uint32_t stg = smem_u32(sm.ostage[warp]);
-        const int rr = lane >> 3, cc = lane & 7;
-        const bool whole = it.ntok_x(x) == TOK;   // every row of the tile is a real query row: the warp's 32 rows go out
-                                                  // as one TMA tensor store per pass (box = 64 columns x G heads x 32/G tokens)
-        __nv_bfloat16* obase = (__nv_bfloat16*)a.out + ((size_t)(it.t0 + x * TOK) * prm.hq + it.kvh * G) * D + cc * 8;
-#pragma unroll 1
-        for (int pass = 0; pass < 2; ++pass) {
-          float o[64];
-          if (n > 0) {
-            tmem_ld32(t_o + pass * 64, o); tmem_ld32(t_o + pass * 64 + 32, o + 32);
-            tmem_wait_ld();
-            if (pass == 1) { tc_fence_before(); mbar_arrive(bar(O_FREE + x)); }   // O is in registers: the next item may start
-          } else {
-#pragma unroll
-            for (int e = 0; e < 64; ++e) o[e] = 0.f;
-          }
-          if (lane == 0) tma_store_wait_read();   // the previous store out of this staging buffer has been read
-          __syncwarp();
-#pragma unroll
-          for (int c = 0; c < 8; ++c) {
-            uint4 v;
-            v.x = pack_bf16(o[8 * c] * inv, o[8 * c + 1] * inv); v.y = pack_bf16(o[8 * c + 2] * inv, o[8 * c + 3] * inv);
-            v.z = pack_bf16(o[8 * c + 4] * inv, o[8 * c + 5] * inv); v.w = pack_bf16(o[8 * c + 6] * inv, o[8 * c + 7] * inv);
-            sts128(stg + lane * 128 + ((c ^ (lane & 7)) << 4), v);
-          }
-          if (whole) {
-            fence_proxy_async();
-            __syncwarp();
-            if (lane == 0) {
-              tma_store_3d(&tmap_o, stg, pass * 64, it.kvh * G, it.t0 + x * TOK + ((warp & 3) * 32) / G);
-              tma_store_commit();
-            }
-          } else {
-            __syncwarp();
-#pragma unroll
-            for (int itr = 0; itr < 8; ++itr) {
-              const int r = itr * 4 + rr, rowg = (warp & 3) * 32 + r;
-              const uint4 v = lds128(stg + r * 128 + ((cc ^ (r & 7)) << 4));
-              if (rowg / G < it.ntok_x(x))
-                *reinterpret_cast<uint4*>(obase + ((size_t)(rowg / G) * prm.hq + rowg % G) * D + pass * 64) = v;
-            }
-            __syncwarp();
-          }
-        }
-      }
-      if ((warp & 3) == 0) TRACE_L0(3 + x, 43);
-      if (row_ok)
-        a.lse[(size_t)(it.t0 + tok) * prm.hq + it.kvh * G + hg] =
-            l_run > 0.f ? (m_used + log2f(l_run)) * 0.6931471805599453f : -INFINITY;
+      // the epilogue of an item is DEFERRED until this tile's Q rows of the next item are rotated (below), so that QK of the
+      // next item starts ~3 K cycles earlier; pe = what it needs
+      pe.valid = it.ntok_x(x) > 0; pe.t0 = it.t0; pe.kvh = it.kvh; pe.ntok_x = it.ntok_x(x); pe.n = n; pe.l = l_run; pe.m = m_used;
     }
     if (lane == 0) tma_store_wait_all();   // the staging buffers must outlive the last tensor stores
   }
