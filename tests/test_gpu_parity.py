@@ -178,6 +178,31 @@ def test_non_consecutive_positions_all_group_sizes(group):
     assert st["out_max"] > 0.0
 
 
+def test_other_span_techniques_through_the_same_descriptor():
+    """the per-row interval descriptor also expresses (a) EPIC / LegoLink style link
+    tokens - the first 16 tokens (one block) of every span see the whole prefix (vis_lo = 0) while the rest of the span
+    stays span-local, so vis_lo changes in the middle of a Q super-tile - and (b) Prompt-Cache style layouts where every
+    span keeps positions from its own module range (span i starts at 4096 * i), i.e. non-contiguous logical positions."""
+    w = W.single_request_prefill(name="epic", hq=16, hkv=2, d=128, theta=5e5, dtype="bf16", sigma=1.0,
+                                 span_lens=[160, 208, 96], suffix_len=48, num_blocks=64, seed=23)
+    lo = w.q_vis_lo.copy()
+    idx = w.q_seq_idx
+    link = (idx - lo) < 16                      # first block of each span (suffix rows have lo = 0 already)
+    lo[link] = 0
+    w.q_vis_lo = lo.astype(np.int32)
+    dw = DeviceWorkload(w); dw.step(); torch.cuda.synchronize()
+    compare(dw, expect_variant="prefill_sm100_tcgen05")
+    w2 = W.single_request_prefill(name="promptcache", hq=16, hkv=2, d=128, theta=5e5, dtype="bf16", sigma=1.0,
+                                  span_lens=[160, 208, 96], suffix_len=48, num_blocks=64, seed=24)
+    starts = np.unique(w2.q_vis_lo[w2.q_vis_lo > 0]).tolist()
+    seq = np.arange(w2.kv_positions.shape[0])
+    span_of = np.searchsorted(np.asarray([0] + starts), seq, side="right") - 1
+    span_start = np.asarray([0] + starts)[span_of]
+    w2.kv_positions = (4096 * span_of + (seq - span_start)).astype(np.int32)
+    dw2 = DeviceWorkload(w2); dw2.step(); torch.cuda.synchronize()
+    compare(dw2, expect_variant="prefill_sm100_tcgen05")
+
+
 def test_k_prerotated_control_matches():
     """MINIPIC_K_PREROTATED control: a cache holding oracle-rotated keys (rounded to bf16) with the in-kernel
     K RoPE switched off gives the same attention within the same tolerances."""
