@@ -38,6 +38,9 @@ constexpr int kKStages = 2, kVStages = 2, kRing = 4;
 //    finishing item's tile-B slot): parity-green, dense +3 %, but span items -7 % (2.30 ms): the four rotation warps are
 //    saturated at item boundaries (K0', Q_A', Q_B', K1' = 4.5 tile rotations per ~3-tile item) and starting Q earlier only
 //    takes issue slots from the current item's softmax;  a single V stage (needed for a full Q double buffer) costs 7 %;
+//  * K rotation by the eight softmax warps in the gap where they wait for S_FULL (16 rows each, no dedicated rotation
+//    warps): parity-green but 2.78 ms - the exact restart per 16 rows (~600 cycles of dependent latency) lands on the
+//    softmax critical path instead of running ahead on separate warps;
 //  * Q rotation unrolled like the K path, or two rows per iteration: 8 % / 7 % slower (instruction cache);
 //  * L2 prefetch of the next item's Q tiles: no change.
 // Two restructurings of the softmax were measured on config 5 (2.38 ms at the time) and dropped:
