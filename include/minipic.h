@@ -54,7 +54,8 @@ typedef enum {
   MINIPIC_ERR_INVALID_ARG = 1,
   MINIPIC_ERR_UNSUPPORTED = 2,
   MINIPIC_ERR_WORKSPACE_TOO_SMALL = 3,
-  MINIPIC_ERR_CUDA = 4
+  MINIPIC_ERR_CUDA = 4,
+  MINIPIC_ERR_KERNEL_TIMEOUT = 5 /* a hand-off barrier inside the prefill kernel was never signalled (internal fault) */
 } minipic_status;
 
 typedef enum { MINIPIC_BF16 = 0, MINIPIC_F32 = 1 } minipic_dtype;
@@ -174,6 +175,14 @@ int minipic_decode_step_host(const minipic_config* cfg,
                              int32_t num_seqs, int32_t max_kv_len,
                              void* out_host, float* lse_host,
                              void* arena, size_t arena_bytes, void* cuda_stream);
+
+/* Health of the last minipic_prefill_attention call that used `workspace` (DEVICE pointer, as passed to that call).
+ * The tcgen05 prefill kernel is a pipeline of warp roles that hand tiles to each other through mbarriers; every wait is
+ * bounded, and a wait that runs out records the barrier in the workspace header and drains the kernel instead of hanging
+ * the GPU.  This call synchronises `cuda_stream`, reads that word back and returns MINIPIC_OK, MINIPIC_ERR_KERNEL_TIMEOUT
+ * (outputs of that call are then undefined) or MINIPIC_ERR_CUDA.  Optional: the attention calls themselves stay
+ * asynchronous.  Other kernels have no such state; for them (workspace of a call that dispatched elsewhere) it returns OK. */
+int minipic_prefill_status(const void* workspace, void* cuda_stream);
 
 /* ---- misc ---------------------------------------------------------------------------------------*/
 const char* minipic_status_string(int status);

@@ -32,6 +32,7 @@ EXPORTS = [
     "minipic_prefill_host_arena_bytes", "minipic_prefill_step_host",
     "minipic_decode_host_arena_bytes", "minipic_decode_step_host",
     "minipic_status_string", "minipic_last_cuda_error", "minipic_launch_count", "minipic_last_variant",
+    "minipic_prefill_status",
 ]
 
 
@@ -84,6 +85,8 @@ def lib() -> C.CDLL:
     L.minipic_last_cuda_error.restype = C.c_char_p
     L.minipic_launch_count.restype = C.c_uint64
     L.minipic_last_variant.restype = C.c_char_p
+    L.minipic_prefill_status.restype = C.c_int
+    L.minipic_prefill_status.argtypes = [VP, VP]
     _lib = L
     return L
 
@@ -210,3 +213,8 @@ def minipic_launch_count() -> int:
 
 def minipic_last_variant() -> str:
     return lib().minipic_last_variant().decode()
+
+
+def minipic_prefill_status(workspace, stream=None) -> None:
+    """Synchronises the stream and raises if the last tcgen05 prefill call on `workspace` recorded a barrier timeout."""
+    _check(lib().minipic_prefill_status(_ptr(workspace), _stream(stream)))

@@ -99,12 +99,22 @@ const char* minipic_status_string(int status) {
     case MINIPIC_ERR_UNSUPPORTED: return "MINIPIC_ERR_UNSUPPORTED";
     case MINIPIC_ERR_WORKSPACE_TOO_SMALL: return "MINIPIC_ERR_WORKSPACE_TOO_SMALL";
     case MINIPIC_ERR_CUDA: return "MINIPIC_ERR_CUDA";
+    case MINIPIC_ERR_KERNEL_TIMEOUT: return "MINIPIC_ERR_KERNEL_TIMEOUT";
     default: return "MINIPIC_ERR_UNKNOWN";
   }
 }
 const char* minipic_last_cuda_error(void) { return g_cuda_err; }
 uint64_t minipic_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
 const char* minipic_last_variant(void) { return g_variant; }
+
+int minipic_prefill_status(const void* workspace, void* cuda_stream) {
+  if (!workspace) return MINIPIC_ERR_INVALID_ARG;
+  if (std::strcmp(g_variant, "prefill_sm100_tcgen05") != 0) return MINIPIC_OK;   // only that kernel keeps a health word
+  int word = 0;
+  const int e = prefill_sm100_error_word(workspace, (cudaStream_t)cuda_stream, &word);
+  if (e != 0) { std::snprintf(g_cuda_err, sizeof(g_cuda_err), "%s", cudaGetErrorString((cudaError_t)e)); return MINIPIC_ERR_CUDA; }
+  return word == 0 ? MINIPIC_OK : MINIPIC_ERR_KERNEL_TIMEOUT;
+}
 
 size_t minipic_rope_table_bytes(const minipic_config* cfg, int32_t num_positions) {
   if (validate_cfg(cfg) != MINIPIC_OK || num_positions < 0) return 0;

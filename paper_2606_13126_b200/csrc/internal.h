@@ -45,5 +45,6 @@ void launch_decode_mma(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, f
 bool prefill_sm100_supported(const Ctx& c);
 size_t prefill_sm100_workspace_bytes(const Ctx& c, int num_reqs, int num_q_tokens);
 bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a);
+int prefill_sm100_error_word(const void* workspace, cudaStream_t s, int* word);   // cudaError as int; *word = 0 if healthy
 
 }  // namespace minipic

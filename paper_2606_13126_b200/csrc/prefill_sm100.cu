@@ -22,6 +22,7 @@
 //
 // All hand-offs are mbarriers; generic-proxy smem writes are fenced with fence.proxy.async before the MMA reads.
 #include <cuda.h>
+#include <cstddef>
 
 #include "internal.h"
 
@@ -88,7 +89,7 @@ __device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity) {
 }
 // A protocol bug must neither hang the GPU nor kill the context: a wait that exceeds the timeout records
 // (barrier, parity, block, thread) in the plan header, and every thread that sees the flag stops waiting, so the
-// kernel drains and the host can read the error word (prefill_sm100_status()).
+// kernel drains and the host can read the error word (minipic_prefill_status()).
 struct Waiter {
   int* err;
   bool dead;
@@ -1061,6 +1062,13 @@ extern "C" int minipic_debug_trace_copy(long long* host, int* counts) {
   return kTraceLen;
 }
 #endif
+
+int prefill_sm100_error_word(const void* workspace, cudaStream_t st, int* word) {
+  *word = 0;
+  cudaError_t e = cudaMemcpyAsync(word, (const char*)workspace + offsetof(PlanHeader, err), sizeof(int), cudaMemcpyDeviceToHost, st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  return (int)e;
+}
 
 bool prefill_sm100_supported(const Ctx& c) {
   return c.dtype == MINIPIC_BF16 && c.d == 128 && (c.group == 1 || c.group == 2 || c.group == 4 || c.group == 8);

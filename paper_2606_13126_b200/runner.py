@@ -119,6 +119,11 @@ class DeviceWorkload:
         self.write_new()
         self.attention()
 
+    def check_health(self):
+        """Synchronise and raise if the prefill kernel recorded a hand-off timeout (minipic_prefill_status)."""
+        if self.w.kind == "prefill":
+            mp.minipic_prefill_status(self.workspace)
+
     # ---- results back on the host
     def out_f64(self) -> np.ndarray:
         o = self.out

@@ -37,6 +37,7 @@ def test_sass_is_sm100a_only(lib):
 def test_status_strings(lib):
     assert mp.minipic_status_string(0) == "MINIPIC_OK"
     assert mp.minipic_status_string(3) == "MINIPIC_ERR_WORKSPACE_TOO_SMALL"
+    assert mp.minipic_status_string(5) == "MINIPIC_ERR_KERNEL_TIMEOUT"
     assert "UNKNOWN" in mp.minipic_status_string(99)
 
 

@@ -28,6 +28,7 @@ OUT_MAX, OUT_MEAN, LSE_TOL, LSE_CAP = 2e-2, 2e-3, 1e-3, 8e-3
 
 def compare(dw, rows=None, heads=None, oracle_cache=None, expect_variant=None, k_prerot=False):
     w = dw.w
+    dw.check_health()   # no hand-off barrier of the prefill pipeline timed out
     kc, vc = oracle_cache if oracle_cache is not None else O.build_cache(w)
     of, lf = O.run_workload(w, kc, vc, mode="F", rows=rows, heads=heads, k_prerotated=k_prerot)
     variant = mp.minipic_last_variant()
