@@ -43,7 +43,11 @@ constexpr int kKStages = 2, kVStages = 2, kRing = 4;
 //    warps): parity-green but 2.78 ms - the exact restart per 16 rows (~600 cycles of dependent latency) lands on the
 //    softmax critical path instead of running ahead on separate warps;
 //  * Q rotation unrolled like the K path, or two rows per iteration: 8 % / 7 % slower (instruction cache);
-//  * L2 prefetch of the next item's Q tiles: no change.
+//  * L2 prefetch of the next item's Q tiles: no change;  MMA N / K trimmed to the visible columns of a diagonal tile: no
+//    change (the tensor pipe is not the limiter on span items);
+//  * speculative row max (exps against the running max at once, tile max tracked inside the exp loop, redo if it grew by
+//    more than the lazy-rescale threshold): 2.41 ms - the exp loop is issue-bound, 64 more FMNMX in it cost more than the
+//    separate max pass saves;  second half of S loaded from TMEM under the first half's max: no change.
 // Two restructurings of the softmax were measured on config 5 (2.38 ms at the time) and dropped:
 //  * every 2nd / 3rd / 4th exp2 pair on the FMA pipe (Cody-Waite + cubic minimax) instead of MUFU: 2.59 / 2.56 / 2.45 ms -
 //    the softmax warps are issue / latency bound, not MUFU bound, at this tile period;
