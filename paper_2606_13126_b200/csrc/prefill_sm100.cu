@@ -47,7 +47,9 @@ constexpr int kKStages = 2, kVStages = 2, kRing = 4;
 //    change (the tensor pipe is not the limiter on span items);
 //  * speculative row max (exps against the running max at once, tile max tracked inside the exp loop, redo if it grew by
 //    more than the lazy-rescale threshold): 2.41 ms - the exp loop is issue-bound, 64 more FMNMX in it cost more than the
-//    separate max pass saves;  second half of S loaded from TMEM under the first half's max: no change.
+//    separate max pass saves;  second half of S loaded from TMEM under the first half's max: no change;
+//  * mbarrier.try_wait with a suspend-time hint (500 / 4000 ns) to take the wait loops (44 % of the issued instructions)
+//    off the issue slots: no change on dense tiles, 2 % slower on config 5 - try_wait already sleeps in hardware.
 // Two restructurings of the softmax were measured on config 5 (2.38 ms at the time) and dropped:
 //  * every 2nd / 3rd / 4th exp2 pair on the FMA pipe (Cody-Waite + cubic minimax) instead of MUFU: 2.59 / 2.56 / 2.45 ms -
 //    the softmax warps are issue / latency bound, not MUFU bound, at this tile period;
