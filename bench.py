@@ -243,6 +243,8 @@ def run_ours(args):
     roofline = {"kernel": variant5, "bound": "tensor", "achieved": tf, "peak": peaks["bf16_tflops"], "unit": "TFLOP/s",
                 "frac": tf / peaks["bf16_tflops"], "traffic": traffic.get("prefill_dram_bytes_per_launch"),
                 "peak_source": peaks["source"] + " (bf16 burst)", "frac_of_nominal_2250": tf / 2250.0,
+                "frac_of_sustained_peak": tf / peaks["bf16_tflops_sustained"],
+                "note": "duration = plan kernels (~20 us) + prefill kernel of one minipic_prefill_attention call",
                 "algorithmic_flops_per_launch": flops5, "ms_per_launch": seg_mean[1]}
     kvb4 = w4.logical_kv_bytes()
     dec_gbs = kvb4 / (seg_mean[3] * 1e-3) / 1e9
