@@ -204,6 +204,16 @@ def test_other_span_techniques_through_the_same_descriptor():
     compare(dw2, expect_variant="prefill_sm100_tcgen05")
 
 
+@pytest.mark.parametrize("hkv", [1, 3, 8])
+def test_decode_any_kv_head_count(hkv):
+    """The decode launcher packs 4, 2 or 1 warps (KV heads) into a CTA depending on Hkv: cover a single-warp CTA (Hkv = 1,
+    3) and the full one; every warp count has to see the whole 64-entry RoPE phase table."""
+    wd = W.shared_pool_decode(name=f"dec_hkv{hkv}", seed=40 + hkv, hq=2 * hkv, hkv=hkv, num_seqs=5, ctx_min=40, ctx_max=900,
+                              span_len=64, pool_spans=16)
+    dd = DeviceWorkload(wd); dd.step(); torch.cuda.synchronize()
+    compare(dd, expect_variant="decode_mma")
+
+
 def test_k_prerotated_control_matches():
     """MINIPIC_K_PREROTATED control: a cache holding oracle-rotated keys (rounded to bf16) with the in-kernel
     K RoPE switched off gives the same attention within the same tolerances."""
