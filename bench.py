@@ -97,9 +97,11 @@ class ClockSampler(threading.Thread):
 _ORACLE_CACHES = {}
 
 
-def oracle_sample_time(w5, w4, span_rows=1024, suffix_rows=256, heads5=1, seqs4=4, heads4=1):
+def oracle_sample_time(w5, w4, span_rows=1024, suffix_rows=256, heads5=1, seqs4=4, heads4=1, keep=None):
     """Time the oracle, as it stands, on a bounded sample of the step's workload; extrapolate by visible
-    (query, key, head) pair count.  Returns (seconds_per_full_step_estimate, sample description, seconds)."""
+    (query, key, head) pair count.  Returns (seconds_per_full_step_estimate, sample description, seconds).
+    `keep` (a dict) receives the sample's rows / heads and the oracle's outputs, so the cpu_baseline leg can also
+    check the GPU results of the timed launch configuration against them."""
     from oracle import minipic_oracle as O
     for w in (w5, w4):
         if id(w) not in _ORACLE_CACHES:
@@ -110,9 +112,11 @@ def oracle_sample_time(w5, w4, span_rows=1024, suffix_rows=256, heads5=1, seqs4=
     rows = np.concatenate([np.arange(t0, t0 + span_rows), np.arange(t1 - suffix_rows, t1)])
     h5, s4, h4 = np.arange(heads5), np.arange(seqs4), np.arange(heads4)
     tic = time.perf_counter()
-    O.run_workload(w5, kc5, vc5, mode="F", rows=rows, heads=h5)
-    O.run_workload(w4, kc4, vc4, mode="F", rows=s4, heads=h4)
+    o5, l5 = O.run_workload(w5, kc5, vc5, mode="F", rows=rows, heads=h5)
+    o4, l4 = O.run_workload(w4, kc4, vc4, mode="F", rows=s4, heads=h4)
     sec = time.perf_counter() - tic
+    if keep is not None:
+        keep.update(rows5=rows, heads5=h5, out5=o5, lse5=l5, rows4=s4, heads4=h4, out4=o4, lse4=l4)
     pairs5 = int((w5.q_seq_idx[rows].astype(np.int64) - w5.q_vis_lo[rows] + 1).sum()) * heads5
     pairs4 = int(w4.kv_lens[s4].astype(np.int64).sum()) * heads4
     total = w5.visible_pairs() * w5.num_q_heads + w4.visible_pairs() * w4.num_q_heads
@@ -194,8 +198,8 @@ def run_ours(args):
 
     w5 = W.config5(seed=4 + 1000 * rank)
     w4 = W.config4(seed=3 + 1000 * rank)
-    d5 = DeviceWorkload(w5, device=dev, rope_table_positions=w5.max_kv_len)
-    d4 = DeviceWorkload(w4, device=dev, rope_table_positions=w4.max_kv_len)
+    d5 = DeviceWorkload(w5, device=dev)   # no cos/sin table: the bf16 tensor-core kernels compute the phase in-kernel
+    d4 = DeviceWorkload(w4, device=dev)
     tokens_per_step = w5.num_q_tokens + w4.num_q_tokens
 
     def step(ev=None):
@@ -230,6 +234,10 @@ def run_ours(args):
     torch.cuda.synchronize(); dist.barrier()
     sampler.stop_flag.set(); sampler.join(2.0)
     launches = mp.minipic_launch_count() - launches0
+    d5.check_health()    # raises if a hand-off barrier of the prefill pipeline timed out during the timed region
+    # results of the LAST timed step (verified against the oracle sample in the cpu_baseline leg below)
+    out5_timed, lse5_timed = d5.out.clone(), d5.lse.clone()
+    out4_timed, lse4_timed = d4.out.clone(), d4.lse.clone()
     total_s = t_start.elapsed_time(t_end) * 1e-3
     agg = dist.aggregate(tokens_per_step * args.steps, total_s)
     seg = np.array([[e[i].elapsed_time(e[i + 1]) for i in range(4)] for e in evs])   # ms: write5, prefill, write4, decode
@@ -264,7 +272,7 @@ def run_ours(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": {"workload": WORKLOAD, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
                        "l2": "inputs larger than L2: each step touches ~3.5 GB (Q/O 2.2 GB) between repeats of any kernel",
-                       "rope": "in-kernel K and Q rotation; cos/sin from an exact 64-bit fixed-point phase + MUFU (prefill adds an angle-addition recurrence); table built but unused by the bf16 kernels",
+                       "rope": "in-kernel K and Q rotation; cos/sin from an exact 64-bit fixed-point phase + MUFU (prefill adds an angle-addition recurrence; decode shares one (cos, sin) tile per 16-key block between the KV heads of a CTA)",
                        "tokens_per_step": tokens_per_step},
             "roofline": roofline, "roofline_decode": roofline_decode, "roofline_cache_write": roofline_cache_write,
             "kernels_ms": {"c5_cache_write": seg_mean[0], "c5_prefill": seg_mean[1], "c4_cache_write": seg_mean[2],
@@ -294,7 +302,10 @@ def run_ours(args):
     if rank == 0 and world == 1 and not args.no_extras:
         extras = {}
         try:
-            # in-kernel RoPE overhead: same kernel with MINIPIC_K_PREROTATED (timing only: values irrelevant)
+            # in-kernel RoPE overhead: same kernel with MINIPIC_K_PREROTATED.  The flag is flipped on the UNROTATED cache:
+            # timing only, the values of those runs are meaningless (correctness of the flag on a really pre-rotated
+            # cache is tests/test_gpu_parity.py::test_k_prerotated_control_matches)
+            extras["k_prerotated_note"] = "flag-only on the unrotated cache: timing control, outputs not meaningful"
             t_rope = time_calls(d5.attention, 10, 2, torch)
             d5.set_flags(mp.MINIPIC_K_PREROTATED)
             t_pre = time_calls(d5.attention, 10, 2, torch)
@@ -308,7 +319,7 @@ def run_ours(args):
             flush = torch.empty(512 * 1024 * 1024, dtype=torch.uint8, device=dev)
             for name, mk in (("c2", W.config2), ("c3", W.config3)):
                 w = mk()
-                dw = DeviceWorkload(w, device=dev, rope_table_positions=w.max_kv_len)
+                dw = DeviceWorkload(w, device=dev)
                 def f():
                     flush.zero_()
                     dw.attention()
@@ -327,7 +338,7 @@ def run_ours(args):
                                 "tflops_warm": fl / (warm[0] * 1e-3) / 1e12, "variant": mp.minipic_last_variant()}
                 del dw
             wp = W.config4(private_pool=True)
-            dp = DeviceWorkload(wp, device=dev, rope_table_positions=wp.max_kv_len)
+            dp = DeviceWorkload(wp, device=dev)
             dp.step(); torch.cuda.synchronize()
             tp = time_calls(dp.attention, 20, 3, torch)
             gb = wp.logical_kv_bytes() / (tp[0] * 1e-3) / 1e9
@@ -344,9 +355,24 @@ def run_ours(args):
 
     # ---- CPU oracle baseline (rank 0, N = 1 only)
     if rank == 0 and world == 1:
-        est, desc, sec = oracle_sample_time(w5, w4)
+        keep = {}
+        est, desc, sec = oracle_sample_time(w5, w4, keep=keep)
         line["cpu_baseline"] = {"value": tokens_per_step / est, "unit": UNIT, "cores": host_threads(), "kind": "oracle",
                                 "sample": desc, "sample_seconds": sec}
+        # the same oracle sample doubles as a check of what the timed region produced (full size, bench launch shape)
+        def _dev_f64(t, bf16=True):
+            return (t.view(torch.bfloat16) if bf16 else t).double().cpu().numpy()
+        chk = {}
+        for tag, o_g, l_g, rows, heads, o_o, l_o in (
+                ("c5", out5_timed, lse5_timed, keep["rows5"], keep["heads5"], keep["out5"], keep["lse5"]),
+                ("c4", out4_timed, lse4_timed, keep["rows4"], keep["heads4"], keep["out4"], keep["lse4"])):
+            ix = np.ix_(rows, heads)
+            do = np.abs(_dev_f64(o_g)[ix] - o_o[ix]); dl = np.abs(_dev_f64(l_g, False)[ix] - l_o[ix])
+            chk[tag] = {"rows": int(len(rows)), "heads": int(len(heads)), "out_max_abs": float(do.max()),
+                        "out_mean_abs": float(do.mean()), "lse_mean_abs": float(dl.mean()), "lse_max_abs_F": float(dl.max())}
+        ok = all(c["out_max_abs"] <= 2e-2 and c["out_mean_abs"] <= 2e-3 and c["lse_mean_abs"] <= 1e-3 for c in chk.values())
+        line["verified"] = {"ok": bool(ok), "prefill_health": "ok", "against": "oracle mode F on the cpu_baseline sample",
+                            "gates": "out max-abs 2e-2, mean-abs 2e-3; LSE mean-abs 1e-3", **chk}
     if rank == 0:
         print(json.dumps(line), flush=True)
     dist.shutdown()

@@ -17,7 +17,8 @@
  * Conventions (every entry point):
  *   * All array arguments are DEVICE pointers owned by the caller unless the name ends in
  *     `_host` (see the *_host entry points at the end).  The library allocates nothing on the
- *     device path, keeps no state between calls and never synchronises the stream.
+ *     device path, keeps no state between calls (beyond the diagnostics at the end of this file: a launch counter
+ *     and per-thread last-error / last-variant strings) and never synchronises the stream.
  *   * `cuda_stream` is a cudaStream_t passed as void* (NULL = legacy default stream).
  *   * The return value is a minipic_status.  Argument errors are detected on the host before
  *     any launch.  Out-of-range block ids / slots / positions are undefined behaviour.
@@ -79,8 +80,11 @@ typedef struct {
   uint32_t flags;        /* MINIPIC_* bits                                         */
   /* Optional cos/sin table ("a cos/sin table lookup"): device float2
    * [rope_table_len][head_dim/2] = (cos, sin)(p * f_i), built by minipic_rope_table_build for this
-   * (rope_theta, head_dim).  Positions >= rope_table_len (or a NULL table) are computed inside the
-   * kernels from a 64-bit fixed-point phase, to the same accuracy (~2e-7). */
+   * (rope_theta, head_dim).  It is read ONLY by the generic fp32 CUDA-core kernels (fp32 I/O, head_dim 64,
+   * MINIPIC_FORCE_SIMT); positions >= rope_table_len (or a NULL table) are computed there from a 64-bit
+   * fixed-point phase to the same accuracy (~2e-7).  The bf16 tensor-core kernels (head_dim 128) IGNORE the
+   * table: they always compute the phase in-kernel (a table read per K tile would cost as much on-chip
+   * traffic as the tile itself), so callers of those shapes need not build one. */
   const void* rope_table;
   int32_t rope_table_len;
   int32_t reserved;
@@ -176,12 +180,14 @@ int minipic_decode_step_host(const minipic_config* cfg,
                              void* out_host, float* lse_host,
                              void* arena, size_t arena_bytes, void* cuda_stream);
 
-/* Health of the last minipic_prefill_attention call that used `workspace` (DEVICE pointer, as passed to that call).
+/* Health of the last tcgen05 minipic_prefill_attention call that used `workspace` (DEVICE pointer, as passed to that call).
  * The tcgen05 prefill kernel is a pipeline of warp roles that hand tiles to each other through mbarriers; every wait is
  * bounded, and a wait that runs out records the barrier in the workspace header and drains the kernel instead of hanging
- * the GPU.  This call synchronises `cuda_stream`, reads that word back and returns MINIPIC_OK, MINIPIC_ERR_KERNEL_TIMEOUT
- * (outputs of that call are then undefined) or MINIPIC_ERR_CUDA.  Optional: the attention calls themselves stay
- * asynchronous.  Other kernels have no such state; for them (workspace of a call that dispatched elsewhere) it returns OK. */
+ * the GPU.  This call synchronises `cuda_stream`, reads the header's (error word, kernel tag) back and returns MINIPIC_OK,
+ * MINIPIC_ERR_KERNEL_TIMEOUT (outputs of that call are then undefined) or MINIPIC_ERR_CUDA.  The state lives in the
+ * workspace, not in the library: the answer is the same from any host thread and whatever was called in between.  The
+ * other kernels keep no health word and never write the header; a workspace that no tcgen05 call has used reads as OK.
+ * Optional: the attention calls themselves stay asynchronous. */
 int minipic_prefill_status(const void* workspace, void* cuda_stream);
 
 /* ---- misc ---------------------------------------------------------------------------------------*/

@@ -14,6 +14,18 @@ static thread_local char g_cuda_err[256] = "";
 static thread_local const char* g_variant = "";
 
 void note_launch(int n) { g_launches.fetch_add((uint64_t)n, std::memory_order_relaxed); }
+void note_error(const char* what) { snprintf(g_cuda_err, sizeof(g_cuda_err), "%s", what); }
+int current_sm_count() {   // SM count of the CURRENT device (cached per device ordinal)
+  static std::atomic<int> cache[64];
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return 148;
+  int sms = cache[dev].load(std::memory_order_relaxed);
+  if (sms == 0) {
+    if (cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) sms = 148;
+    cache[dev].store(sms, std::memory_order_relaxed);
+  }
+  return sms;
+}
 bool check_launch(const char* what) {
   cudaError_t e = cudaGetLastError();
   if (e == cudaSuccess) return true;
@@ -69,7 +81,7 @@ SplitPlan decode_split_plan(const Ctx& c, int num_seqs, int max_kv_len) {
   // scalars only so that the grid has >= ~8 waves of (sequence, split) slices when the batch allows it (swept 3..16 on
   // config 4: 1.15 / 1.15 / 1.12 / 1.10 / 1.10 / 1.13 ms for 3 / 4 / 6 / 8 / 12 / 16).
   SplitPlan sp;
-  int sms = 148;
+  const int sms = current_sm_count();
   const long long want_ctas = (long long)sms * 2 * 8;
   long long per_seq = (want_ctas + num_seqs - 1) / (num_seqs > 0 ? num_seqs : 1);
   if (per_seq < 1) per_seq = 1;
@@ -110,7 +122,8 @@ const char* minipic_last_variant(void) { return g_variant; }
 
 int minipic_prefill_status(const void* workspace, void* cuda_stream) {
   if (!workspace) return MINIPIC_ERR_INVALID_ARG;
-  if (std::strcmp(g_variant, "prefill_sm100_tcgen05") != 0) return MINIPIC_OK;   // only that kernel keeps a health word
+  // the health word lives in the workspace header, tagged by the kernel that keeps one: the answer does not depend on
+  // which thread asks or on what this thread called in between
   int word = 0;
   const int e = prefill_sm100_error_word(workspace, (cudaStream_t)cuda_stream, &word);
   if (e != 0) { std::snprintf(g_cuda_err, sizeof(g_cuda_err), "%s", cudaGetErrorString((cudaError_t)e)); return MINIPIC_ERR_CUDA; }
@@ -208,6 +221,7 @@ int minipic_decode_attention(const minipic_config* cfg, const void* q, const voi
   if (workspace_bytes < need || !workspace) return MINIPIC_ERR_WORKSPACE_TOO_SMALL;
   if ((uintptr_t)workspace & 255) return MINIPIC_ERR_INVALID_ARG;
   const SplitPlan sp = decode_split_plan(c, num_seqs, max_kv_len);
+  if ((long long)num_seqs * sp.max_splits > 0x7fffffffLL) return MINIPIC_ERR_UNSUPPORTED;   // (sequence, split) is grid.x
   const size_t rows = (size_t)num_seqs * c.hq * sp.max_splits;
   float* o_part = (float*)workspace;
   float* lse_part = (float*)((char*)workspace + align_up(rows * c.d * sizeof(float)));

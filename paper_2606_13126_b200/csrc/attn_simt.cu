@@ -99,12 +99,12 @@ __global__ void __launch_bounds__(128) prefill_simt_kernel(PrefillArgs a, int hq
   if (lane == 0) a.lse[(size_t)t * hq + h] = wa.l_run > 0.f ? wa.m_run + logf(wa.l_run) : -INFINITY;
 }
 
-// decode partial: grid (split, head, seq); one warp per CTA
+// decode partial: grid (seq * max_splits + split, head); one warp per CTA (the sequence count lives in grid.x: no 65535 limit)
 template <typename T, int D>
 __global__ void __launch_bounds__(32) decode_simt_kernel(DecodeArgs a, int hq, int hkv, float scale, RopeParams rp,
                                                          unsigned flags, int split_len, int max_splits,
                                                          float* __restrict__ o_part, float* __restrict__ lse_part) {
-  const int lane = threadIdx.x, s = blockIdx.x, h = blockIdx.y, r = blockIdx.z;
+  const int lane = threadIdx.x, s = blockIdx.x % max_splits, r = blockIdx.x / max_splits, h = blockIdx.y;
   const int kv_len = __ldg(a.kv_lens + r);
   if (s * split_len >= kv_len) return;  // empty split: the merge kernel never reads it
   const int idx = kv_len - 1;
@@ -134,7 +134,7 @@ __global__ void __launch_bounds__(128) lse_merge_kernel(const float* __restrict_
   if (w >= num_seqs * hq) return;
   const int r = w / hq;
   const int kv_len = __ldg(kv_lens + r);
-  const int ns = (kv_len + split_len - 1) / split_len;
+  const int ns = min((kv_len + split_len - 1) / split_len, max_splits);   // kv_len > max_kv_len is a caller error: stay inside the row
   const float* lp = lse_part + (size_t)w * max_splits;
   const float* op = o_part + (size_t)w * max_splits * D;
   float m = -INFINITY;
@@ -175,7 +175,7 @@ void launch_prefill_simt(const Ctx& c, const PrefillArgs& a) {
 
 template <typename T, int D>
 static void decode_simt_t(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, float* o_part, float* lse_part) {
-  dim3 grid(sp.max_splits, c.hq, a.num_seqs);
+  dim3 grid((unsigned)sp.max_splits * (unsigned)a.num_seqs, c.hq);
   decode_simt_kernel<T, D><<<grid, 32, 0, c.stream>>>(a, c.hq, c.hkv, c.scale, c.rope, c.flags, sp.split_len,
                                                       sp.max_splits, o_part, lse_part);
   note_launch();

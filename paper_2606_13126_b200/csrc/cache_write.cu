@@ -51,8 +51,7 @@ void launch_cache_write(int itemsize, int hkv, int d, const void* k_new, const v
   const int row_vecs = d * itemsize / 16;
   const long long total = (long long)num_tokens * hkv * row_vecs;
   constexpr int kUnroll = 4;
-  int sms = 148;
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, 0);
+  const int sms = current_sm_count();
   long long blocks = (total + 256LL * kUnroll - 1) / (256LL * kUnroll);
   const long long cap = (long long)sms * 16;  // 8 resident CTAs/SM x 2 waves; grid-stride beyond that
   if (blocks > cap) blocks = cap;
@@ -79,7 +78,7 @@ void launch_rope_table(const RopeParams& rp, int num_positions, float2* table, c
   if (num_positions <= 0) return;
   const long long n = (long long)num_positions * rp.half;
   long long blocks = (n + 255) / 256;
-  if (blocks > 148 * 8) blocks = 148 * 8;
+  if (blocks > current_sm_count() * 8LL) blocks = current_sm_count() * 8LL;
   rope_table_kernel<<<(unsigned)blocks, 256, 0, s>>>(rp, num_positions, table);
   note_launch();
 }

@@ -67,6 +67,29 @@ __device__ __forceinline__ uint4 ldg_stream16(const void* p) {  // 16-byte strea
   return r;
 }
 
+// packed fp32 pairs (one 64-bit register = two lanes of an FFMA2)
+__device__ __forceinline__ uint64_t pk2(float a, float b) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+  return r;
+}
+__device__ __forceinline__ void upk2(uint64_t v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t d;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+  return d;
+}
+__device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+  uint64_t d;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+  return d;
+}
+
 // ------------------------------------------------------------------------------------ host side
 struct Ctx {  // what every launcher needs, derived once from minipic_config
   int hq, hkv, d, group, num_blocks;
@@ -80,6 +103,8 @@ struct Ctx {  // what every launcher needs, derived once from minipic_config
 };
 
 void note_launch(int n = 1);
+void note_error(const char* what);    // text for minipic_last_cuda_error() on non-CUDA failure paths
+int current_sm_count();               // SMs of the current device
 bool check_launch(const char* what);  // cudaGetLastError -> records text, returns ok
 
 }  // namespace minipic

@@ -7,6 +7,8 @@
 // bf16->fp32 conversion and the two FMAs per K element.  The G query heads of the group share the
 // rotated K tile.  Online softmax uses warp shuffles across the 4 lanes that hold one head's scores.
 // Partials (o_s normalised over the split, lse_s) go to the workspace; lse_merge_kernel (a11) combines them.
+// The W warps of a CTA are W KV heads of the SAME (sequence, split): they share the (cos, sin) tile of every 16-key block
+// through a small shared-memory ring instead of each recomputing it (see "cos/sin ring" below).
 //
 // Fragment trick: the dot products are sums over head_dim (QK^T) and over keys (PV), so any permutation of the
 // summation index is legal as long as both operands use it.  That lets each lane feed the MMA fragments from
@@ -33,8 +35,8 @@ __device__ __forceinline__ void mma16816(float (&d)[4], unsigned a0, unsigned a1
 
 // cos/sin of 8 consecutive frequencies i0..i0+7 at position p, computed in registers: exact 64-bit fixed-point phase
 // (common.cuh) -> signed half-turns -> MUFU sin/cos on the reduced angle in [-pi, pi) (|err| < 1e-6, far below the
-// bf16 rounding of the rotated operand).  No memory traffic: in this HBM-bound kernel a cos/sin table lookup
-// costs as many L1 wavefronts as the KV stream itself (ncu: l1tex 92% with the table, profiles/).
+// bf16 rounding of the rotated operand).  No global-memory traffic: in this HBM-bound kernel a cos/sin table lookup
+// from global memory costs as many L1 wavefronts as the KV stream itself (ncu: l1tex 92% with the table).
 __device__ __forceinline__ void rope_cs8(const unsigned long long* __restrict__ finc, int p, int i0, float (&c)[8],
                                          float (&s)[8]) {
 #pragma unroll
@@ -60,21 +62,78 @@ __device__ __forceinline__ void rotate_chunks(uint4& lo, uint4& hi, const float 
   }
 }
 
-template <bool kRotK>
-__global__ void __launch_bounds__(128, 4)   // 4-warp CTAs: 6 % faster than 8-warp CTAs at the same 16 warps / SM (finer-grained block scheduling)
+// ---- cos/sin ring shared by the warps (KV heads) of a CTA ------------------------------------------------------------
+// The warps of a CTA work on the SAME 16 key positions of the same (sequence, split); only the KV head differs.  The
+// (cos, sin) tile of a block - 16 positions x 64 frequencies - is therefore computed ONCE per CTA: every warp computes 1/W
+// of it for the block kLook iterations ahead (8 * 4/W exact evaluations per lane instead of 32), stores it to a ring of
+// kSlots tiles in shared memory, and picks up its own 32 pairs with 16 LDS.128.  Hand-off is two mbarriers per slot
+// (full / empty, one arrival per warp), so the warps stay loosely coupled (up to kLook blocks of skew) instead of running
+// in lock step.  Tile layout: row r (512 B) x 8 chunks of 8 frequencies (64 B) x 4 pieces of 16 B = (c0, c1, s0, s1) of two
+// neighbouring frequencies - the operand order of the packed f32x2 rotation; the piece index is XOR-swizzled with
+// ((r & 1) << 1 | (chunk >> 1) & 1) so that both the writers' and the readers' quarter-warps touch 32 distinct banks.
+constexpr int kSlots = 4, kLook = 2, kCsTileBytes = kBlock * 512;
+constexpr unsigned kSpinLimit = 1u << 26;
+
+__device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  unsigned spins = 0;
+  for (;;) {
+    uint32_t done;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+    if (done) return;
+    if (++spins > kSpinLimit) __trap();   // a protocol bug must fail loudly instead of hanging the GPU
+  }
+}
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ void sts128(uint32_t addr, float a, float b, float c, float d) {
+  asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
+}
+// rotate word w of a (lo, hi) chunk pair with the piece (c0, c1, s0, s1): packed f32x2 math, one RN to bf16
+__device__ __forceinline__ void rotate_word(unsigned& l, unsigned& h, const uint4& cs) {
+  const uint64_t a = pk2(bf16lo(l), bf16hi(l)), b = pk2(bf16lo(h), bf16hi(h));
+  const uint64_t c = ((uint64_t)cs.y << 32) | cs.x, s = ((uint64_t)cs.w << 32) | cs.z;
+  const uint64_t ns = mul2(s, pk2(-1.f, -1.f));
+  float x0, x1, y0, y1;
+  upk2(fma2(b, ns, mul2(a, c)), x0, x1);
+  upk2(fma2(a, s, mul2(b, c)), y0, y1);
+  l = pack_bf16(x0, x1);
+  h = pack_bf16(y0, y1);
+}
+
+template <bool kRotK, int W>
+__global__ void __launch_bounds__(32 * W, 16 / W)   // 16 warps / SM; 4-warp CTAs measured 6 % faster than 8-warp CTAs
 decode_mma_kernel(DecodeArgs a, int hq, int hkv, int group, float scale_log2, RopeParams rp, unsigned flags,
                   int split_len, int max_splits, float* __restrict__ o_part, float* __restrict__ lse_part) {
   constexpr int D = 128;
   __shared__ unsigned long long finc[64];  // F_i: 64-bit fixed-point phase increments (turns per position)
-  if (threadIdx.x < 64) finc[threadIdx.x] = rp.phase_inc[threadIdx.x];
-  if (blockDim.x == 32) finc[threadIdx.x + 32] = rp.phase_inc[threadIdx.x + 32];   // a CTA can be a single warp (odd Hkv)
+  __shared__ __align__(128) unsigned char cs_ring[kRotK ? kSlots * kCsTileBytes : 16];
+  __shared__ unsigned long long bars[2 * kSlots];
+  for (int i = threadIdx.x; i < 64; i += 32 * W) finc[i] = rp.phase_inc[i];
+  if (kRotK && threadIdx.x == 0) {
+    for (int i = 0; i < 2 * kSlots; ++i) mbar_init(smem_addr(&bars[i]), W);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
   __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int g = lane >> 2, q4 = lane & 3;
-  const int s = blockIdx.x, r = blockIdx.y;
-  const int kvh = blockIdx.z * (blockDim.x >> 5) + warp;
+  const int s = blockIdx.x % max_splits, r = blockIdx.x / max_splits;   // the sequence count lives in grid.x: no 65535 limit
+  const int kvh = blockIdx.y * W + warp;
   const int kv_len = __ldg(a.kv_lens + r);
-  if (s * split_len >= kv_len) return;  // the merge kernel never reads empty splits
+  if (s * split_len >= kv_len) return;  // the merge kernel never reads empty splits (uniform over the CTA)
   const int vis_lo = a.q_vis_lo ? max(__ldg(a.q_vis_lo + r), 0) : 0;
   const int j_begin = max(vis_lo, s * split_len), j_end = min(kv_len, (s + 1) * split_len);
   const int* __restrict__ pos = a.kv_positions + __ldg(a.cu_kv_lens + r);
@@ -116,8 +175,39 @@ decode_mma_kernel(DecodeArgs a, int hq, int hkv, int group, float scale_log2, Ro
   float m_run = -INFINITY, l_run = 0.f;
 
   const int kb0 = j_begin / kBlock, kb1 = (j_end + kBlock - 1) / kBlock;
+
+  // ---- this lane's share of a (cos, sin) tile: rows prow0 + 4 i (i < 4 / W), frequency chunk pc
+  const int pc = (lane & 3) + 4 * ((lane >> 3) & 1);
+  const int prow0 = warp * (kBlock / W) + ((lane >> 2) & 1) + 2 * (lane >> 4);
+  const uint32_t ring0 = smem_addr(cs_ring), bar0 = smem_addr(bars);
+  const uint32_t psw = (uint32_t)((((lane >> 2) & 1) << 1) | ((pc >> 1) & 1));   // row parity of prow0 + 4 i = (lane >> 2) & 1
+  const uint32_t rsw = (uint32_t)(((g & 1) << 1) | (q4 >> 1));                   // reader: rows g, g + 8, chunks q4, q4 + 4
+  auto produce = [&](int n) {   // tile of block kb0 + n -> slot n % kSlots
+    const int slot = n % kSlots, kb = kb0 + n;
+    if (n >= kSlots) mbar_wait(bar0 + 8u * (kSlots + slot), ((n / kSlots) & 1) ^ 1);   // every warp is done with block n - kSlots
+    const uint32_t tile = ring0 + slot * kCsTileBytes;
+#pragma unroll
+    for (int i = 0; i < 4 / W; ++i) {
+      const int row = prow0 + 4 * i;
+      const int p = __ldg(pos + min(kb * kBlock + row, kv_len - 1));
+      float c[8], sn[8];
+      rope_cs8(finc, p, pc * 8, c, sn);
+      const uint32_t base = tile + row * 512 + pc * 64;
+#pragma unroll
+      for (int k = 0; k < 4; ++k) sts128(base + ((k ^ psw) << 4), c[2 * k], c[2 * k + 1], sn[2 * k], sn[2 * k + 1]);
+    }
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar0 + 8u * slot);
+  };
+  if (kRotK) {
+#pragma unroll 1
+    for (int n = 0; n < kLook && kb0 + n < kb1; ++n) produce(n);
+  }
+
   int blk = __ldg(bt + kb0);
+#pragma unroll 1
   for (int kb = kb0; kb < kb1; ++kb) {
+    const int n = kb - kb0;
     const size_t base = ((size_t)blk * hkv + kvh) * (kBlock * D);
     if (kb + 1 < kb1) blk = __ldg(bt + kb + 1);
     // ---- a4: K rows g and g+8, chunks q4 + 4j: 8 x 16-byte streaming loads
@@ -126,19 +216,25 @@ decode_mma_kernel(DecodeArgs a, int hq, int hkv, int group, float scale_log2, Ro
     for (int t = 0; t < 2; ++t)
 #pragma unroll
       for (int j = 0; j < 4; ++j) kr[t][j] = ldg_stream16(kc + base + (g + 8 * t) * D + (q4 + 4 * j) * 8);
-    // ---- a5: rotate in registers at pi_r(j)
+    // ---- a5: rotate in registers at pi_r(j); cos/sin from the CTA's shared tile (this warp's share of the tile kLook
+    //      blocks ahead is computed first, under the latency of the loads above)
     if (kRotK) {
+      if (kb + kLook < kb1) produce(n + kLook);
+      const int slot = n % kSlots;
+      mbar_wait(bar0 + 8u * slot, (n / kSlots) & 1);
+      const uint32_t tile = ring0 + slot * kCsTileBytes;
 #pragma unroll
-      for (int t = 0; t < 2; ++t) {
-        const int jrow = kb * kBlock + g + 8 * t;
-        const int p = __ldg(pos + min(jrow, kv_len - 1));
+      for (int t = 0; t < 2; ++t)
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
-          float c[8], sn[8];
-          rope_cs8(finc, p, (q4 + 4 * j) * 8, c, sn);
-          rotate_chunks(kr[t][j], kr[t][j + 2], c, sn);
+          const uint32_t src = tile + (g + 8 * t) * 512 + (q4 + 4 * j) * 64;
+          unsigned* l = reinterpret_cast<unsigned*>(&kr[t][j]);
+          unsigned* h = reinterpret_cast<unsigned*>(&kr[t][j + 2]);
+#pragma unroll
+          for (int k = 0; k < 4; ++k) rotate_word(l[k], h[k], lds128(src + ((k ^ rsw) << 4)));
         }
-      }
+      __syncwarp();
+      if (lane == 0) mbar_arrive(bar0 + 8u * (kSlots + slot));   // this warp no longer needs the tile
     }
     // ---- a6: S^T[head, key] for the two 8-key halves of the block
     float st[2][4];
@@ -232,22 +328,27 @@ decode_mma_kernel(DecodeArgs a, int hq, int hkv, int group, float scale_log2, Ro
   }
 }
 
+template <int W>
+void launch_w(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, float* o_part, float* lse_part) {
+  dim3 grid((unsigned)sp.max_splits * (unsigned)a.num_seqs, c.hkv / W);
+  if (c.flags & MINIPIC_K_PREROTATED)
+    decode_mma_kernel<false, W><<<grid, 32 * W, 0, c.stream>>>(a, c.hq, c.hkv, c.group, c.scale_log2, c.rope, c.flags,
+                                                               sp.split_len, sp.max_splits, o_part, lse_part);
+  else
+    decode_mma_kernel<true, W><<<grid, 32 * W, 0, c.stream>>>(a, c.hq, c.hkv, c.group, c.scale_log2, c.rope, c.flags,
+                                                              sp.split_len, sp.max_splits, o_part, lse_part);
+}
+
 }  // namespace
 
 bool decode_mma_supported(const Ctx& c) { return c.dtype == MINIPIC_BF16 && c.d == 128 && c.group <= 8; }
 
 void launch_decode_mma(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, float* o_part, float* lse_part) {
   if (a.num_seqs == 0) return;
-  int warps = 1;
-  for (int w = 4; w >= 1; --w)
-    if (c.hkv % w == 0) { warps = w; break; }
-  dim3 grid(sp.max_splits, a.num_seqs, c.hkv / warps);
-  if (c.flags & MINIPIC_K_PREROTATED)
-    decode_mma_kernel<false><<<grid, 32 * warps, 0, c.stream>>>(a, c.hq, c.hkv, c.group, c.scale_log2, c.rope, c.flags,
-                                                               sp.split_len, sp.max_splits, o_part, lse_part);
-  else
-    decode_mma_kernel<true><<<grid, 32 * warps, 0, c.stream>>>(a, c.hq, c.hkv, c.group, c.scale_log2, c.rope, c.flags,
-                                                              sp.split_len, sp.max_splits, o_part, lse_part);
+  // W warps = W KV heads of one (sequence, split) per CTA; they share the (cos, sin) tiles through shared memory
+  if (c.hkv % 4 == 0) launch_w<4>(c, a, sp, o_part, lse_part);
+  else if (c.hkv % 2 == 0) launch_w<2>(c, a, sp, o_part, lse_part);
+  else launch_w<1>(c, a, sp, o_part, lse_part);
   note_launch();
 }
 

@@ -70,7 +70,10 @@ constexpr int kMaxBins = 4096;
 constexpr unsigned kWaitMaxSpins = 1u << 26;   // x (>= 30 cycles per failed try_wait) = seconds
 
 struct TileDesc { int t0, ntok, r, idx0, lo, n_kv, kv_hi, kv_len, kv_off, pad; };   // kv_off = cu_kv_lens[r]
-struct PlanHeader { int n_tiles; int next_item; int err; int err_info[5]; int pad[56]; int hist[kMaxBins]; };
+// magic tags a header written by THIS kernel family, so minipic_prefill_status() can tell it from a workspace that a call
+// dispatched to another kernel never touched (err and magic are adjacent: one 8-byte read)
+constexpr int kPlanMagic = 0x4d504943;   // "MPIC"
+struct PlanHeader { int n_tiles; int next_item; int err; int magic; int err_info[4]; int pad[56]; int hist[kMaxBins]; };
 struct ItemInfo { int t0, ntok, r, idx0, lo, kvh, n_kv, kv_hi, kv_len, kv_off, pad[2]; };   // 48 B ring entry; t0 < 0 = stop
 
 // ------------------------------------------------------------------------------------------------ PTX wrappers
@@ -211,28 +214,6 @@ __device__ __forceinline__ float max3(float a, float b, float c) {
   asm("max.f32 %0, %1, %2, %3;" : "=f"(d) : "f"(a), "f"(b), "f"(c));
   return d;
 }
-// packed fp32 pairs (one 64-bit register = two lanes of an FFMA2)
-__device__ __forceinline__ uint64_t pk2(float a, float b) {
-  uint64_t r;
-  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
-  return r;
-}
-__device__ __forceinline__ void upk2(uint64_t v, float& a, float& b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
-__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
-  uint64_t d;
-  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-  return d;
-}
-__device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) {
-  uint64_t d;
-  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-  return d;
-}
-__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
-  uint64_t d;
-  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-  return d;
-}
 __device__ __forceinline__ uint4 lds128(uint32_t addr) {
   uint4 v;
   asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
@@ -268,6 +249,7 @@ __device__ __forceinline__ bool tile_starts(const PrefillArgs& a, int t, int r, 
 // one thread per query token: the tokens that start a super-tile emit its descriptor and count it in the cost histogram
 __global__ void __launch_bounds__(256) plan_mark_kernel(PrefillArgs a, int tok, PlanHeader* hdr, TileDesc* tmp) {
   const int t = blockIdx.x * blockDim.x + threadIdx.x;
+  if (t == 0) hdr->magic = kPlanMagic;
   if (t >= a.num_q_tokens) return;
   int lo_r = 0, hi_r = a.num_reqs;
   while (hi_r - lo_r > 1) {
@@ -1023,11 +1005,15 @@ template <int G>
 bool launch_g(const Ctx& c, const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mo,
               const Params& prm, int sms) {
   const size_t smem = sizeof(Smem);
-  static bool attr_done = false;
-  if (!attr_done) {
-    if (cudaFuncSetAttribute(prefill_sm100_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess)
+  static bool attr_done[64] = {};   // the attribute is per (function, device): track it per device ordinal
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (dev < 0 || dev >= 64 || !attr_done[dev]) {
+    if (cudaFuncSetAttribute(prefill_sm100_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+      note_error("prefill_sm100: cudaFuncSetAttribute(MaxDynamicSharedMemorySize) failed");
       return false;
-    attr_done = true;
+    }
+    if (dev >= 0 && dev < 64) attr_done[dev] = true;
   }
   prefill_sm100_kernel<G><<<sms, kThreads, smem, c.stream>>>(mq, mk, mv, mo, prm);
   note_launch();
@@ -1049,8 +1035,11 @@ extern "C" int minipic_debug_trace_copy(long long* host, int* counts) {
 
 int prefill_sm100_error_word(const void* workspace, cudaStream_t st, int* word) {
   *word = 0;
-  cudaError_t e = cudaMemcpyAsync(word, (const char*)workspace + offsetof(PlanHeader, err), sizeof(int), cudaMemcpyDeviceToHost, st);
+  int pair[2] = {0, 0};   // {err, magic}
+  static_assert(offsetof(PlanHeader, magic) == offsetof(PlanHeader, err) + sizeof(int), "err and magic must be adjacent");
+  cudaError_t e = cudaMemcpyAsync(pair, (const char*)workspace + offsetof(PlanHeader, err), sizeof(pair), cudaMemcpyDeviceToHost, st);
   if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+  if (e == cudaSuccess && pair[1] == kPlanMagic) *word = pair[0];   // any other tag: not a header of this kernel -> healthy
   return (int)e;
 }
 
@@ -1065,8 +1054,10 @@ size_t prefill_sm100_workspace_bytes(const Ctx&, int, int num_q_tokens) {
 bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
   CUtensorMap mq, mk, mv, mo;
   if (!make_cache_map(&mk, a.k_cache, c.num_blocks, c.hkv) || !make_cache_map(&mv, a.v_cache, c.num_blocks, c.hkv) ||
-      !make_q_map(&mq, a.q, a.num_q_tokens, c.hq, c.group) || !make_out_map(&mo, a.out, a.num_q_tokens, c.hq, c.group))
+      !make_q_map(&mq, a.q, a.num_q_tokens, c.hq, c.group) || !make_out_map(&mo, a.out, a.num_q_tokens, c.hq, c.group)) {
+    note_error("prefill_sm100: cuTensorMapEncodeTiled failed (driver entry point missing or bad tensor geometry)");
     return false;
+  }
   PlanHeader* hdr = (PlanHeader*)a.workspace;
   TileDesc* sorted = (TileDesc*)((char*)a.workspace + sizeof(PlanHeader));
   TileDesc* tmp = sorted + (a.num_q_tokens + 1);
@@ -1087,9 +1078,7 @@ bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
     prm.step1[i] = make_float2((float)c1, (float)s1);
     prm.step4[i] = make_float2((float)(c2 * c2 - s2 * s2), (float)(2.0 * s2 * c2));
   }
-  int dev = 0, sms = 148;
-  cudaGetDevice(&dev);
-  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  const int sms = current_sm_count();
   switch (c.group) {
     case 1: return launch_g<1>(c, mq, mk, mv, mo, prm, sms);
     case 2: return launch_g<2>(c, mq, mk, mv, mo, prm, sms);

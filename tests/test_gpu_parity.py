@@ -4,14 +4,28 @@ seeded inputs.  All tests here need a GPU (-m gpu).
 Bars (BASELINE.json north_star, reading R1):
   * cache write, block-table indexing: bit exact.
   * bf16 I/O attention output: max-abs <= 2e-2 and mean-abs <= 2e-3 against the pure-fp64 oracle (mode F).
-  * LSE: mean-abs <= 1e-3 against mode F, and against the oracle whose score operands have the kernel's
-    precision (mode Q = q', k_j rounded to bf16 for the tensor-core kernels; mode F for the fp32 CUDA-core
-    kernels): max-abs <= 1e-3 for the CUDA-core kernels; for the tensor-core kernels <= 1e-3 on at least 99.9 %
-    of the entries and <= 8e-3 everywhere - the kernel rotates in fp32 and the oracle in fp64, so an operand
-    that lands within ~1e-7 relative of a bf16 rounding boundary can round the other way (one bf16 ulp of one
-    of the 256 operand elements of a score), which shows up undamped in rows that see only a few keys.
+  * LSE: mean-abs <= 1e-3 against mode F, and max-abs against the oracle whose score operands have the kernel's
+    precision (mode Q = q', k_j rounded to bf16 for the tensor-core kernels; mode F for the fp32 CUDA-core kernels):
+      - CUDA-core kernels: max-abs <= 1e-3, every entry;
+      - tensor-core kernels: <= 1e-3 on EVERY row that sees >= 128 keys and on >= 99.9 % of all entries.  The
+        kernel rotates in fp32 and the oracle in fp64, so a rotated operand that lands within ~3e-7 relative of a bf16
+        rounding boundary can round the other way: one bf16 ulp of one of the 256 operand elements of a score.  One
+        flip of k_ji moves score (t, j) by |q'_ti| ulp(k_ji) / sqrt(D); one flip of q'_ti moves every score of row t by
+        ulp(q'_ti) |k_ji| / sqrt(D).  LSE is 1-Lipschitz in the sup norm of the scores, so a row's LSE moves by at most
+        the largest score change: with up to two flips in one score (flip probability per operand element ~1.5e-4)
+            |dLSE(t)| <= 2 max(qmax_t ulp(kmax_t), ulp(qmax_t) kmax_t) / sqrt(D)
+        where qmax_t / kmax_t bound any element of the rotated q'_t / visible k_j (rotation preserves
+        sqrt(x_i^2 + x_{i+D/2}^2)).  In rows with many keys the change of one score is damped by its softmax weight
+        and independent flips average out; the undamped bound is only ever approached by rows with a handful of keys.
+        The test therefore asserts that every entry above 1e-3 belongs to a row with < 128 visible keys AND stays
+        under that row's computed bound (no flat cap).
   * fp32 I/O (config 1): out and LSE within 1e-4 of mode F.
+Set MINIPIC_PARITY_STATS=<file> to append the measured statistics of every comparison as JSON lines.
 """
+import json
+import math
+import os
+
 import numpy as np
 import pytest
 import torch
@@ -23,7 +37,54 @@ from paper_2606_13126_b200.runner import DeviceWorkload, HostStep
 
 pytestmark = pytest.mark.gpu
 
-OUT_MAX, OUT_MEAN, LSE_TOL, LSE_CAP = 2e-2, 2e-3, 1e-3, 8e-3
+OUT_MAX, OUT_MEAN, LSE_TOL = 2e-2, 2e-3, 1e-3
+LONG_ROW = 128          # rows that see at least this many keys must meet LSE_TOL against mode Q, strictly
+LSE_FRAC = 0.999        # ... and so must this fraction of all entries
+
+
+def _pair_norm_max(x):
+    """max_i sqrt(x_i^2 + x_{i+D/2}^2) over the last axis: an upper bound on |element| of R(p) x for any p."""
+    h = x.shape[-1] // 2
+    return np.sqrt(x[..., :h] ** 2 + x[..., h:] ** 2).max(axis=-1)
+
+
+def _ulp_bf16(x):
+    """Spacing of bfloat16 (8 significant bits) at magnitude x > 0."""
+    return 2.0 ** (math.floor(math.log2(x)) - 7)
+
+
+def _request_of(w, t):
+    return int(np.searchsorted(w.cu_q_lens, t, side="right") - 1)
+
+
+def _visible_counts(w, rows):
+    """Number of visible keys of each query row (integer descriptor arithmetic only)."""
+    rows = np.arange(w.num_q_tokens) if rows is None else np.asarray(rows)
+    idx = w.q_seq_idx[rows].astype(np.int64)
+    lo = np.maximum(w.q_vis_lo[rows].astype(np.int64), 0)
+    return rows, np.clip(idx - lo + 1, 0, None)
+
+
+def _flip_bound(w, kc, t, h):
+    """Two-flip bound on |dLSE| of query row t, head h (module docstring), from the inputs alone."""
+    r = _request_of(w, t)
+    g = h // (w.num_q_heads // w.num_kv_heads)
+    scale = 1.0 / math.sqrt(w.head_dim)
+    qmax = float(_pair_norm_max(O.to_f64(w.q[t, h], w.dtype)))
+    lo, idx = max(int(w.q_vis_lo[t]), 0), int(w.q_seq_idx[t])
+    j = np.arange(lo, idx + 1)
+    blk = w.block_tables[r][j // w.block_size]
+    kmax = float(_pair_norm_max(O.to_f64(kc[blk, g, j % w.block_size, :], w.dtype)).max())
+    if qmax == 0.0 or kmax == 0.0:
+        return 0.0
+    return 2.0 * max(qmax * _ulp_bf16(kmax), _ulp_bf16(qmax) * kmax) * scale
+
+
+def _record(stats, w):
+    path = os.environ.get("MINIPIC_PARITY_STATS")
+    if path:
+        with open(path, "a") as f:
+            f.write(json.dumps({"workload": w.name, **stats}) + "\n")
 
 
 def compare(dw, rows=None, heads=None, oracle_cache=None, expect_variant=None, k_prerot=False):
@@ -39,21 +100,39 @@ def compare(dw, rows=None, heads=None, oracle_cache=None, expect_variant=None, k
     assert sel.any()
     do = np.abs(go - of)[sel]
     dl = np.abs(gl - lf)[sel]
-    stats = dict(variant=variant, out_max=float(do.max()), out_mean=float(do.mean()), lse_max_F=float(dl.max()),
-                 lse_mean_F=float(dl.mean()))
+    stats = dict(variant=variant, entries=int(sel.sum()), out_max=float(do.max()), out_mean=float(do.mean()),
+                 lse_max_F=float(dl.max()), lse_mean_F=float(dl.mean()))
     if w.dtype == "f32":
         assert do.max() <= 1e-4 and dl.max() <= 1e-4, stats
+        _record(stats, w)
         return stats
     assert do.max() <= OUT_MAX and do.mean() <= OUT_MEAN, stats
     assert dl.mean() <= LSE_TOL, stats
     if "simt" in variant:
         assert dl.max() <= LSE_TOL, stats
-    else:
-        _, lq = O.run_workload(w, kc, vc, mode="Q", rows=rows, heads=heads, k_prerotated=k_prerot)
-        dq = np.abs(gl - lq)[sel]
-        stats["lse_max_Q"] = float(dq.max())
-        stats["lse_p999_Q"] = float(np.quantile(dq, 0.999))
-        assert stats["lse_p999_Q"] <= LSE_TOL and dq.max() <= LSE_CAP, stats
+        _record(stats, w)
+        return stats
+    _, lq = O.run_workload(w, kc, vc, mode="Q", rows=rows, heads=heads, k_prerotated=k_prerot)
+    dq_full = np.where(sel, np.abs(gl - lq), 0.0)                    # [Tq, Hq]
+    dq = dq_full[sel]
+    row_ids, nvis = _visible_counts(w, None)
+    long_rows = nvis >= LONG_ROW
+    over = np.argwhere(dq_full > LSE_TOL)
+    stats.update(lse_max_Q=float(dq.max()), lse_p999_Q=float(np.quantile(dq, 0.999)), lse_over_tol=int(len(over)),
+                 lse_frac_within_tol=float((dq <= LSE_TOL).mean()),
+                 lse_max_Q_long_rows=float(dq_full[long_rows].max()) if long_rows.any() else 0.0,
+                 long_row_entries=int((sel & long_rows[:, None]).sum()))
+    worst_ratio = 0.0
+    for t, h in over:
+        assert nvis[t] < LONG_ROW, dict(stats, row=int(t), head=int(h), visible=int(nvis[t]), d=float(dq_full[t, h]))
+        bound = _flip_bound(w, kc, int(t), int(h))
+        worst_ratio = max(worst_ratio, float(dq_full[t, h]) / bound if bound > 0 else float("inf"))
+        assert dq_full[t, h] <= bound, dict(stats, row=int(t), head=int(h), visible=int(nvis[t]), d=float(dq_full[t, h]),
+                                            bound=bound)
+    stats["lse_over_tol_worst_fraction_of_flip_bound"] = worst_ratio
+    assert stats["lse_max_Q_long_rows"] <= LSE_TOL, stats
+    assert stats["lse_frac_within_tol"] >= LSE_FRAC, stats
+    _record(stats, w)
     return stats
 
 
@@ -233,10 +312,9 @@ def test_k_prerotated_control_matches():
     dw.step(); torch.cuda.synchronize()
     kc2, vc2 = O.build_cache(w2)
     compare(dw, oracle_cache=(kc2, vc2), k_prerot=True)
-    # and it agrees with the in-kernel-RoPE run on the unrotated cache
+    # the in-kernel-RoPE run on the unrotated cache is held to the same oracle ("algebraically equivalent")
     d0 = DeviceWorkload(w); d0.step(); torch.cuda.synchronize()
-    assert np.abs(d0.out_f64() - dw.out_f64()).max() <= OUT_MAX
-    assert np.abs(d0.lse_f64() - dw.lse_f64()).max() <= 2e-2
+    compare(d0, oracle_cache=(kc, vc))
 
 
 def test_shared_and_duplicate_blocks_on_gpu():
@@ -281,11 +359,18 @@ def test_degenerate_inputs():
     wd = W.shared_pool_decode(name="one", seed=1, hq=8, hkv=2, num_seqs=3, ctx_min=1, ctx_max=1, span_len=64, pool_spans=2)
     dd = DeviceWorkload(wd); dd.step(); torch.cuda.synchronize()
     compare(dd)
-    # empty batch: no launch, OK status
+    # empty batch: OK status (the binding raises on anything else), no kernel launched, outputs untouched
     cfg = dw.cfg
+    before, o0, l0 = mp.minipic_launch_count(), dw.out.clone(), dw.lse.clone()
     mp.minipic_prefill_attention(cfg, dw.q, dw.k_cache, dw.v_cache, dw.block_tables, 1, dw.cu_q_lens, dw.kv_lens,
                                  dw.cu_kv_lens, dw.kv_positions, dw.q_seq_idx, dw.q_vis_lo, 1, 0, 16, dw.out, dw.lse,
                                  dw.workspace, dw.ws_bytes)
+    mp.minipic_decode_attention(dd.cfg, dd.q, dd.k_cache, dd.v_cache, dd.block_tables, int(dd.block_tables.shape[1]),
+                                dd.kv_lens, dd.cu_kv_lens, dd.kv_positions, dd.q_vis_lo, 0, 1, dd.out, dd.lse,
+                                dd.workspace, dd.ws_bytes)
+    torch.cuda.synchronize()
+    assert mp.minipic_launch_count() == before
+    assert torch.equal(o0, dw.out) and torch.equal(l0, dw.lse)
 
 
 def test_host_step_entry_points_match_device_path():
@@ -308,38 +393,85 @@ def _sampled(w, n_rows, n_heads, seed=0):
     return rows, heads
 
 
+def _stratified_rows(w, n_random, seed=0, per_request_suffix=48, span_starts_per_request=24):
+    """Query rows stratified over what the persistent scheduler does with them: every request; suffix rows (the long
+    items the LPT order starts with) incl. the first and last of each request; the first rows of spans (few visible keys:
+    the last, shortest items) and rows around 32-token super-tile and 128-key tile boundaries; plus a uniform sample."""
+    rng = np.random.default_rng(seed)
+    picks = [rng.choice(w.num_q_tokens, size=min(n_random, w.num_q_tokens), replace=False), [0, w.num_q_tokens - 1]]
+    for r in range(w.num_reqs):
+        t0, t1 = int(w.cu_q_lens[r]), int(w.cu_q_lens[r + 1])
+        if t1 <= t0:
+            continue
+        lo = w.q_vis_lo[t0:t1]
+        idx = w.q_seq_idx[t0:t1]
+        suffix = np.flatnonzero(lo == 0) + t0
+        if suffix.size:
+            picks.append(suffix[:4]); picks.append(suffix[-4:])
+            picks.append(rng.choice(suffix, size=min(per_request_suffix, suffix.size), replace=False))
+        starts = np.flatnonzero((idx == lo) & (lo > 0)) + t0                     # first token of a span-local stretch
+        if starts.size:
+            for s0 in rng.choice(starts, size=min(span_starts_per_request, starts.size), replace=False):
+                picks.append(np.arange(s0, min(s0 + 3, t1)))                     # 1, 2, 3 visible keys
+                for off in (31, 32, 33, 127, 128, 129):                          # super-tile / KV-tile boundaries
+                    if s0 + off < t1 and w.q_vis_lo[s0 + off] == w.q_vis_lo[s0]:
+                        picks.append([s0 + off])
+                last = s0 + int(np.searchsorted(w.q_vis_lo[s0:t1] != w.q_vis_lo[s0], True))  # end of this span's rows
+                picks.append([last - 1])
+    return np.unique(np.concatenate([np.asarray(p, np.int64).ravel() for p in picks]))
+
+
 def test_config2_full():
     w = W.config2()
-    dw = DeviceWorkload(w, rope_table_positions=2112)
+    dw = DeviceWorkload(w)
     dw.step(); torch.cuda.synchronize()
-    compare(dw, heads=np.array([0, 5, 17, 31]))
+    compare(dw, heads=np.array([0, 5, 10, 15, 17, 22, 27, 31]))        # every row x one head per KV head
     gk, gv = dw.cache_bits(); kc, vc = O.build_cache(w)
     assert gk.tobytes() == kc.tobytes() and gv.tobytes() == vc.tobytes()
 
 
 def test_config3_full_sampled():
     w = W.config3()
-    dw = DeviceWorkload(w, rope_table_positions=w.max_kv_len)
+    dw = DeviceWorkload(w)
     dw.step(); torch.cuda.synchronize()
-    rows, heads = _sampled(w, 160, 3)
-    compare(dw, rows=rows, heads=heads)
+    rows = _stratified_rows(w, 1500, seed=1, per_request_suffix=16, span_starts_per_request=1)
+    assert rows.size >= 2000
+    compare(dw, rows=rows, heads=np.array([1, 6, 11, 12, 19, 20, 25, 30]))
     gk, gv = dw.cache_bits(); kc, vc = O.build_cache(w)
     assert gk.tobytes() == kc.tobytes() and gv.tobytes() == vc.tobytes()
 
 
 def test_config4_full_sampled():
     w = W.config4()
-    dw = DeviceWorkload(w, rope_table_positions=8192)
+    dw = DeviceWorkload(w)
     dw.step(); torch.cuda.synchronize()
-    compare(dw, rows=np.array([0, 1, 17, 100, 255]), heads=np.array([0, 9, 31]))
+    rng = np.random.default_rng(7)
+    seqs = np.unique(np.concatenate([[0, 1, 255, int(np.argmax(w.kv_lens)), int(np.argmin(w.kv_lens))],
+                                     rng.choice(256, size=32, replace=False)]))
+    assert seqs.size >= 32
+    compare(dw, rows=seqs, heads=np.array([0, 5, 10, 15, 17, 22, 27, 31]), expect_variant="decode_mma")
 
 
 def test_config5_full_sampled():
     w = W.config5()
-    dw = DeviceWorkload(w, rope_table_positions=w.max_kv_len)
+    dw = DeviceWorkload(w)
     dw.step(); torch.cuda.synchronize()
-    rows, heads = _sampled(w, 96, 2)
-    # add suffix rows of every request (they see ~33K keys) and first rows of a span
-    extra = [int(w.cu_q_lens[r + 1]) - 1 for r in range(w.num_reqs)] + [int(w.cu_q_lens[r]) for r in range(w.num_reqs)]
-    rows = np.unique(np.concatenate([rows, extra]))
-    compare(dw, rows=rows, heads=heads)
+    rows = _stratified_rows(w, 1200, seed=2)
+    assert rows.size >= 2000
+    compare(dw, rows=rows, heads=np.array([3, 12, 17, 30, 36, 41, 55, 58]), expect_variant="prefill_sm100_tcgen05")
+    gk, gv = dw.cache_bits(); kc, vc = O.build_cache(w)
+    assert gk.tobytes() == kc.tobytes() and gv.tobytes() == vc.tobytes()
+
+
+def test_midsize_many_items_per_cta_full_compare():
+    """Everything that only happens when a CTA of the persistent prefill kernel runs MANY work items - ring-slot parity wrap
+    (more than 4 items per CTA), the deferred epilogue across items, the longest-first tail - compared in full (every row,
+    every head): 2 requests x (40 new + 40 cached 256-token spans + 128 suffix) = 20 736 query tokens, G = 8, 2 KV heads
+    -> 1 296 work items over 148 CTAs (~8.8 per CTA)."""
+    w = W.long_context_prefill(name="m5_mid", seed=77, hq=16, hkv=2, num_reqs=2, slots_per_req=80, span_len=256,
+                               suffix_len=128, pool_spans=48, cached_per_req=40)
+    assert w.num_q_tokens == 20736
+    dw = DeviceWorkload(w)
+    dw.step(); torch.cuda.synchronize()
+    st = compare(dw, expect_variant="prefill_sm100_tcgen05")
+    assert st["entries"] == w.num_q_tokens * w.num_q_heads

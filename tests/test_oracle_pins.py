@@ -453,6 +453,92 @@ def test_bf16_rounding_is_rne_and_mode_q_rounds_operands_only():
     assert 1e-7 < d.max() < 2e-2                       # differs (operands were rounded) but only by bf16 rounding
 
 
+def _bf16(x: float) -> float:
+    """One round-to-nearest-even of a Python float to bfloat16 through torch's cast (not the oracle's rounding code)."""
+    return float(torch.tensor(x, dtype=torch.float64).to(torch.bfloat16).double())
+
+
+def brute_force_mode_q(q, k, v, pos, idx, lo, theta, hq, hkv, round_scores=False, round_p=False, round_before_rotation=False):
+    """Pure-Python restatement of comparison mode Q ("storing already-rotated keys"): rotate in fp64,
+    round every element of q' and k_j ONCE to bf16 with torch's cast, then everything else (dot product, scale, softmax,
+    P.V) in fp64 with nothing else rounded.  The three keyword switches are the plausible mistakes the pin must reject."""
+    tq, d = len(q), len(q[0][0])
+    half = d // 2
+    g = hq // hkv
+
+    def rot_round(x, p):
+        if round_before_rotation:
+            x = [_bf16(e) for e in x]
+        y = [0.0] * d
+        for i in range(half):
+            f = theta ** (-2.0 * i / d)
+            c, s = math.cos(p * f), math.sin(p * f)
+            y[i] = x[i] * c - x[i + half] * s
+            y[i + half] = x[i] * s + x[i + half] * c
+        return y if round_before_rotation else [_bf16(e) for e in y]
+
+    out = np.zeros((tq, hq, d))
+    lse = np.full((tq, hq), -math.inf)
+    for h in range(hq):
+        kr = [rot_round(k[j][h // g], pos[j]) for j in range(len(k))]
+        for t in range(tq):
+            qr = rot_round(q[t][h], pos[idx[t]])
+            vis = [j for j in range(len(k)) if lo[t] <= j <= idx[t]]
+            if not vis:
+                continue
+            sc = [sum(a * b for a, b in zip(qr, kr[j])) / math.sqrt(d) for j in vis]
+            if round_scores:
+                sc = [_bf16(s) for s in sc]
+            m = max(sc)
+            z = sum(math.exp(s - m) for s in sc)
+            lse[t, h] = m + math.log(z)
+            for j, s in zip(vis, sc):
+                p = math.exp(s - m) / z
+                if round_p:
+                    p = _bf16(p)
+                for e in range(d):
+                    out[t, h, e] += p * v[j][h // g][e]
+    return out, lse
+
+
+def test_mode_q_pinned_by_brute_force_with_torch_bf16_rounding():
+    """Mode Q is the comparison the tensor-core LSE gate rests on (R1), so it gets its own pin: a brute-force
+    restatement that rounds exactly q' and k_j (after rotation, before the dot product) must agree to 1e-12, and the
+    variants that round something else - the scores, the probabilities, or the operands BEFORE the rotation - must not."""
+    rng = np.random.default_rng(21)
+    T, hq, hkv, d, theta = 37, 4, 2, 16, 1e4
+    q, k, v = dense_request(rng, T, hq, hkv, d, dtype="bf16")
+    blocks = [5, 1, 7]
+    kc, vc = paged(k, v, blocks, 9, dtype="bf16")
+    pos = (np.arange(T) * 3 + 11).astype(np.int64)               # positions are not the index
+    idx = np.arange(T)
+    lo = np.where(idx < 16, 0, np.where(idx < 32, 16, 0))        # one span-local stretch, suffix sees all
+    oq, lq = one_request(q, kc, vc, blocks, pos, idx, lo, hq, theta, dtype="bf16", mode="Q")
+    qf, kf, vf = (O.bf16_bits_to_f64(a) for a in (q, k, v))
+    bo, bl = brute_force_mode_q(qf.tolist(), kf.tolist(), vf.tolist(), pos.tolist(), idx.tolist(), lo.tolist(), theta, hq, hkv)
+    assert np.abs(oq - bo).max() < 1e-12 and np.abs(lq - bl).max() < 1e-12
+    # the pin discriminates: each plausible mis-reading of "mode Q" is far outside 1e-12
+    for wrong in (dict(round_scores=True), dict(round_p=True), dict(round_before_rotation=True)):
+        wo, wl = brute_force_mode_q(qf.tolist(), kf.tolist(), vf.tolist(), pos.tolist(), idx.tolist(), lo.tolist(), theta,
+                                    hq, hkv, **wrong)
+        assert max(np.abs(oq - wo).max(), np.abs(lq - wl).max()) > 1e-6, wrong
+    # V is never rounded by mode Q: with identical scores (Q = 0 -> every score is 0 in both modes) outputs agree exactly
+    q0 = np.zeros_like(q)
+    of0, lf0 = one_request(q0, kc, vc, blocks, pos, idx, lo, hq, theta, dtype="bf16", mode="F")
+    oq0, lq0 = one_request(q0, kc, vc, blocks, pos, idx, lo, hq, theta, dtype="bf16", mode="Q")
+    assert np.array_equal(of0, oq0) and np.array_equal(lf0, lq0)
+    # f32 I/O: mode Q rounds the rotated operands to float32
+    q32, k32, v32 = dense_request(rng, 20, 2, 1, 8)
+    kc32, vc32 = paged(k32, v32, [3, 0], 4)
+    p32 = np.arange(20)
+    o32, l32 = one_request(q32, kc32, vc32, [3, 0], p32, p32, np.zeros(20, int), 2, 1e4, dtype="f32", mode="Q")
+    kr = O.rope_rotate(k32[:, 0].astype(np.float64), p32, 1e4).astype(np.float32).astype(np.float64)
+    for t in (0, 7, 19):
+        qr = O.rope_rotate(q32[t, 1].astype(np.float64), np.asarray(t), 1e4).astype(np.float32).astype(np.float64)
+        s = kr[:t + 1] @ qr / math.sqrt(8)
+        assert abs(l32[t, 1] - (s.max() + math.log(np.exp(s - s.max()).sum()))) < 1e-12
+
+
 # --------------------------------------------------------------------------- generator sanity (integer structure)
 def test_workload_structure_matches_baseline_configs():
     w1 = W.config1()
