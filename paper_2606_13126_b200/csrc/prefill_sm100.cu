@@ -31,9 +31,15 @@ namespace minipic {
 namespace {
 
 constexpr int BM = 128, BN = 128, D = 128;
-constexpr int kTileBytes = BN * D * 2;       // 32 KB: one K / V / Q tile
+constexpr int kTileBytes = BM * D * 2;       // 32 KB: one Q tile (128 rows)
 constexpr int kHalfBytes = kTileBytes / 2;   // [half of head_dim][128 rows][128 B]
-constexpr int kKStages = 2, kVStages = 2, kRing = 4;
+// CTA PAIR (cta_group::2): one tcgen05.mma covers M = 256 rows = the same tile (A or B) of BOTH CTAs of the cluster.  The B
+// operand is split between the two CTAs: for QK^T by keys (each CTA gathers + rotates 64 of the tile's 128 keys), for PV
+// by head_dim (each CTA holds its 64-column half of V for all 128 keys).  Per CTA a K stage and a V stage are 16 KB.
+constexpr int kKeysCta = BN / 2;
+constexpr int kKTileBytes = kKeysCta * D * 2;    // 8 row groups of [half (2)][8 rows x 128 B]
+constexpr int kVTileBytes = BN * (D / 2) * 2;    // 16 row groups of [8 rows x 128 B] (this CTA's half of head_dim)
+constexpr int kKStages = 3, kVStages = 3, kRing = 4;
 // Measured and dropped (config 5, in-kernel RoPE; the kept version runs 2.24 ms):
 //  * a ring of three Q tile slots (next item's tile A loaded + rotated during the current item, epilogue staged in the
 //    finishing item's tile-B slot): parity-green, dense +3 %, but span items -7 % (2.30 ms): the four rotation warps are
@@ -58,7 +64,7 @@ constexpr int kKStages = 2, kVStages = 2, kRing = 4;
 //    step, so the softmax warps still wait (49 % of their samples) and A / B no longer alternate on the MUFU unit.
 // K / V tile in shared memory: 16 row groups of [half of head_dim (2)][8 rows x 128 B] = 2048 B each, so one (block, head)
 // of the cache (16 tokens x 256 B) is ONE 4-D TMA box of two groups.  Q tile: [half (2)][128 rows x 128 B].
-constexpr int kGroupBytes = 2048, kKvHalfOff = 1024;
+constexpr int kGroupBytes = 2048, kKvHalfOff = 1024, kVGroupBytes = 1024;
 constexpr int kStageBytes = 4096;            // epilogue staging per softmax warp: 32 rows x 128 B (64 bf16 columns)
 // 16 warps = 4 warpgroups: softmax A, softmax B (184 registers each after setmaxnreg), rotation (96), control (TMA, MMA and
 // two idle warps, 48).  setmaxnreg is a WARPGROUP-wide instruction (all four warps, same count), and the split must fit the
@@ -86,6 +92,43 @@ __device__ __forceinline__ void mbar_arrive(uint32_t bar) {
 }
 __device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
   asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+// ---- cluster (CTA pair) helpers
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ uint32_t mapa(uint32_t addr, uint32_t rank) {   // shared::cta address -> shared::cluster address in CTA rank
+  uint32_t r;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(addr), "r"(rank));
+  return r;
+}
+// arrive on a barrier of any CTA of the pair.  Default semantics (release at CTA scope), as in CUTLASS' 2-SM pipelines: what
+// the waiting MMA issuer hands on is consumed by the tensor core of the ARRIVING thread's own SM (its shared memory through
+// the async proxy after fence.proxy.async, its TMEM after tcgen05.fence).  A cluster-scope release costs a MEMBAR.ALL.GPU
+// per arrival (measured: config 5 2.19 -> 2.61 ms).
+__device__ __forceinline__ void mbar_arrive_cl(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+// the scheduler's arrive publishes ring entries written into the peer's shared memory: release at cluster scope
+__device__ __forceinline__ void mbar_arrive_cl_release(uint32_t cluster_addr) {
+  asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(cluster_addr) : "memory");
+}
+__device__ __forceinline__ void st_cluster_v4(uint32_t cluster_addr, int a, int b, int c, int d) {
+  asm volatile("st.shared::cluster.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(cluster_addr), "r"(a), "r"(b), "r"(c), "r"(d) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ bool mbar_try_cl(uint32_t bar, uint32_t parity) {   // acquire at cluster scope: remote arrivals
+  uint32_t done;
+  asm volatile(
+      "{\n\t.reg .pred p;\n\t"
+      "mbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 p, [%1], %2;\n\t"
+      "selp.u32 %0, 1, 0, p;\n\t}"
+      : "=r"(done) : "r"(bar), "r"(parity) : "memory");
+  return done != 0;
 }
 __device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity) {
   uint32_t done;
@@ -115,6 +158,18 @@ struct Waiter {
       }
     }
   }
+  // same, for barriers that threads of the PEER CTA arrive on (acquire at cluster scope)
+  __device__ __forceinline__ void wait_cl(uint32_t bar, uint32_t parity) {
+    if (dead) return;
+    unsigned spins = 0;
+    while (!mbar_try_cl(bar, parity)) {
+      if ((++spins & 4095u) == 0 && (*(volatile int*)err != 0 || spins > kWaitMaxSpins)) {
+        atomicCAS(err, 0, (int)(bar | 0x20000000u));
+        dead = true;
+        return;
+      }
+    }
+  }
 };
 // Debug-only event trace (-DMINIPIC_TRACE, never in the shipped library): CTA 0 records (tag, SM clock) per role.
 #ifdef MINIPIC_TRACE
@@ -136,7 +191,9 @@ __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
 __device__ __forceinline__ void tc_commit(uint32_t bar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+  // arrives on the barrier at this offset in BOTH CTAs of the pair once every MMA issued so far has completed
+  asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               ::"r"(bar), "h"((unsigned short)3) : "memory");
 }
 __device__ __forceinline__ void tma_load_3d(uint32_t dst, const CUtensorMap* tmap, uint32_t bar, int x, int y, int z) {
   asm volatile(
@@ -159,13 +216,14 @@ __device__ __forceinline__ void tma_store_wait_all() { asm volatile("cp.async.bu
 // offset (>> 4, bits 16-29); the high word is the same for every operand of this kernel: stride byte offset 1024
 // (8 rows x 128 B), descriptor version 1 (bit 46), swizzle mode 128B (2 << 61).
 constexpr uint32_t kDescHiQ = (1024u >> 4) | (1u << 14) | (2u << 29);                    // Q tile: 8-row groups 1024 B apart
-constexpr uint32_t kDescHiKV = ((uint32_t)kGroupBytes >> 4) | (1u << 14) | (2u << 29);   // K / V tile: 2048 B apart
+constexpr uint32_t kDescHiKV = ((uint32_t)kGroupBytes >> 4) | (1u << 14) | (2u << 29);   // K tile: 8-row groups 2048 B apart
+constexpr uint32_t kDescHiV = ((uint32_t)kVGroupBytes >> 4) | (1u << 14) | (2u << 29);   // V half tile: 8-key groups 1024 B apart
 // D[tmem] (+)= A[smem] * B[smem]
 __device__ __forceinline__ void umma_ss(uint32_t d_tmem, uint32_t a_lo, uint32_t b_lo, uint32_t idesc, uint32_t acc) {
   asm volatile(
       "{\n\t.reg .pred p;\n\t.reg .b64 da, db;\n\tsetp.ne.b32 p, %4, 0;\n\t"
       "mov.b64 da, {%1, %5};\n\tmov.b64 db, {%2, %6};\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], da, db, %3, p;\n\t}"
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], da, db, %3, p;\n\t}"
       ::"r"(d_tmem), "r"(a_lo), "r"(b_lo), "r"(idesc), "r"(acc), "r"(kDescHiQ), "r"(kDescHiKV) : "memory");
 }
 // D[tmem] (+)= A[tmem] * B[smem]
@@ -173,8 +231,8 @@ __device__ __forceinline__ void umma_ts(uint32_t d_tmem, uint32_t a_tmem, uint32
   asm volatile(
       "{\n\t.reg .pred p;\n\t.reg .b64 db;\n\tsetp.ne.b32 p, %4, 0;\n\t"
       "mov.b64 db, {%2, %5};\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], db, %3, p;\n\t}"
-      ::"r"(d_tmem), "r"(a_tmem), "r"(b_lo), "r"(idesc), "r"(acc), "r"(kDescHiKV) : "memory");
+      "tcgen05.mma.cta_group::2.kind::f16 [%0], [%1], db, %3, p;\n\t}"
+      ::"r"(d_tmem), "r"(a_tmem), "r"(b_lo), "r"(idesc), "r"(acc), "r"(kDescHiV) : "memory");
 }
 __device__ __forceinline__ void tmem_ld32(uint32_t taddr, float* v) {
   uint32_t* r = reinterpret_cast<uint32_t*>(v);
@@ -233,9 +291,10 @@ __device__ __forceinline__ bool elect_one() {   // one lane of a converged warp 
 template <int N> __device__ __forceinline__ void reg_inc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(N)); }
 template <int N> __device__ __forceinline__ void reg_dec() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(N)); }
 
-// instruction descriptor: D fp32, A/B bf16, M=128, N=128; b_mn = B operand is MN-major (V tile)
+// instruction descriptor: D fp32, A/B bf16, M = 256 (128 rows in each CTA of the pair), N = 128; b_mn = B operand is
+// MN-major (V tile)
 __host__ __device__ constexpr uint32_t instr_desc(bool b_mn) {
-  return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn ? 1u : 0u) << 16) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((b_mn ? 1u : 0u) << 16) | ((uint32_t)(BN >> 3) << 17) | ((uint32_t)(2 * BM >> 4) << 24);
 }
 
 // ------------------------------------------------------------------------------------------------ a2: plan
@@ -311,25 +370,41 @@ __global__ void __launch_bounds__(256) plan_scatter_kernel(PlanHeader* hdr, cons
 // ------------------------------------------------------------------------------------------------ main kernel
 struct Smem {
   alignas(1024) unsigned char q[2][kTileBytes];
-  alignas(1024) unsigned char k[kKStages][kTileBytes];
-  alignas(1024) unsigned char v[kVStages][kTileBytes];
+  alignas(1024) unsigned char k[kKStages][kKTileBytes];
+  alignas(1024) unsigned char v[kVStages][kVTileBytes];
   alignas(1024) unsigned char ostage[8][kStageBytes];
-  unsigned long long bars[40];
-  ItemInfo ring[kRing];
+  unsigned long long bars[48];
+  alignas(16) ItemInfo ring[kRing];
   alignas(16) unsigned long long finc[64];   // F_i (common.cuh), read by the rotation lanes at every exact restart
   alignas(16) float2 step1[64];              // (cos f_i, sin f_i): one-position step, used by the Q rotation
   alignas(16) float2 step4[64];              // (cos 4 f_i, sin 4 f_i): four-position step, used by the K rotation
   uint32_t tmem_base;
 };
+// Barriers live at the same offset in both CTAs.  "local" ones are completed and waited on inside one CTA; "leader" ones
+// are waited on only by the MMA issuer / scheduler of CTA rank 0 and collect arrivals from BOTH CTAs (mbar_arrive_cl);
+// "multicast" ones are completed in both CTAs at once by a tcgen05.commit of the leader's MMA issuer.
 enum Bar {
-  SCHED_FULL = 0, SCHED_EMPTY = SCHED_FULL + kRing,
-  Q_FULL = SCHED_EMPTY + kRing, Q_READY, Q_EMPTY = Q_READY + 2,
-  K_FULL, K_READY = K_FULL + kKStages, K_EMPTY = K_READY + kKStages,
-  V_FULL = K_EMPTY + kKStages, V_EMPTY = V_FULL + kVStages, V_FIX = V_EMPTY + kVStages,
-  S_FULL, P_FULL = S_FULL + 2, O_FULL = P_FULL + 2, O_FREE = O_FULL + 2, NUM_BARS = O_FREE + 2
+  SCHED_FULL = 0,                       // [kRing] local, 1 arrival by the leader's scheduler (remote for rank 1)
+  SCHED_EMPTY = SCHED_FULL + kRing,     // [kRing] leader, 15 consumer warps per CTA
+  Q_FULL = SCHED_EMPTY + kRing,         // local (TMA)
+  Q_READY,                              // [2] leader, 4 softmax warps per CTA
+  Q_EMPTY = Q_READY + 2,                // multicast
+  K_FULL,                               // [kKStages] local (TMA)
+  K_READY = K_FULL + kKStages,          // [kKStages] leader, 4 rotation warps per CTA
+  K_EMPTY = K_READY + kKStages,         // [kKStages] multicast
+  V_FULL = K_EMPTY + kKStages,          // [kVStages] local (TMA)
+  V_PEER = V_FULL + kVStages,           // [kVStages] leader, 1 arrival by rank 1's forwarder warp: its half of V has landed
+  V_EMPTY = V_PEER + kVStages,          // [kVStages] multicast
+  V_FIX = V_EMPTY + kVStages,           // local, 128 rotation threads
+  S_FULL,                               // [2] multicast
+  P_FULL = S_FULL + 2,                  // [2] leader, 4 softmax warps per CTA
+  O_FULL = P_FULL + 2,                  // [2] multicast
+  O_FREE = O_FULL + 2,                  // [2] leader, 4 softmax warps per CTA
+  NUM_BARS = O_FREE + 2
 };
-static_assert(NUM_BARS <= 40, "barrier array too small");
+static_assert(NUM_BARS <= 48, "barrier array too small");
 static_assert(sizeof(Smem) <= 232448, "shared memory budget");
+static_assert(sizeof(ItemInfo) == 48, "ring entries are copied to the peer CTA as three 16-byte stores");
 
 struct Params {
   PrefillArgs a;
@@ -344,24 +419,28 @@ struct Params {
   float2 step4[64];                  // (cos 4 f_i, sin 4 f_i): the four-position RoPE step of the rotation lanes
 };
 
+// A work item as one CTA of the pair sees it.  The item covers up to 4 * TOK query tokens (TOK = 128 / G tokens fill one
+// 128-row MMA tile): CTA rank c owns tokens [2 c TOK, 2 c TOK + 2 TOK) of it, tile A the first TOK of those, tile B the rest.
+// Both CTAs run the SAME number of KV tiles for a tile slot (the MMA covers both); rows a CTA does not own are masked.
 struct Item {
   int t0, ntok, r, idx0, lo, kvh, n_kv, kv_hi, kv_len, kv_off;
-  int kv_lo, ntok_a, ntok_b, n_a, n_b;
+  int kv_lo, tb, ntok_a, ntok_b, n_b;
   __device__ __forceinline__ int ntok_x(int x) const { return x ? ntok_b : ntok_a; }
-  __device__ __forceinline__ int n_x(int x) const { return x ? n_b : n_a; }
+  __device__ __forceinline__ int n_x(int x) const { return x ? n_b : n_kv; }   // tile B is skipped by the whole pair if empty
 };
 template <int TOK>
-__device__ __forceinline__ Item load_item(const ItemInfo& ii) {
+__device__ __forceinline__ Item load_item(const ItemInfo& ii, int rank) {
   Item it;
   it.t0 = ii.t0; it.ntok = ii.ntok; it.r = ii.r; it.idx0 = ii.idx0; it.lo = ii.lo; it.kvh = ii.kvh; it.n_kv = ii.n_kv;
   it.kv_hi = ii.kv_hi; it.kv_len = ii.kv_len; it.kv_off = ii.kv_off;
   it.kv_lo = it.lo & ~(kBlock - 1);
-  it.ntok_a = min(it.ntok, TOK); it.ntok_b = it.ntok - it.ntok_a;
-  const int hi_a = min(it.idx0 + it.ntok_a, it.kv_len);
-  it.n_a = hi_a > it.kv_lo ? (hi_a - it.kv_lo + BN - 1) / BN : 0;
-  it.n_b = it.ntok_b > 0 ? it.n_kv : 0;
+  it.tb = rank * 2 * TOK;
+  const int mine = min(max(it.ntok - it.tb, 0), 2 * TOK);
+  it.ntok_a = min(mine, TOK); it.ntok_b = mine - it.ntok_a;
+  it.n_b = it.ntok > TOK ? it.n_kv : 0;
   return it;
 }
+
 
 // RoPE state of one rotation lane.  A warp covers 4 tile rows per step: lane = (row-in-step = lane >> 3, 16-byte
 // chunk = lane & 7); the lane owns dims [8*chunk, 8*chunk + 8) of both halves of its row, i.e. 8 RoPE pairs (i, i + 64)
@@ -412,7 +491,7 @@ struct Rot8 {
 };
 
 template <int G>
-__global__ void __launch_bounds__(kThreads, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
                      const __grid_constant__ CUtensorMap tmap_v, const __grid_constant__ CUtensorMap tmap_o,
                      const __grid_constant__ Params prm) {
@@ -420,9 +499,12 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
   Smem& sm = *reinterpret_cast<Smem*>(smem_raw);
   constexpr int TOK = BM / G;
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int rank = (int)cluster_ctarank();   // 0 = leader: owns the scheduler, the MMA issuer and every "leader" barrier
   const PrefillArgs& a = prm.a;
   const uint32_t bar0 = smem_u32(sm.bars);
+  const uint32_t lbar0 = mapa(bar0, 0);      // the leader's barrier array in the cluster window (== own array for rank 0)
   auto bar = [&](int b) { return bar0 + 8u * (uint32_t)b; };
+  auto lbar = [&](int b) { return lbar0 + 8u * (uint32_t)b; };
   Waiter w{&prm.hdr->err, false};
 
   if (threadIdx.x >= 64 && threadIdx.x < 128) {
@@ -432,78 +514,112 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
   }
   if (threadIdx.x == 0) {
     if (smem_u32(smem_raw) & 1023u) atomicCAS(&prm.hdr->err, 0, 2);   // swizzled tiles need a 1024-byte aligned base
-    for (int s = 0; s < kRing; ++s) { mbar_init(bar(SCHED_FULL + s), 1); mbar_init(bar(SCHED_EMPTY + s), 14); }
-    mbar_init(bar(Q_FULL), 1); mbar_init(bar(Q_READY), 128); mbar_init(bar(Q_READY + 1), 128); mbar_init(bar(Q_EMPTY), 1);
-    for (int s = 0; s < kKStages; ++s) { mbar_init(bar(K_FULL + s), 1); mbar_init(bar(K_READY + s), 128); mbar_init(bar(K_EMPTY + s), 1); }
-    for (int s = 0; s < kVStages; ++s) { mbar_init(bar(V_FULL + s), 1); mbar_init(bar(V_EMPTY + s), 1); }
+    for (int s = 0; s < kRing; ++s) { mbar_init(bar(SCHED_FULL + s), 1); mbar_init(bar(SCHED_EMPTY + s), 30); }
+    mbar_init(bar(Q_FULL), 1); mbar_init(bar(Q_READY), 8); mbar_init(bar(Q_READY + 1), 8); mbar_init(bar(Q_EMPTY), 1);
+    for (int s = 0; s < kKStages; ++s) { mbar_init(bar(K_FULL + s), 1); mbar_init(bar(K_READY + s), 8); mbar_init(bar(K_EMPTY + s), 1); }
+    for (int s = 0; s < kVStages; ++s) { mbar_init(bar(V_FULL + s), 1); mbar_init(bar(V_PEER + s), 1); mbar_init(bar(V_EMPTY + s), 1); }
     mbar_init(bar(V_FIX), 128);
     for (int x = 0; x < 2; ++x) {
-      mbar_init(bar(S_FULL + x), 1); mbar_init(bar(P_FULL + x), 128); mbar_init(bar(O_FULL + x), 1); mbar_init(bar(O_FREE + x), 128);
+      mbar_init(bar(S_FULL + x), 1); mbar_init(bar(P_FULL + x), 8); mbar_init(bar(O_FULL + x), 1); mbar_init(bar(O_FREE + x), 8);
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  if (warp == 13) {  // TMEM: 512 columns = S_A | S_B | O_A | O_B, 128 each; P_X aliases the first 64 columns of S_X
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&sm.tmem_base)), "r"(512));
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::);
+  if (warp == 13) {  // TMEM: 512 columns = S_A | S_B | O_A | O_B, 128 each; P_X aliases the first 64 columns of S_X.
+                     // cta_group::2: the same warp of both CTAs allocates; both get all 512 columns (base 0)
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(&sm.tmem_base)), "r"(512));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::);
   }
   tc_fence_before();
-  __syncthreads();
+  cluster_sync_all();   // barriers of BOTH CTAs are initialised before anyone arrives remotely
   tc_fence_after();
   const uint32_t tmem = sm.tmem_base;
   const int n_items = prm.hdr->n_tiles * prm.hkv;
 
   if (warp >= 12) {
     reg_dec<kRegsCtl>();
-    if (warp == 12) {
-      // ============================================================ scheduler + Q / K TMA producer (a4)
+    if (warp == 15 && rank == 0) {
+      // ============================================================ scheduler (leader only): item ring of both CTAs
+      const uint32_t ring_l = smem_u32(sm.ring), ring_p = mapa(ring_l, 1), full_p = mapa(bar(SCHED_FULL), 1);
+      if (lane == 0) {
+        for (uint32_t it_n = 0;; ++it_n) {
+          const int slot = it_n & (kRing - 1);
+          w.wait(bar(SCHED_EMPTY + slot), ((it_n / kRing) & 1) ^ 1);
+          const int item = w.dead ? n_items : atomicAdd(&prm.hdr->next_item, 1);
+          ItemInfo ii;
+          if (item >= n_items) {
+            ii.t0 = -1; ii.ntok = 0; ii.r = 0; ii.idx0 = 0; ii.lo = 0; ii.kvh = 0; ii.n_kv = 0; ii.kv_hi = 0; ii.kv_len = 0; ii.kv_off = 0;
+          } else {
+            const TileDesc td = prm.tiles[item / prm.hkv];
+            ii.t0 = td.t0; ii.ntok = td.ntok; ii.r = td.r; ii.idx0 = td.idx0; ii.lo = td.lo; ii.kvh = item % prm.hkv; ii.n_kv = td.n_kv;
+            ii.kv_hi = td.kv_hi; ii.kv_len = td.kv_len; ii.kv_off = td.kv_off;
+          }
+          ii.pad[0] = ii.pad[1] = 0;
+          sm.ring[slot] = ii;
+          const uint32_t dst = ring_p + (uint32_t)slot * (uint32_t)sizeof(ItemInfo);
+          st_cluster_v4(dst, ii.t0, ii.ntok, ii.r, ii.idx0);
+          st_cluster_v4(dst + 16, ii.lo, ii.kvh, ii.n_kv, ii.kv_hi);
+          st_cluster_v4(dst + 32, ii.kv_len, ii.kv_off, 0, 0);
+          mbar_arrive_cl_release(lbar(SCHED_FULL + slot));
+          mbar_arrive_cl_release(full_p + 8u * (uint32_t)slot);
+          TRACE(0, 1);
+          if (item >= n_items) break;
+        }
+      }
+    } else if (warp == 15) {
+      // ============================================================ V forwarder (rank 1): tells the leader's MMA issuer that
+      // this CTA's half of a V tile has landed (and, for a partial last block, that its tail rows are zeroed)
+      uint32_t vc = 0, fixc = 0;
+      for (uint32_t it_n = 0;; ++it_n) {
+        const int slot = it_n & (kRing - 1);
+        w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
+        if (__any_sync(0xffffffffu, w.dead) || sm.ring[slot].t0 < 0) break;
+        const int n = sm.ring[slot].n_kv, kv_hi = sm.ring[slot].kv_hi;
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
+        const bool vfix = (kv_hi & (kBlock - 1)) != 0;
+        for (int i = 0; i < n; ++i, ++vc) {
+          const int st = vc % kVStages;
+          w.wait(bar(V_FULL + st), (vc / kVStages) & 1);
+          if (i == n - 1 && vfix) { w.wait(bar(V_FIX), fixc & 1); ++fixc; }
+          __syncwarp();
+          if (lane == 0) mbar_arrive_cl(lbar(V_PEER + st));
+        }
+      }
+    } else if (warp == 12) {
+      // ============================================================ Q / K TMA producer (a4): this CTA's 64 keys of every K tile
       uint32_t kc = 0, qc = 0;
       for (uint32_t it_n = 0;; ++it_n) {
         const int slot = it_n & (kRing - 1);
-        int item = 0;
-        if (lane == 0) {
-          w.wait(bar(SCHED_EMPTY + slot), ((it_n / kRing) & 1) ^ 1);
-          item = w.dead ? n_items : atomicAdd(&prm.hdr->next_item, 1);
-        }
-        item = __shfl_sync(0xffffffffu, item, 0);
-        if (item >= n_items) {
-          if (lane == 0) { sm.ring[slot].t0 = -1; mbar_arrive(bar(SCHED_FULL + slot)); }
-          break;
-        }
-        const TileDesc td = prm.tiles[item / prm.hkv];
-        const int kvh = item % prm.hkv;
-        TRACE_L0(0, 1);
-        if (lane == 0) {
-          ItemInfo& ii = sm.ring[slot];
-          ii.t0 = td.t0; ii.ntok = td.ntok; ii.r = td.r; ii.idx0 = td.idx0; ii.lo = td.lo; ii.kvh = kvh; ii.n_kv = td.n_kv;
-          ii.kv_hi = td.kv_hi; ii.kv_len = td.kv_len; ii.kv_off = td.kv_off;
-          mbar_arrive(bar(SCHED_FULL + slot));
-        }
-        if (td.n_kv == 0) continue;
-        const int kv_lo = td.lo & ~(kBlock - 1);
-        const int nblk_total = (td.kv_hi + kBlock - 1) / kBlock;   // blocks [0, nblk_total) of the request hold visible keys
-        const int* bt = a.block_tables + (size_t)td.r * a.max_blocks;
-        auto block_grp = [&](int i) {   // cache row-group coordinate of this lane's block (lanes 0-7) of KV tile i
-          const int b = (kv_lo >> 4) + i * (BN / kBlock) + lane;
-          return (lane < BN / kBlock && b < nblk_total) ? (__ldg(bt + b) * prm.hkv + kvh) * 2 : prm.oob_grp;
+        w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
+        if (__any_sync(0xffffffffu, w.dead) || sm.ring[slot].t0 < 0) break;
+        const Item it = load_item<TOK>(sm.ring[slot], rank);
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
+        if (it.n_kv == 0) continue;
+        const int nblk_total = (it.kv_hi + kBlock - 1) / kBlock;   // blocks [0, nblk_total) of the request hold visible keys
+        const int* bt = a.block_tables + (size_t)it.r * a.max_blocks;
+        auto block_grp = [&](int i) {   // cache row-group coordinate of this lane's block (lanes 0-3) of KV tile i
+          const int b = (it.kv_lo >> 4) + i * (BN / kBlock) + rank * (kKeysCta / kBlock) + lane;
+          return (lane < kKeysCta / kBlock && b < nblk_total) ? (__ldg(bt + b) * prm.hkv + it.kvh) * 2 : prm.oob_grp;
         };
         int y = block_grp(0);
-        for (int i = 0; i < td.n_kv; ++i) {
-          const int y_next = (i + 1 < td.n_kv) ? block_grp(i + 1) : 0;
+        for (int i = 0; i < it.n_kv; ++i) {
+          const int y_next = (i + 1 < it.n_kv) ? block_grp(i + 1) : 0;
           {  // K tile i: one 4 KB box per physical block
             const int st = kc % kKStages;
-            if (lane == 0) { w.wait(bar(K_EMPTY + st), ((kc / kKStages) & 1) ^ 1); mbar_expect_tx(bar(K_FULL + st), kTileBytes); }
+            if (lane == 0) { w.wait(bar(K_EMPTY + st), ((kc / kKStages) & 1) ^ 1); mbar_expect_tx(bar(K_FULL + st), kKTileBytes); }
             __syncwarp();
-            if (lane < BN / kBlock) tma_load_4d(smem_u32(sm.k[st]) + lane * 4096, &tmap_k, bar(K_FULL + st), 0, 0, 0, y);
+            if (lane < kKeysCta / kBlock) tma_load_4d(smem_u32(sm.k[st]) + lane * 4096, &tmap_k, bar(K_FULL + st), 0, 0, 0, y);
             ++kc;
             TRACE_L0(0, 2);
           }
-          if (i == 0) {  // Q super-tile: rows (token, head-in-group), tile A then tile B
-            const int ntile = td.ntok > TOK ? 2 : 1;
+          if (i == 0) {  // this CTA's Q rows: (token, head-in-group), tile A then tile B
+            const int ntile = it.ntok_b > 0 ? 2 : (it.ntok_a > 0 ? 1 : 0);
             if (lane == 0) { w.wait(bar(Q_EMPTY), (qc & 1) ^ 1); mbar_expect_tx(bar(Q_FULL), ntile * kTileBytes); }
             __syncwarp();
             if (lane < 2 * ntile) {
               const int x = lane >> 1, h = lane & 1;
-              tma_load_3d(smem_u32(sm.q[x]) + h * kHalfBytes, &tmap_q, bar(Q_FULL), 64 * h, kvh * G, td.t0 + x * TOK);
+              tma_load_3d(smem_u32(sm.q[x]) + h * kHalfBytes, &tmap_q, bar(Q_FULL), 64 * h, it.kvh * G, it.t0 + it.tb + x * TOK);
             }
             ++qc;
             TRACE_L0(0, 3);
@@ -512,15 +628,15 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         }
       }
     } else if (warp == 14) {
-      // ============================================================ V TMA producer (a4): follows the item ring
+      // ============================================================ V TMA producer (a4): this CTA's half of head_dim, all 128 keys
       uint32_t vc = 0;
       for (uint32_t it_n = 0;; ++it_n) {
         const int slot = it_n & (kRing - 1);
-        w.wait(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
+        w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
         if (__any_sync(0xffffffffu, w.dead) || sm.ring[slot].t0 < 0) break;
         const ItemInfo ii = sm.ring[slot];
         __syncwarp();
-        if (lane == 0) mbar_arrive(bar(SCHED_EMPTY + slot));
+        if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
         if (ii.n_kv == 0) continue;
         const int kv_lo = ii.lo & ~(kBlock - 1);
         const int nblk_total = (ii.kv_hi + kBlock - 1) / kBlock;
@@ -533,43 +649,43 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         for (int i = 0; i < ii.n_kv; ++i) {
           const int y_next = (i + 1 < ii.n_kv) ? block_grp(i + 1) : 0;
           const int st = vc % kVStages;
-          if (lane == 0) { w.wait(bar(V_EMPTY + st), ((vc / kVStages) & 1) ^ 1); mbar_expect_tx(bar(V_FULL + st), kTileBytes); }
+          if (lane == 0) { w.wait(bar(V_EMPTY + st), ((vc / kVStages) & 1) ^ 1); mbar_expect_tx(bar(V_FULL + st), kVTileBytes); }
           __syncwarp();
-          if (lane < BN / kBlock) tma_load_4d(smem_u32(sm.v[st]) + lane * 4096, &tmap_v, bar(V_FULL + st), 0, 0, 0, y);
+          if (lane < BN / kBlock) tma_load_4d(smem_u32(sm.v[st]) + lane * 2048, &tmap_v, bar(V_FULL + st), 0, 0, rank, y);
           ++vc;
           TRACE_L0(0, 4);
           y = y_next;
         }
       }
-    } else if (warp == 13) {
-      // ============================================================ MMA issuer (a6, a8)
+    } else if (warp == 13 && rank == 0) {
+      // ============================================================ MMA issuer (a6, a8), leader CTA only
       // The whole warp runs the control flow converged on warp-uniform values (item fields are broadcast from
       // lane 0, so descriptors, stages and phases live in uniform registers); one elected lane issues every
-      // tcgen05.mma / tcgen05.commit.  This role lives in 48 registers: 32-bit descriptor words, running
+      // tcgen05.mma / tcgen05.commit for the PAIR.  This role lives in 48 registers: 32-bit descriptor words, running
       // stage / phase counters, no per-stage tables.
       constexpr uint32_t idesc_qk = instr_desc(false), idesc_pv = instr_desc(true);
       const uint32_t q_lo = ((smem_u32(sm.q[0]) >> 4) & 0x3FFF) | (1u << 16);          // + x * 2048
-      const uint32_t k_lo = ((smem_u32(sm.k[0]) >> 4) & 0x3FFF) | (1u << 16);          // + stage * 2048
-      const uint32_t v_lo = ((smem_u32(sm.v[0]) >> 4) & 0x3FFF) | ((uint32_t)(kKvHalfOff >> 4) << 16);
+      const uint32_t k_lo = ((smem_u32(sm.k[0]) >> 4) & 0x3FFF) | (1u << 16);          // + stage * 1024
+      const uint32_t v_lo = ((smem_u32(sm.v[0]) >> 4) & 0x3FFF) | (1u << 16);          // + stage * 1024
       uint32_t k_st = 0, k_ph = 0, v_st = 0, v_ph = 0;   // next K / V stage to consume and its full-barrier parity
       uint32_t ph = 0;   // bit 0,1: P_FULL parity of tile A,B; bit 2,3: O_FREE; bit 4: Q_READY; bit 5: V_FIX
       for (uint32_t it_n = 0;; ++it_n) {
         const int slot = it_n & (kRing - 1);
-        w.wait(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
+        w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
         if (__any_sync(0xffffffffu, w.dead) || sm.ring[slot].t0 < 0) break;
-        int n, nx0, nx1, kv_hi;
+        int n, nx1, kv_hi;
         {
-          const Item it = load_item<TOK>(sm.ring[slot]);
-          n = __shfl_sync(0xffffffffu, it.n_kv, 0); nx0 = __shfl_sync(0xffffffffu, it.n_a, 0);
+          const Item it = load_item<TOK>(sm.ring[slot], 0);
+          n = __shfl_sync(0xffffffffu, it.n_kv, 0);
           nx1 = __shfl_sync(0xffffffffu, it.n_b, 0); kv_hi = __shfl_sync(0xffffffffu, it.kv_hi, 0);
         }
         const bool vfix = (kv_hi & (kBlock - 1)) != 0;
         __syncwarp();
-        if (lane == 0) mbar_arrive(bar(SCHED_EMPTY + slot));
+        if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
         if (n == 0) continue;
-        // QK^T of tile x against K stage st: S_x = Q_x K'^T (elected lane only)
+        // QK^T of tile x against K stage st: S_x = Q_x K'^T for both CTAs (elected lane only)
         auto qk = [&](int x, uint32_t st) {
-          const uint32_t a_lo = q_lo + (uint32_t)x * (kTileBytes >> 4), b_lo = k_lo + st * (kTileBytes >> 4);
+          const uint32_t a_lo = q_lo + (uint32_t)x * (kTileBytes >> 4), b_lo = k_lo + st * (kKTileBytes >> 4);
 #pragma unroll
           for (int ks = 0; ks < D / 16; ++ks) {
             const uint32_t off_q = (ks >> 2) * (kHalfBytes >> 4) + (ks & 3) * 2, off_k = (ks >> 2) * (kKvHalfOff >> 4) + (ks & 3) * 2;
@@ -581,7 +697,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         w.wait(bar(Q_READY), (ph >> 4) & 1);   // tile A of Q is rotated; tile B follows while QK_A already runs
         w.wait(bar(K_READY + k_st), k_ph);
         tc_fence_after();
-        if (nx0 > 0 && elect_one()) qk(0, k_st);
+        if (elect_one()) qk(0, k_st);
         __syncwarp();
         w.wait(bar(Q_READY + 1), (ph >> 4) & 1); ph ^= 16u;
         tc_fence_after();
@@ -595,11 +711,12 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
 #pragma unroll 1
         for (int i = 0; i < n; ++i) {
           w.wait(bar(V_FULL + v_st), v_ph);
+          w.wait(bar(V_PEER + v_st), v_ph);
           if (i == n - 1 && vfix) { w.wait(bar(V_FIX), (ph >> 5) & 1); ph ^= 32u; }
           bool k_waited = false;
 #pragma unroll 1
           for (int x = 0; x < 2; ++x) {
-            const int nx = x ? nx1 : nx0;
+            const int nx = x ? nx1 : n;
             const bool do_pv = i < nx, do_qk = i + 1 < nx;
             if (do_pv) {
               w.wait(bar(P_FULL + x), (ph >> x) & 1); ph ^= 1u << x;
@@ -607,10 +724,10 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
             }
             tc_fence_after();
             if (do_pv && elect_one()) {
-              const uint32_t b_lo = v_lo + v_st * (kTileBytes >> 4);
+              const uint32_t b_lo = v_lo + v_st * (kVTileBytes >> 4);
 #pragma unroll
               for (int ks = 0; ks < BN / 16; ++ks)
-                umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, b_lo + ks * (2 * kGroupBytes >> 4), idesc_pv, (i > 0 || ks > 0));
+                umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, b_lo + ks * (2 * kVGroupBytes >> 4), idesc_pv, (i > 0 || ks > 0));
               if (i == nx - 1) tc_commit(bar(O_FULL + x));
               TRACE(1, 20 + x);
             }
@@ -633,7 +750,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       }
     }
   } else if (warp >= 8) {
-    // ============================================================ rotation warps: K tiles (a5)
+    // ============================================================ rotation warps: this CTA's 64 keys of every K tile (a5)
     // NOTE on code shape: the kernel is instruction-cache bound (four roles with different code share an SM), so only the
     // per-tile K path is unrolled.  The once-per-item Q rotation (a3) lives in the softmax warps as a rolled loop.
     reg_dec<kRegsRot>();
@@ -651,47 +768,48 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
     const uint32_t off_e = (uint32_t)(rsub * 128 + ((ch ^ rsub) << 4));
     const uint32_t off_o = (uint32_t)((4 + rsub) * 128 + ((ch ^ (4 + rsub)) << 4));
     const bool k_prerot = (prm.flags & MINIPIC_K_PREROTATED) != 0;
+    constexpr int RW = kKeysCta / 4;   // 16 tile rows (= 2 row groups) per rotation warp
     uint32_t kc = 0, vc = 0;
     for (uint32_t it_n = 0;; ++it_n) {
       const int slot = it_n & (kRing - 1);
-      w.wait(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
+      w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
       if (w.dead || sm.ring[slot].t0 < 0) break;
-      const Item it = load_item<TOK>(sm.ring[slot]);
+      const Item it = load_item<TOK>(sm.ring[slot], rank);
       __syncwarp();
-      if (lane == 0) mbar_arrive(bar(SCHED_EMPTY + slot));
+      if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
       if (it.n_kv == 0) continue;
       const int* pos = a.kv_positions + it.kv_off;
-      // lane l holds the position of key 32 rw + l of the tile / of Q token 32 rw / G + l of tile A, B (fetched early)
-      int myp = __ldg(pos + min(it.kv_lo + 32 * rw + lane, it.kv_len - 1));
+      const int jw = it.kv_lo + rank * kKeysCta + RW * rw;   // first key of this warp's rows in tile 0
+      // lane l (< 16) holds the position of key jw + i * 128 + l (fetched one tile early)
+      int myp = __ldg(pos + min(jw + (lane & (RW - 1)), it.kv_len - 1));
       for (int i = 0; i < it.n_kv; ++i) {
         const int st = kc % kKStages;
-        const int j0 = it.kv_lo + i * BN + 32 * rw;
-        const int myp_next = (i + 1 < it.n_kv) ? __ldg(pos + min(j0 + BN + lane, it.kv_len - 1)) : 0;
+        const int j0 = jw + i * BN;
+        const int myp_next = (i + 1 < it.n_kv) ? __ldg(pos + min(j0 + BN + (lane & (RW - 1)), it.kv_len - 1)) : 0;
         const int nrow = it.kv_hi - j0;                   // rows of this warp's chunk that hold visible keys
         const bool work = !k_prerot && nrow > 0;
         const int p0 = __shfl_sync(0xffffffffu, myp, 0);
         // consecutive positions (every workload the paper describes): one exact restart, then 4-position steps
-        const bool contig = __all_sync(0xffffffffu, lane >= nrow || myp == p0 + lane);
+        const bool contig = __all_sync(0xffffffffu, (lane & (RW - 1)) >= nrow || myp == p0 + (lane & (RW - 1)));
         if (work && contig) rot.restart(p0 + rsub, finc_addr);          // before the wait: overlaps the TMA latency
         w.wait(bar(K_FULL + st), (kc / kKStages) & 1);
         if (rw == 0) TRACE_L0(2, 30);
         if (work) {
-          const uint32_t kt = smem_u32(sm.k[st]) + (uint32_t)rw * (4 * kGroupBytes);
+          const uint32_t kt = smem_u32(sm.k[st]) + (uint32_t)rw * (2 * kGroupBytes);
           auto row_addr = [&](int k) { return kt + (k >> 1) * kGroupBytes + ((k & 1) ? off_o : off_e); };
           if (contig) {
             uint4 lo = lds128(row_addr(0)), hi = lds128(row_addr(0) + kKvHalfOff);
 #pragma unroll
-            for (int k = 0; k < 8; ++k) {
-              if (k == 4 && nrow <= 16) break;
+            for (int k = 0; k < RW / 4; ++k) {
               uint4 lo_n = lo, hi_n = hi;
-              if (k < 7) { lo_n = lds128(row_addr(k + 1)); hi_n = lds128(row_addr(k + 1) + kKvHalfOff); }
+              if (k < RW / 4 - 1) { lo_n = lds128(row_addr(k + 1)); hi_n = lds128(row_addr(k + 1) + kKvHalfOff); }
               rot.rotate_store(row_addr(k), kKvHalfOff, lo, hi);
-              if (k < 7) rot.advance(c4, s4, ns4);
+              if (k < RW / 4 - 1) rot.advance(c4, s4, ns4);
               lo = lo_n; hi = hi_n;
             }
           } else {
 #pragma unroll 1
-            for (int k = 0; k < 8; ++k) {
+            for (int k = 0; k < RW / 4; ++k) {
               if (4 * k >= nrow) break;
               rot.restart(__shfl_sync(0xffffffffu, myp, 4 * k + rsub), finc_addr);
               const uint4 lo = lds128(row_addr(k)), hi = lds128(row_addr(k) + kKvHalfOff);
@@ -700,7 +818,8 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           }
         }
         fence_proxy_async();
-        mbar_arrive(bar(K_READY + st));
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cl(lbar(K_READY + st));
         if (rw == 0) TRACE_L0(2, 31);
         ++kc;
         myp = myp_next;
@@ -711,9 +830,9 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           w.wait(bar(V_FULL + vs), ((vc + i) / kVStages) & 1);
           const int first = it.kv_hi - (it.kv_lo + i * BN), last = (first + kBlock - 1) & ~(kBlock - 1);
           if (rot_tid >= first && rot_tid < last) {
-            const uint32_t vrow = smem_u32(sm.v[vs]) + (rot_tid >> 3) * kGroupBytes + (rot_tid & 7) * 128;
+            const uint32_t vrow = smem_u32(sm.v[vs]) + (rot_tid >> 3) * kVGroupBytes + (rot_tid & 7) * 128;
 #pragma unroll
-            for (int c = 0; c < 8; ++c) { sts128z(vrow + c * 16); sts128z(vrow + kKvHalfOff + c * 16); }
+            for (int c = 0; c < 8; ++c) sts128z(vrow + c * 16);
           }
           fence_proxy_async();
           mbar_arrive(bar(V_FIX));
@@ -739,19 +858,26 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       const float inv = pe.l > 0.f ? 1.f / pe.l : 0.f;
       if (pe.n > 0) { w.wait(bar(O_FULL + x), oc & 1); ++oc; tc_fence_after(); }
       if ((warp & 3) == 0) TRACE_L0(3 + x, 42);
+      if (pe.ntok_x <= 0) {   // this CTA owns no row of the tile (the peer does): only release O
+        if (pe.n > 0) { tc_fence_before(); __syncwarp(); if (lane == 0) mbar_arrive_cl(lbar(O_FREE + x)); }
+        return;
+      }
       {
         const uint32_t stg = smem_u32(sm.ostage[warp]);
         const int rr = lane >> 3, cc = lane & 7;
         const bool whole = pe.ntok_x == TOK;   // every row of the tile is a real query row: the warp's 32 rows go out
                                                   // as one TMA tensor store per pass (box = 64 columns x G heads x 32/G tokens)
-        __nv_bfloat16* obase = (__nv_bfloat16*)a.out + ((size_t)(pe.t0 + x * TOK) * prm.hq + pe.kvh * G) * D + cc * 8;
+        __nv_bfloat16* obase = (__nv_bfloat16*)a.out + ((size_t)pe.t0 * prm.hq + pe.kvh * G) * D + cc * 8;
 #pragma unroll 1
         for (int pass = 0; pass < 2; ++pass) {
           float o[64];
           if (pe.n > 0) {
             tmem_ld32(t_o + pass * 64, o); tmem_ld32(t_o + pass * 64 + 32, o + 32);
             tmem_wait_ld();
-            if (pass == 1) { tc_fence_before(); mbar_arrive(bar(O_FREE + x)); }   // O is in registers: the next item may start
+            if (pass == 1) {   // O is in registers: the next item may start
+              tc_fence_before(); __syncwarp();
+              if (lane == 0) mbar_arrive_cl(lbar(O_FREE + x));
+            }
           } else {
 #pragma unroll
             for (int e = 0; e < 64; ++e) o[e] = 0.f;
@@ -769,7 +895,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
             fence_proxy_async();
             __syncwarp();
             if (lane == 0) {
-              tma_store_3d(&tmap_o, stg, pass * 64, pe.kvh * G, pe.t0 + x * TOK + ((warp & 3) * 32) / G);
+              tma_store_3d(&tmap_o, stg, pass * 64, pe.kvh * G, pe.t0 + ((warp & 3) * 32) / G);
               tma_store_commit();
             }
           } else {
@@ -787,7 +913,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       }
       if ((warp & 3) == 0) TRACE_L0(3 + x, 43);
       if ((tok_in < pe.ntok_x))
-        a.lse[(size_t)(pe.t0 + x * TOK + tok_in) * prm.hq + pe.kvh * G + hg] =
+        a.lse[(size_t)(pe.t0 + tok_in) * prm.hq + pe.kvh * G + hg] =
             pe.l > 0.f ? (pe.m + log2f(pe.l)) * 0.6931471805599453f : -INFINITY;
         };
     // Q rotation (a3) state of this lane: same row / chunk mapping as the K rotation lanes
@@ -799,11 +925,13 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
     constexpr int NTW = (32 / G) > 0 ? (32 / G) : 1;   // Q tokens per warp per tile
     for (uint32_t it_n = 0;; ++it_n) {
       const int slot = it_n & (kRing - 1);
-      w.wait(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
+      w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
       const bool stop = w.dead || sm.ring[slot].t0 < 0;   // one more trip for the deferred epilogue, then out
-      const Item it = load_item<TOK>(sm.ring[slot]);
+      const Item it = load_item<TOK>(sm.ring[slot], rank);
       __syncwarp();
-      if (!stop && lane == 0) mbar_arrive(bar(SCHED_EMPTY + slot));
+      if (!stop && lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
+      const int n = stop ? 0 : it.n_x(x);      // KV tiles this tile slot runs (the same in both CTAs)
+      const int tile_t = it.tb + x * TOK;      // first token (within the item) of this CTA's tile x
       if (!stop && it.n_kv > 0) {
         // ---- a3: rotate this warp's 32 rows of Q tile x in place: row = token * G + head-in-group, the G rows of a token
         //      share one position.  Exact restart at the first row, one-position steps while the positions are consecutive.
@@ -813,7 +941,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         int qpx = 0;
         if (!q_prerot && ntw > 0) {
           const int tk = min((32 * rw) / G + min(lane, NTW - 1), it.ntok_x(x) - 1);
-          qpx = __ldg(a.kv_positions + it.kv_off + min(it.idx0 + x * TOK + tk, it.kv_len - 1));
+          qpx = __ldg(a.kv_positions + it.kv_off + min(it.idx0 + tile_t + tk, it.kv_len - 1));
         }
         w.wait(bar(Q_FULL), qc & 1); ++qc;
         if (!q_prerot && ntw > 0) {
@@ -841,15 +969,14 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           }
         }
         fence_proxy_async();
-        mbar_arrive(bar(Q_READY + x));
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cl(lbar(Q_READY + x));
       }
       if (pe.valid) epilogue();   // previous item of this tile
       if (stop) break;
       const bool row_ok = tok_in < it.ntok_x(x);
-      const int tok = x * TOK + tok_in;
-      const int idx_first = it.idx0 + x * TOK;                       // lowest query index of this tile
-      const int idx_row = min(it.idx0 + tok, it.kv_len - 1);         // highest visible key of this row
-      const int n = it.n_x(x);
+      const int idx_first = it.idx0 + tile_t;                               // lowest query index of this tile
+      const int idx_row = min(it.idx0 + tile_t + tok_in, it.kv_len - 1);    // highest visible key of this row
       float m_used = -INFINITY, l_run = 0.f;   // m in log2 units (score * scale * log2 e)
       for (int i = 0; i < n; ++i, ++sc) {
         const int j0 = it.kv_lo + i * BN;
@@ -931,22 +1058,26 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         if ((warp & 3) == 0) TRACE_L0(3 + x, 46);
         tmem_wait_st();
         tc_fence_before();
-        mbar_arrive(bar(P_FULL + x));
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cl(lbar(P_FULL + x));
         if ((warp & 3) == 0) TRACE_L0(3 + x, 41);
       }
       // the epilogue of an item is DEFERRED until this tile's Q rows of the next item are rotated (below), so that QK of the
-      // next item starts ~3 K cycles earlier; pe = what it needs
-      pe.valid = it.ntok_x(x) > 0; pe.t0 = it.t0; pe.kvh = it.kvh; pe.ntok_x = it.ntok_x(x); pe.n = n; pe.l = l_run; pe.m = m_used;
+      // next item starts ~3 K cycles earlier; pe = what it needs.  A tile slot that ran KV tiles for the peer's rows only
+      // (ntok_x = 0, n > 0) still has to consume O_FULL and release O.
+      pe.valid = it.ntok_x(x) > 0 || n > 0; pe.t0 = it.t0 + tile_t; pe.kvh = it.kvh; pe.ntok_x = it.ntok_x(x); pe.n = n;
+      pe.l = l_run; pe.m = m_used;
     }
     if (lane == 0) tma_store_wait_all();   // the staging buffers must outlive the last tensor stores
   }
   tc_fence_before();
-  __syncthreads();
+  cluster_sync_all();   // no CTA may exit (or free TMEM) while its peer can still arrive on its barriers / run MMAs on it
   if (warp == 13) {
     tc_fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512));
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(tmem), "r"(512));
   }
 }
+
 
 // ------------------------------------------------------------------------------------------------ host
 typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
@@ -965,12 +1096,13 @@ EncodeTiledFn get_encode() {
 }
 // cache viewed as a 4-D bf16 tensor (64 columns, 8 rows of a group [256 B apart], 2 halves of head_dim [128 B apart],
 // row groups [2048 B apart]); box = (64, 8, 2, 2) = one (block, head) = 4 KB landing as [group][half][8 x 128 B], SWIZZLE_128B
-bool make_cache_map(CUtensorMap* m, const void* cache, int num_blocks, int hkv) {
+// halves = 2: K (both halves of head_dim, 4 KB per block); halves = 1: V (the CTA's half, chosen by the box coordinate, 2 KB)
+bool make_cache_map(CUtensorMap* m, const void* cache, int num_blocks, int hkv, int halves) {
   EncodeTiledFn enc = get_encode();
   if (!enc) return false;
   cuuint64_t dims[4] = {64, 8, 2, (cuuint64_t)num_blocks * hkv * 2};
   cuuint64_t strides[3] = {(cuuint64_t)D * 2, 128, (cuuint64_t)kGroupBytes};
-  cuuint32_t box[4] = {64, 8, 2, 2};
+  cuuint32_t box[4] = {64, 8, (cuuint32_t)halves, 2};
   cuuint32_t estr[4] = {1, 1, 1, 1};
   return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(cache), dims, strides, box, estr,
              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -1053,7 +1185,7 @@ size_t prefill_sm100_workspace_bytes(const Ctx&, int, int num_q_tokens) {
 
 bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
   CUtensorMap mq, mk, mv, mo;
-  if (!make_cache_map(&mk, a.k_cache, c.num_blocks, c.hkv) || !make_cache_map(&mv, a.v_cache, c.num_blocks, c.hkv) ||
+  if (!make_cache_map(&mk, a.k_cache, c.num_blocks, c.hkv, 2) || !make_cache_map(&mv, a.v_cache, c.num_blocks, c.hkv, 1) ||
       !make_q_map(&mq, a.q, a.num_q_tokens, c.hq, c.group) || !make_out_map(&mo, a.out, a.num_q_tokens, c.hq, c.group)) {
     note_error("prefill_sm100: cuTensorMapEncodeTiled failed (driver entry point missing or bad tensor geometry)");
     return false;
@@ -1061,7 +1193,7 @@ bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
   PlanHeader* hdr = (PlanHeader*)a.workspace;
   TileDesc* sorted = (TileDesc*)((char*)a.workspace + sizeof(PlanHeader));
   TileDesc* tmp = sorted + (a.num_q_tokens + 1);
-  const int tok2 = 2 * BM / c.group;
+  const int tok2 = 4 * BM / c.group;   // query tokens per work item: two 128-row tiles in each CTA of a pair
   if (cudaMemsetAsync(hdr, 0, sizeof(PlanHeader), c.stream) != cudaSuccess) return false;
   plan_mark_kernel<<<(a.num_q_tokens + 255) / 256, 256, 0, c.stream>>>(a, tok2, hdr, tmp);
   plan_scan_kernel<<<1, 1024, 0, c.stream>>>(hdr);
@@ -1078,7 +1210,7 @@ bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
     prm.step1[i] = make_float2((float)c1, (float)s1);
     prm.step4[i] = make_float2((float)(c2 * c2 - s2 * s2), (float)(2.0 * s2 * c2));
   }
-  const int sms = current_sm_count();
+  const int sms = current_sm_count() & ~1;   // CTA pairs (clusters of 2)
   switch (c.group) {
     case 1: return launch_g<1>(c, mq, mk, mv, mo, prm, sms);
     case 2: return launch_g<2>(c, mq, mk, mv, mo, prm, sms);
