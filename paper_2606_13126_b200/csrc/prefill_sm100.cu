@@ -23,7 +23,6 @@
 // All hand-offs are mbarriers; generic-proxy smem writes are fenced with fence.proxy.async before the MMA reads.
 #include <cuda.h>
 #include <cstddef>
-#include <cstdlib>
 
 #include "internal.h"
 
@@ -40,7 +39,7 @@ constexpr int kHalfBytes = kTileBytes / 2;   // [half of head_dim][128 rows][128
 constexpr int kKeysCta = BN / 2;
 constexpr int kKTileBytes = kKeysCta * D * 2;    // 8 row groups of [half (2)][8 rows x 128 B]
 constexpr int kVTileBytes = BN * (D / 2) * 2;    // 16 row groups of [8 rows x 128 B] (this CTA's half of head_dim)
-constexpr int kKStages = 4, kVStages = 2, kRing = 4;   // kKStages: power of two (stage = use & 3)
+constexpr int kKStages = 3, kVStages = 3, kRing = 4;
 // Measured and dropped (config 5, in-kernel RoPE; the kept version runs 2.24 ms):
 //  * a ring of three Q tile slots (next item's tile A loaded + rotated during the current item, epilogue staged in the
 //    finishing item's tile-B slot): parity-green, dense +3 %, but span items -7 % (2.30 ms): the four rotation warps are
@@ -66,6 +65,7 @@ constexpr int kKStages = 4, kVStages = 2, kRing = 4;   // kKStages: power of two
 // K / V tile in shared memory: 16 row groups of [half of head_dim (2)][8 rows x 128 B] = 2048 B each, so one (block, head)
 // of the cache (16 tokens x 256 B) is ONE 4-D TMA box of two groups.  Q tile: [half (2)][128 rows x 128 B].
 constexpr int kGroupBytes = 2048, kKvHalfOff = 1024, kVGroupBytes = 1024;
+constexpr int kStageBytes = 4096;            // epilogue staging per softmax warp: 32 rows x 128 B (64 bf16 columns)
 // 16 warps = 4 warpgroups: softmax A, softmax B (184 registers each after setmaxnreg), rotation (96), control (TMA, MMA and
 // two idle warps, 48).  setmaxnreg is a WARPGROUP-wide instruction (all four warps, same count), and the split must fit the
 // launch pool of 512 * 128 registers or setmaxnreg.inc blocks forever: 256*184 + 128*96 + 128*48 = 65536.
@@ -75,7 +75,7 @@ static_assert(256 * kRegsSoftmax + 128 * kRegsRot + 128 * kRegsCtl <= 65536, "se
 constexpr int kMaxBins = 4096;
 constexpr unsigned kWaitMaxSpins = 1u << 26;   // x (>= 30 cycles per failed try_wait) = seconds
 
-struct TileDesc { int t0, ntok, r, idx0, lo, n_kv, kv_hi, kv_len, kv_off, cost; };   // kv_off = cu_kv_lens[r]
+struct TileDesc { int t0, ntok, r, idx0, lo, n_kv, kv_hi, kv_len, kv_off, pad; };   // kv_off = cu_kv_lens[r]
 // magic tags a header written by THIS kernel family, so minipic_prefill_status() can tell it from a workspace that a call
 // dispatched to another kernel never touched (err and magic are adjacent: one 8-byte read)
 constexpr int kPlanMagic = 0x4d504943;   // "MPIC"
@@ -145,8 +145,6 @@ __device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity) {
 struct Waiter {
   int* err;
   bool dead;
-  uint32_t base;
-  uint32_t dbg = 0;
   // kept tiny on purpose: ~25 wait sites inline this, and the kernel is instruction-cache bound (four roles with
   // different code share an SM).  try_wait suspends in hardware for a bounded time, so spins are cheap to count.
   __device__ __forceinline__ void wait(uint32_t bar, uint32_t parity) {
@@ -154,11 +152,7 @@ struct Waiter {
     unsigned spins = 0;
     while (!mbar_try(bar, parity)) {
       if ((++spins & 4095u) == 0 && (*(volatile int*)err != 0 || spins > kWaitMaxSpins)) {
-        if (atomicCAS(err, 0, (int)(bar | 0x40000000u)) == 0) {   // records the barrier that timed out
-          err[2] = (int)bar; err[3] = (int)parity; err[4] = (int)blockIdx.x; err[5] = (int)threadIdx.x;   // err_info
-        }
-        { const unsigned bi = (bar - base) >> 3; const int mine = (int)(blockIdx.x >> 1) + 1; const int first = atomicCAS(err + 7, 0, mine);
-          if ((first == 0 || first == mine) && ((threadIdx.x & 31) == 0 || (threadIdx.x >= 384 && (bi < 4 || bi > 7) && threadIdx.x % 32 == 0))) { const int e = atomicAdd(err + 8, 1); if (e < 48) { err[10 + 2 * e] = (int)(bi | (parity << 8) | (threadIdx.x << 16) | ((blockIdx.x & 1) << 28)); err[11 + 2 * e] = (int)dbg; } } }
+        atomicCAS(err, 0, (int)(bar | 0x40000000u));   // records the barrier that timed out
         dead = true;
         return;
       }
@@ -170,11 +164,7 @@ struct Waiter {
     unsigned spins = 0;
     while (!mbar_try_cl(bar, parity)) {
       if ((++spins & 4095u) == 0 && (*(volatile int*)err != 0 || spins > kWaitMaxSpins)) {
-        if (atomicCAS(err, 0, (int)(bar | 0x20000000u)) == 0) {
-          err[2] = (int)bar; err[3] = (int)parity; err[4] = (int)blockIdx.x; err[5] = (int)threadIdx.x;
-        }
-        { const unsigned bi = (bar - base) >> 3; const int mine = (int)(blockIdx.x >> 1) + 1; const int first = atomicCAS(err + 7, 0, mine);
-          if ((first == 0 || first == mine) && ((threadIdx.x & 31) == 0 || (threadIdx.x >= 384 && (bi < 4 || bi > 7) && threadIdx.x % 32 == 0))) { const int e = atomicAdd(err + 8, 1); if (e < 48) { err[10 + 2 * e] = (int)(bi | (parity << 8) | (threadIdx.x << 16) | ((blockIdx.x & 1) << 28)); err[11 + 2 * e] = (int)dbg; } } }
+        atomicCAS(err, 0, (int)(bar | 0x20000000u));
         dead = true;
         return;
       }
@@ -308,97 +298,112 @@ __host__ __device__ constexpr uint32_t instr_desc(bool b_mn) {
 }
 
 // ------------------------------------------------------------------------------------------------ a2: plan
-// A run of consecutive query rows of one request that share vis_lo is cut into work items:
-//  * RESIDENT region - rows whose keys all lie in the first kKStages * 128 keys from floor16(vis_lo) (a whole span of up to
-//    512 tokens; the head of a longer one): items of up to `cap` tokens (a multiple of T4).  Such an item runs as
-//    cap / T4 SUB-ITEMS over K tiles that are gathered and rotated ONCE and stay in shared memory;
-//  * beyond it: items of T4 tokens (one sub-item) that stream their K tiles through the same ring.
-// T4 = 4 * 128 / G tokens = one 128-row tile A and B in each CTA of the pair.
-constexpr int kResKeys = 4 * BN;   // == kKStages * BN (static_assert below)
-__device__ __forceinline__ bool tile_starts(const PrefillArgs& a, int t, int r, int t4, int cap) {
+__device__ __forceinline__ bool tile_starts(const PrefillArgs& a, int t, int r, int tok) {
   if (t == __ldg(a.cu_q_lens + r)) return true;
   const int i1 = __ldg(a.q_seq_idx + t), i0 = __ldg(a.q_seq_idx + t - 1);
   const int l1 = __ldg(a.q_vis_lo + t), l0 = __ldg(a.q_vis_lo + t - 1);
-  if (i1 != i0 + 1 || l1 != l0) return true;
-  const int lo = max(l1, 0), off = i1 - lo, rel = i1 - (lo & ~(kBlock - 1));
-  if (rel < kResKeys) return (off % cap) == 0;
-  return rel == kResKeys || (off % t4) == 0;
+  return i1 != i0 + 1 || l1 != l0 || ((i1 - max(l1, 0)) % tok) == 0;
 }
 
-// one thread per query token: the tokens that start an item emit its descriptor and count it in the cost histogram
-__global__ void __launch_bounds__(256) plan_mark_kernel(PrefillArgs a, int t4, int cap, PlanHeader* hdr, TileDesc* tmp) {
-  const int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t == 0) hdr->magic = kPlanMagic;
-  if (t >= a.num_q_tokens) return;
-  int lo_r = 0, hi_r = a.num_reqs;
-  while (hi_r - lo_r > 1) {
-    const int mid = (lo_r + hi_r) >> 1;
-    if (__ldg(a.cu_q_lens + mid) <= t) lo_r = mid; else hi_r = mid;
+// ONE launch (a2).  Every block marks its 256 query tokens: the start flags of those tokens and of the next `tok` ones go
+// into a shared bitmask, so a starting token finds the length of its item with a find-first-set instead of a sequential
+// scan (which alone took 22 us on config 2); descriptors and the cost histogram are appended with atomics.  The LAST block
+// to finish (ticket) turns the histogram into offsets in DESCENDING cost order and scatters the descriptors: a counting
+// sort, longest item first, that the persistent kernel's atomic work counter then walks.
+constexpr int kPlanThreads = 256, kPlanMaxTok = 512;   // tok = 4 * 128 / G <= 512
+__global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, int tok, PlanHeader* hdr, TileDesc* tmp, TileDesc* sorted) {
+  constexpr int kWords = (kPlanThreads + kPlanMaxTok) / 32;
+  __shared__ unsigned sflag[kWords];
+  __shared__ int s_last;
+  __shared__ int wsum[kPlanThreads / 32];
+  const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
+  const int b0 = blockIdx.x * kPlanThreads;
+  if (blockIdx.x == 0 && tid == 0) hdr->magic = kPlanMagic;
+  auto request_of = [&](int t) {
+    int lo_r = 0, hi_r = a.num_reqs;
+    while (hi_r - lo_r > 1) {
+      const int mid = (lo_r + hi_r) >> 1;
+      if (__ldg(a.cu_q_lens + mid) <= t) lo_r = mid; else hi_r = mid;
+    }
+    return lo_r;
+  };
+  int my_r = 0;
+  for (int c = 0; c * kPlanThreads < kPlanThreads + tok; ++c) {
+    const int t = b0 + c * kPlanThreads + tid;
+    bool f = true;                       // tokens past the end count as starts (sentinel)
+    if (t < a.num_q_tokens) {
+      const int r = request_of(t);
+      if (c == 0) my_r = r;
+      f = tile_starts(a, t, r, tok);
+    }
+    const unsigned m = __ballot_sync(0xffffffffu, f);
+    if (lane == 0) sflag[c * (kPlanThreads / 32) + wid] = m;
   }
-  const int r = lo_r;
-  if (!tile_starts(a, t, r, t4, cap)) return;
-  const int t_end = __ldg(a.cu_q_lens + r + 1);
-  int n = 1;
-  while (n < cap && t + n < t_end && !tile_starts(a, t + n, r, t4, cap)) ++n;
-  TileDesc td;
-  td.t0 = t; td.ntok = n; td.r = r; td.idx0 = __ldg(a.q_seq_idx + t); td.lo = max(__ldg(a.q_vis_lo + t), 0);
-  td.kv_len = __ldg(a.kv_lens + r);
-  td.kv_off = __ldg(a.cu_kv_lens + r);
-  const int kv_lo = td.lo & ~(kBlock - 1);
-  td.kv_hi = min(td.idx0 + n, td.kv_len);
-  td.n_kv = td.kv_hi > kv_lo ? (td.kv_hi - kv_lo + BN - 1) / BN : 0;
-  int cost = 0;   // KV tile-steps over the sub-items: the sort key (longest first)
-  for (int q0 = 0; q0 < n; q0 += t4) {
-    const int hi = min(td.idx0 + min(q0 + t4, n), td.kv_len);
-    cost += hi > kv_lo ? (hi - kv_lo + BN - 1) / BN : 0;
+  __syncthreads();
+  const int t = b0 + tid;
+  if (t < a.num_q_tokens && ((sflag[tid >> 5] >> (tid & 31)) & 1u)) {
+    int nxt = -1;                        // local index of the next start after tid
+    unsigned wbits = sflag[tid >> 5] & ~((2u << (tid & 31)) - 1u);
+    for (int wi = tid >> 5; nxt < 0; ++wi) {
+      if (wbits) nxt = wi * 32 + __ffs(wbits) - 1;
+      else wbits = sflag[wi + 1];        // a start exists within `tok` tokens (item length rule / end sentinel)
+    }
+    const int n = min(nxt - tid, tok);
+    const int r = my_r;
+    TileDesc td;
+    td.t0 = t; td.ntok = n; td.r = r; td.idx0 = __ldg(a.q_seq_idx + t); td.lo = max(__ldg(a.q_vis_lo + t), 0);
+    td.kv_len = __ldg(a.kv_lens + r);
+    td.kv_off = __ldg(a.cu_kv_lens + r); td.pad = 0;
+    const int kv_lo = td.lo & ~(kBlock - 1);
+    td.kv_hi = min(td.idx0 + n, td.kv_len);
+    td.n_kv = td.kv_hi > kv_lo ? (td.kv_hi - kv_lo + BN - 1) / BN : 0;
+    tmp[atomicAdd(&hdr->n_tiles, 1)] = td;
+    atomicAdd(&hdr->hist[min(td.n_kv, kMaxBins - 1)], 1);
   }
-  td.cost = cost;
-  tmp[atomicAdd(&hdr->n_tiles, 1)] = td;
-  atomicAdd(&hdr->hist[min(cost, kMaxBins - 1)], 1);
-}
-// exclusive prefix over the cost bins in DESCENDING order (longest-first): thread t owns ranks [4t, 4t+4), rank = kMaxBins-1-bin
-__global__ void __launch_bounds__(1024) plan_scan_kernel(PlanHeader* hdr) {
-  __shared__ int wsum[32];
-  const int t = threadIdx.x, lane = t & 31, wid = t >> 5;
-  int v[4], tot = 0;
+  // ---- last block: counting sort of all descriptors, longest first
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) s_last = atomicAdd(&hdr->pad[0], 1) == (int)gridDim.x - 1;
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  constexpr int PER = kMaxBins / kPlanThreads;   // 16 ranks per thread; rank = kMaxBins - 1 - bin (descending cost)
+  volatile int* hist = hdr->hist;
+  int v[PER], tot = 0;
 #pragma unroll
-  for (int e = 0; e < 4; ++e) { v[e] = hdr->hist[kMaxBins - 1 - (4 * t + e)]; tot += v[e]; }
+  for (int e = 0; e < PER; ++e) { v[e] = hist[kMaxBins - 1 - (PER * tid + e)]; tot += v[e]; }
   int incl = tot;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) {
-    const int n = __shfl_up_sync(0xffffffffu, incl, o);
-    if (lane >= o) incl += n;
+    const int nb = __shfl_up_sync(0xffffffffu, incl, o);
+    if (lane >= o) incl += nb;
   }
   if (lane == 31) wsum[wid] = incl;
   __syncthreads();
-  if (wid == 0) {
-    const int w = wsum[lane];
-    int wi = w;
+  int base = incl - tot;
+  for (int w2 = 0; w2 < wid; ++w2) base += wsum[w2];
 #pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const int n = __shfl_up_sync(0xffffffffu, wi, o);
-      if (lane >= o) wi += n;
-    }
-    wsum[lane] = wi - w;
-  }
+  for (int e = 0; e < PER; ++e) { hist[kMaxBins - 1 - (PER * tid + e)] = base; base += v[e]; }
   __syncthreads();
-  int base = wsum[wid] + incl - tot;
+  const int n_tiles = *(volatile int*)&hdr->n_tiles;
+  for (int i = tid; i < n_tiles; i += kPlanThreads) {
+    TileDesc td;   // written by other blocks of this launch: read through L2
+    {
+      const int* src = reinterpret_cast<const int*>(tmp + i);
+      int* dst = reinterpret_cast<int*>(&td);
 #pragma unroll
-  for (int e = 0; e < 4; ++e) { hdr->hist[kMaxBins - 1 - (4 * t + e)] = base; base += v[e]; }
-}
-__global__ void __launch_bounds__(256) plan_scatter_kernel(PlanHeader* hdr, const TileDesc* tmp, TileDesc* sorted) {
-  const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= hdr->n_tiles) return;
-  const TileDesc td = tmp[i];
-  sorted[atomicAdd(&hdr->hist[min(td.cost, kMaxBins - 1)], 1)] = td;
+      for (int e = 0; e < (int)(sizeof(TileDesc) / sizeof(int)); ++e) dst[e] = __ldcg(src + e);
+    }
+    sorted[atomicAdd(&hdr->hist[min(td.n_kv, kMaxBins - 1)], 1)] = td;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------ main kernel
 struct Smem {
-  alignas(1024) unsigned char q[2][2][kTileBytes];   // [buffer][tile A / B]: Q of sub-item s lives in buffer s & 1; after the
-                                                     // sub-item's last QK^T the same bytes stage its epilogue (a9)
+  alignas(1024) unsigned char q[2][kTileBytes];
   alignas(1024) unsigned char k[kKStages][kKTileBytes];
   alignas(1024) unsigned char v[kVStages][kVTileBytes];
+  alignas(1024) unsigned char ostage[8][kStageBytes];
   unsigned long long bars[48];
   alignas(16) ItemInfo ring[kRing];
   alignas(16) unsigned long long finc[64];   // F_i (common.cuh), read by the rotation lanes at every exact restart
@@ -412,10 +417,10 @@ struct Smem {
 enum Bar {
   SCHED_FULL = 0,                       // [kRing] local, 1 arrival by the leader's scheduler (remote for rank 1)
   SCHED_EMPTY = SCHED_FULL + kRing,     // [kRing] leader, 15 consumer warps per CTA
-  Q_FULL = SCHED_EMPTY + kRing,         // [2] local (TMA)
-  Q_READY = Q_FULL + 2,                 // [2] leader, 4 rotation warps per CTA
-  Q_EMPTY = Q_READY + 2,                // [2] local, 8 softmax warps: the sub-item's epilogue has left the buffer
-  K_FULL = Q_EMPTY + 2,                 // [kKStages] local (TMA)
+  Q_FULL = SCHED_EMPTY + kRing,         // local (TMA)
+  Q_READY,                              // [2] leader, 4 softmax warps per CTA
+  Q_EMPTY = Q_READY + 2,                // multicast
+  K_FULL,                               // [kKStages] local (TMA)
   K_READY = K_FULL + kKStages,          // [kKStages] leader, 4 rotation warps per CTA
   K_EMPTY = K_READY + kKStages,         // [kKStages] multicast
   V_FULL = K_EMPTY + kKStages,          // [kVStages] local (TMA)
@@ -431,8 +436,6 @@ enum Bar {
 static_assert(NUM_BARS <= 48, "barrier array too small");
 static_assert(sizeof(Smem) <= 232448, "shared memory budget");
 static_assert(sizeof(ItemInfo) == 48, "ring entries are copied to the peer CTA as three 16-byte stores");
-static_assert(kKStages == 4 && kKStages * BN == kResKeys, "resident items keep all their K tiles in the ring");
-static_assert(kVStages == 2, "V stage = use & 1");
 
 struct Params {
   PrefillArgs a;
@@ -447,46 +450,26 @@ struct Params {
   float2 step4[64];                  // (cos 4 f_i, sin 4 f_i): the four-position RoPE step of the rotation lanes
 };
 
-// A work item: up to `cap` consecutive query tokens of one request with one vis_lo, run as SUB-ITEMS of T4 = 4 * TOK tokens
-// (TOK = 128 / G tokens fill one 128-row MMA tile).  Of a sub-item CTA rank c owns tokens [2 c TOK, 2 c TOK + 2 TOK): tile A
-// the first TOK of those, tile B the rest.  Both CTAs run the SAME number of KV tiles for a tile slot (one MMA covers both);
-// rows a CTA does not own are masked.  An item with several sub-items needs at most kKStages K tiles (the plan guarantees
-// it): tile i is gathered + rotated when the first sub-item that sees it comes up and stays in its ring slot until the
-// last sub-item is done.  V tiles are streamed per sub-item.
+// A work item as one CTA of the pair sees it.  The item covers up to 4 * TOK query tokens (TOK = 128 / G tokens fill one
+// 128-row MMA tile): CTA rank c owns tokens [2 c TOK, 2 c TOK + 2 TOK) of it, tile A the first TOK of those, tile B the rest.
+// Both CTAs run the SAME number of KV tiles for a tile slot (the MMA covers both); rows a CTA does not own are masked.
 struct Item {
-  int t0, ntok, r, idx0, lo, kvh, n_kv, kv_len, kv_off;
-  int kv_lo, nsub;
+  int t0, ntok, r, idx0, lo, kvh, n_kv, kv_hi, kv_len, kv_off;
+  int kv_lo, tb, ntok_a, ntok_b, n_b;
+  __device__ __forceinline__ int ntok_x(int x) const { return x ? ntok_b : ntok_a; }
+  __device__ __forceinline__ int n_x(int x) const { return x ? n_b : n_kv; }   // tile B is skipped by the whole pair if empty
 };
 template <int TOK>
-__device__ __forceinline__ Item load_item(const ItemInfo& ii) {
+__device__ __forceinline__ Item load_item(const ItemInfo& ii, int rank) {
   Item it;
   it.t0 = ii.t0; it.ntok = ii.ntok; it.r = ii.r; it.idx0 = ii.idx0; it.lo = ii.lo; it.kvh = ii.kvh; it.n_kv = ii.n_kv;
-  it.kv_len = ii.kv_len; it.kv_off = ii.kv_off;
+  it.kv_hi = ii.kv_hi; it.kv_len = ii.kv_len; it.kv_off = ii.kv_off;
   it.kv_lo = it.lo & ~(kBlock - 1);
-  it.nsub = max((it.ntok + 4 * TOK - 1) / (4 * TOK), 1);
+  it.tb = rank * 2 * TOK;
+  const int mine = min(max(it.ntok - it.tb, 0), 2 * TOK);
+  it.ntok_a = min(mine, TOK); it.ntok_b = mine - it.ntok_a;
+  it.n_b = it.ntok > TOK ? it.n_kv : 0;
   return it;
-}
-struct Sub {
-  int t_off;               // first token of the sub-item within the item
-  int idx0, kv_hi, n;      // lowest query index, one past the highest visible key, KV tiles [0, n)
-  int tb, ntok_a, ntok_b;  // this CTA: first token within the sub-item, tokens in tile A / B
-  int n_b;                 // KV tiles tile slot B runs (0: the whole pair skips it)
-  __device__ __forceinline__ int ntok_x(int x) const { return x ? ntok_b : ntok_a; }
-  __device__ __forceinline__ int n_x(int x) const { return x ? n_b : n; }
-};
-template <int TOK>
-__device__ __forceinline__ Sub load_sub(const Item& it, int q, int rank) {
-  Sub s;
-  s.t_off = q * 4 * TOK;
-  const int ntok = min(it.ntok - s.t_off, 4 * TOK);
-  s.idx0 = it.idx0 + s.t_off;
-  s.kv_hi = min(s.idx0 + ntok, it.kv_len);
-  s.n = s.kv_hi > it.kv_lo ? (s.kv_hi - it.kv_lo + BN - 1) / BN : 0;
-  s.tb = rank * 2 * TOK;
-  const int mine = min(max(ntok - s.tb, 0), 2 * TOK);
-  s.ntok_a = min(mine, TOK); s.ntok_b = mine - s.ntok_a;
-  s.n_b = ntok > TOK ? s.n : 0;
-  return s;
 }
 
 
@@ -553,7 +536,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
   const uint32_t lbar0 = mapa(bar0, 0);      // the leader's barrier array in the cluster window (== own array for rank 0)
   auto bar = [&](int b) { return bar0 + 8u * (uint32_t)b; };
   auto lbar = [&](int b) { return lbar0 + 8u * (uint32_t)b; };
-  Waiter w{&prm.hdr->err, false, bar0};
+  Waiter w{&prm.hdr->err, false};
 
   if (threadIdx.x >= 64 && threadIdx.x < 128) {
     sm.finc[threadIdx.x - 64] = prm.phase_inc[threadIdx.x - 64];
@@ -563,7 +546,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
   if (threadIdx.x == 0) {
     if (smem_u32(smem_raw) & 1023u) atomicCAS(&prm.hdr->err, 0, 2);   // swizzled tiles need a 1024-byte aligned base
     for (int s = 0; s < kRing; ++s) { mbar_init(bar(SCHED_FULL + s), 1); mbar_init(bar(SCHED_EMPTY + s), 30); }
-    for (int b = 0; b < 2; ++b) { mbar_init(bar(Q_FULL + b), 1); mbar_init(bar(Q_READY + b), 8); mbar_init(bar(Q_EMPTY + b), 8); }
+    mbar_init(bar(Q_FULL), 1); mbar_init(bar(Q_READY), 8); mbar_init(bar(Q_READY + 1), 8); mbar_init(bar(Q_EMPTY), 1);
     for (int s = 0; s < kKStages; ++s) { mbar_init(bar(K_FULL + s), 1); mbar_init(bar(K_READY + s), 8); mbar_init(bar(K_EMPTY + s), 1); }
     for (int s = 0; s < kVStages; ++s) { mbar_init(bar(V_FULL + s), 1); mbar_init(bar(V_PEER + s), 1); mbar_init(bar(V_EMPTY + s), 1); }
     mbar_init(bar(V_FIX), 128);
@@ -601,12 +584,12 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
             ii.t0 = td.t0; ii.ntok = td.ntok; ii.r = td.r; ii.idx0 = td.idx0; ii.lo = td.lo; ii.kvh = item % prm.hkv; ii.n_kv = td.n_kv;
             ii.kv_hi = td.kv_hi; ii.kv_len = td.kv_len; ii.kv_off = td.kv_off;
           }
-          ii.pad[0] = (int)it_n; ii.pad[1] = 0;
+          ii.pad[0] = ii.pad[1] = 0;
           sm.ring[slot] = ii;
           const uint32_t dst = ring_p + (uint32_t)slot * (uint32_t)sizeof(ItemInfo);
           st_cluster_v4(dst, ii.t0, ii.ntok, ii.r, ii.idx0);
           st_cluster_v4(dst + 16, ii.lo, ii.kvh, ii.n_kv, ii.kv_hi);
-          st_cluster_v4(dst + 32, ii.kv_len, ii.kv_off, ii.pad[0], 0);
+          st_cluster_v4(dst + 32, ii.kv_len, ii.kv_off, 0, 0);
           mbar_arrive_cl_release(lbar(SCHED_FULL + slot));
           mbar_arrive_cl_release(full_p + 8u * (uint32_t)slot);
           TRACE(0, 1);
@@ -621,66 +604,59 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         const int slot = it_n & (kRing - 1);
         w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
         if (__any_sync(0xffffffffu, w.dead) || sm.ring[slot].t0 < 0) break;
-        const Item it = load_item<TOK>(sm.ring[slot]);
+        const int n = sm.ring[slot].n_kv, kv_hi = sm.ring[slot].kv_hi;
         __syncwarp();
         if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
-        for (int q = 0; q < it.nsub; ++q) {
-          const Sub sb = load_sub<TOK>(it, q, rank);
-          const bool vfix = (sb.kv_hi & (kBlock - 1)) != 0;
-          for (int i = 0; i < sb.n; ++i, ++vc) {
-            const int st = vc & 1;
-            w.wait(bar(V_FULL + st), (vc >> 1) & 1);
-            if (i == sb.n - 1 && vfix) { w.wait(bar(V_FIX), fixc & 1); ++fixc; }
-            __syncwarp();
-            if (lane == 0) mbar_arrive_cl(lbar(V_PEER + st));
-          }
+        const bool vfix = (kv_hi & (kBlock - 1)) != 0;
+        for (int i = 0; i < n; ++i, ++vc) {
+          const int st = vc % kVStages;
+          w.wait(bar(V_FULL + st), (vc / kVStages) & 1);
+          if (i == n - 1 && vfix) { w.wait(bar(V_FIX), fixc & 1); ++fixc; }
+          __syncwarp();
+          if (lane == 0) mbar_arrive_cl(lbar(V_PEER + st));
         }
       }
     } else if (warp == 12) {
-      // ============================================================ Q / K TMA producer (a4): per sub-item this CTA's Q rows,
-      // then this CTA's 64 keys of every K tile the sub-item is the first to see
-      uint32_t kbase = 0, qn = 0;
+      // ============================================================ Q / K TMA producer (a4): this CTA's 64 keys of every K tile
+      uint32_t kc = 0, qc = 0;
       for (uint32_t it_n = 0;; ++it_n) {
         const int slot = it_n & (kRing - 1);
         w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
         if (__any_sync(0xffffffffu, w.dead) || sm.ring[slot].t0 < 0) break;
-        const Item it = load_item<TOK>(sm.ring[slot]);
-        const int item_kv_hi = sm.ring[slot].kv_hi;
+        const Item it = load_item<TOK>(sm.ring[slot], rank);
         __syncwarp();
         if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
-        const int nblk_total = (item_kv_hi + kBlock - 1) / kBlock;   // blocks [0, nblk_total) of the request hold visible keys
+        if (it.n_kv == 0) continue;
+        const int nblk_total = (it.kv_hi + kBlock - 1) / kBlock;   // blocks [0, nblk_total) of the request hold visible keys
         const int* bt = a.block_tables + (size_t)it.r * a.max_blocks;
         auto block_grp = [&](int i) {   // cache row-group coordinate of this lane's block (lanes 0-3) of KV tile i
           const int b = (it.kv_lo >> 4) + i * (BN / kBlock) + rank * (kKeysCta / kBlock) + lane;
           return (lane < kKeysCta / kBlock && b < nblk_total) ? (__ldg(bt + b) * prm.hkv + it.kvh) * 2 : prm.oob_grp;
         };
-        int n_prev = 0;
-        for (int q = 0; q < it.nsub; ++q, ++qn) {
-          const Sub sb = load_sub<TOK>(it, q, rank);
-          {  // this CTA's Q rows of the sub-item: (token, head-in-group), tile A then tile B
-            const int b = qn & 1;
-            const int ntile = sb.ntok_b > 0 ? 2 : (sb.ntok_a > 0 ? 1 : 0);
-            if (lane == 0) { w.wait(bar(Q_EMPTY + b), ((qn >> 1) & 1) ^ 1); if (!w.dead) mbar_expect_tx(bar(Q_FULL + b), ntile * kTileBytes); }
+        int y = block_grp(0);
+        for (int i = 0; i < it.n_kv; ++i) {
+          const int y_next = (i + 1 < it.n_kv) ? block_grp(i + 1) : 0;
+          {  // K tile i: one 4 KB box per physical block
+            const int st = kc % kKStages;
+            if (lane == 0) { w.wait(bar(K_EMPTY + st), ((kc / kKStages) & 1) ^ 1); if (!w.dead) mbar_expect_tx(bar(K_FULL + st), kKTileBytes); }
             if (__any_sync(0xffffffffu, w.dead)) break;   // a timed-out wait: stop issuing, let the kernel drain
-            if (lane < 2 * ntile) {
-              const int x = lane >> 1, h = lane & 1;
-              tma_load_3d(smem_u32(sm.q[b][x]) + h * kHalfBytes, &tmap_q, bar(Q_FULL + b), 64 * h, it.kvh * G,
-                          it.t0 + sb.t_off + sb.tb + x * TOK);
-            }
-            TRACE_L0(0, 3);
-          }
-          for (int i = n_prev; i < sb.n; ++i) {   // K tile i: one 4 KB box per physical block
-            const uint32_t u = kbase + i;
-            const int st = u & (kKStages - 1);
-            const int y = block_grp(i);
-            if (lane == 0) { w.wait(bar(K_EMPTY + st), ((u / kKStages) & 1) ^ 1); if (!w.dead) mbar_expect_tx(bar(K_FULL + st), kKTileBytes); }
-            if (__any_sync(0xffffffffu, w.dead)) break;
             if (lane < kKeysCta / kBlock) tma_load_4d(smem_u32(sm.k[st]) + lane * 4096, &tmap_k, bar(K_FULL + st), 0, 0, 0, y);
+            ++kc;
             TRACE_L0(0, 2);
           }
-          n_prev = max(n_prev, sb.n);
+          if (i == 0) {  // this CTA's Q rows: (token, head-in-group), tile A then tile B
+            const int ntile = it.ntok_b > 0 ? 2 : (it.ntok_a > 0 ? 1 : 0);
+            if (lane == 0) { w.wait(bar(Q_EMPTY), (qc & 1) ^ 1); if (!w.dead) mbar_expect_tx(bar(Q_FULL), ntile * kTileBytes); }
+            if (__any_sync(0xffffffffu, w.dead)) break;
+            if (lane < 2 * ntile) {
+              const int x = lane >> 1, h = lane & 1;
+              tma_load_3d(smem_u32(sm.q[x]) + h * kHalfBytes, &tmap_q, bar(Q_FULL), 64 * h, it.kvh * G, it.t0 + it.tb + x * TOK);
+            }
+            ++qc;
+            TRACE_L0(0, 3);
+          }
+          y = y_next;
         }
-        kbase += it.n_kv;
       }
     } else if (warp == 14) {
       // ============================================================ V TMA producer (a4): this CTA's half of head_dim, all 128 keys
@@ -689,27 +665,27 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         const int slot = it_n & (kRing - 1);
         w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
         if (__any_sync(0xffffffffu, w.dead) || sm.ring[slot].t0 < 0) break;
-        const Item it = load_item<TOK>(sm.ring[slot]);
+        const ItemInfo ii = sm.ring[slot];
         __syncwarp();
         if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
-        const int* bt = a.block_tables + (size_t)it.r * a.max_blocks;
-        for (int q = 0; q < it.nsub; ++q) {
-          const Sub sb = load_sub<TOK>(it, q, rank);
-          const int nblk_total = (sb.kv_hi + kBlock - 1) / kBlock;
-          auto block_grp = [&](int i) {
-            const int b = (it.kv_lo >> 4) + i * (BN / kBlock) + lane;
-            return (lane < BN / kBlock && b < nblk_total) ? (__ldg(bt + b) * prm.hkv + it.kvh) * 2 : prm.oob_grp;
-          };
-          int y = sb.n > 0 ? block_grp(0) : 0;
-          for (int i = 0; i < sb.n; ++i, ++vc) {
-            const int y_next = (i + 1 < sb.n) ? block_grp(i + 1) : 0;
-            const int st = vc & 1;
-            if (lane == 0) { w.wait(bar(V_EMPTY + st), ((vc >> 1) & 1) ^ 1); if (!w.dead) mbar_expect_tx(bar(V_FULL + st), kVTileBytes); }
-            if (__any_sync(0xffffffffu, w.dead)) break;
-            if (lane < BN / kBlock) tma_load_4d(smem_u32(sm.v[st]) + lane * 2048, &tmap_v, bar(V_FULL + st), 0, 0, rank, y);
-            TRACE_L0(0, 4);
-            y = y_next;
-          }
+        if (ii.n_kv == 0) continue;
+        const int kv_lo = ii.lo & ~(kBlock - 1);
+        const int nblk_total = (ii.kv_hi + kBlock - 1) / kBlock;
+        const int* bt = a.block_tables + (size_t)ii.r * a.max_blocks;
+        auto block_grp = [&](int i) {
+          const int b = (kv_lo >> 4) + i * (BN / kBlock) + lane;
+          return (lane < BN / kBlock && b < nblk_total) ? (__ldg(bt + b) * prm.hkv + ii.kvh) * 2 : prm.oob_grp;
+        };
+        int y = block_grp(0);
+        for (int i = 0; i < ii.n_kv; ++i) {
+          const int y_next = (i + 1 < ii.n_kv) ? block_grp(i + 1) : 0;
+          const int st = vc % kVStages;
+          if (lane == 0) { w.wait(bar(V_EMPTY + st), ((vc / kVStages) & 1) ^ 1); if (!w.dead) mbar_expect_tx(bar(V_FULL + st), kVTileBytes); }
+          if (__any_sync(0xffffffffu, w.dead)) break;
+          if (lane < BN / kBlock) tma_load_4d(smem_u32(sm.v[st]) + lane * 2048, &tmap_v, bar(V_FULL + st), 0, 0, rank, y);
+          ++vc;
+          TRACE_L0(0, 4);
+          y = y_next;
         }
       }
     } else if (warp == 13 && rank == 0) {
@@ -719,234 +695,171 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       // tcgen05.mma / tcgen05.commit for the PAIR.  This role lives in 48 registers: 32-bit descriptor words, running
       // stage / phase counters, no per-stage tables.
       constexpr uint32_t idesc_qk = instr_desc(false), idesc_pv = instr_desc(true);
-      const uint32_t q_lo = ((smem_u32(sm.q[0][0]) >> 4) & 0x3FFF) | (1u << 16);       // + (2 b + x) * 2048
+      const uint32_t q_lo = ((smem_u32(sm.q[0]) >> 4) & 0x3FFF) | (1u << 16);          // + x * 2048
       const uint32_t k_lo = ((smem_u32(sm.k[0]) >> 4) & 0x3FFF) | (1u << 16);          // + stage * 1024
       const uint32_t v_lo = ((smem_u32(sm.v[0]) >> 4) & 0x3FFF) | (1u << 16);          // + stage * 1024
-      uint32_t kbase = 0, vc = 0, qn = 0;
-      uint32_t ph = 0;   // bit 0,1: P_FULL parity of tile A,B; bit 2,3: O_FREE; bit 5: V_FIX
+      uint32_t k_st = 0, k_ph = 0, v_st = 0, v_ph = 0;   // next K / V stage to consume and its full-barrier parity
+      uint32_t ph = 0;   // bit 0,1: P_FULL parity of tile A,B; bit 2,3: O_FREE; bit 4: Q_READY; bit 5: V_FIX
       for (uint32_t it_n = 0;; ++it_n) {
         const int slot = it_n & (kRing - 1);
         w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
         if (__any_sync(0xffffffffu, w.dead) || sm.ring[slot].t0 < 0) break;
-        int nsub, n_kv_item;
-        Item it = load_item<TOK>(sm.ring[slot]);
-        nsub = __shfl_sync(0xffffffffu, it.nsub, 0); n_kv_item = __shfl_sync(0xffffffffu, it.n_kv, 0);
-        it.ntok = __shfl_sync(0xffffffffu, it.ntok, 0); it.idx0 = __shfl_sync(0xffffffffu, it.idx0, 0);
-        it.kv_len = __shfl_sync(0xffffffffu, it.kv_len, 0); it.kv_lo = __shfl_sync(0xffffffffu, it.kv_lo, 0);
+        int n, nx1, kv_hi;
+        {
+          const Item it = load_item<TOK>(sm.ring[slot], 0);
+          n = __shfl_sync(0xffffffffu, it.n_kv, 0);
+          nx1 = __shfl_sync(0xffffffffu, it.n_b, 0); kv_hi = __shfl_sync(0xffffffffu, it.kv_hi, 0);
+        }
+        const bool vfix = (kv_hi & (kBlock - 1)) != 0;
         __syncwarp();
         if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
-#pragma unroll 1
-        for (int q = 0; q < nsub; ++q, ++qn) {
-          const Sub sb = load_sub<TOK>(it, q, 0);
-          const int n = sb.n, nx1 = sb.n_b;
-          const bool vfix = (sb.kv_hi & (kBlock - 1)) != 0, last = q == nsub - 1;
-          const uint32_t qb_lo = q_lo + (qn & 1) * (2 * kTileBytes >> 4);
-          w.dbg = (it_n << 20) | (qn << 8) | (vc & 0xff);
-          w.wait(bar(Q_READY + (qn & 1)), (qn >> 1) & 1);   // both tiles of the sub-item's Q are rotated (one sub-item ahead)
-          if (n == 0) continue;
-          // QK^T of tile x against K tile i (ring use kbase + i): S_x = Q_x K'^T for both CTAs (elected lane only)
-          auto qk = [&](int x, int i) {
-            const uint32_t st = (kbase + i) & (kKStages - 1);
-            const uint32_t a_lo = qb_lo + (uint32_t)x * (kTileBytes >> 4), b_lo = k_lo + st * (kKTileBytes >> 4);
+        if (n == 0) continue;
+        // QK^T of tile x against K stage st: S_x = Q_x K'^T for both CTAs (elected lane only)
+        auto qk = [&](int x, uint32_t st) {
+          const uint32_t a_lo = q_lo + (uint32_t)x * (kTileBytes >> 4), b_lo = k_lo + st * (kKTileBytes >> 4);
 #pragma unroll
-            for (int ks = 0; ks < D / 16; ++ks) {
-              const uint32_t off_q = (ks >> 2) * (kHalfBytes >> 4) + (ks & 3) * 2, off_k = (ks >> 2) * (kKvHalfOff >> 4) + (ks & 3) * 2;
-              umma_ss(tmem + x * BN, a_lo + off_q, b_lo + off_k, idesc_qk, ks > 0);
-            }
-            tc_commit(bar(S_FULL + x));
-            TRACE(1, 10 + x);
-          };
-          auto k_wait = [&](int i) {
-            const uint32_t u = kbase + i;
-            w.wait(bar(K_READY + (u & (kKStages - 1))), (u / kKStages) & 1);
-          };
-          k_wait(0);
-          tc_fence_after();
-          if (elect_one()) {
-            qk(0, 0);
-            if (nx1 > 0) qk(1, 0);
-            if (last) tc_commit(bar(K_EMPTY + (kbase & (kKStages - 1))));
+          for (int ks = 0; ks < D / 16; ++ks) {
+            const uint32_t off_q = (ks >> 2) * (kHalfBytes >> 4) + (ks & 3) * 2, off_k = (ks >> 2) * (kKvHalfOff >> 4) + (ks & 3) * 2;
+            umma_ss(tmem + x * BN, a_lo + off_q, b_lo + off_k, idesc_qk, ks > 0);
           }
-          __syncwarp();
-#pragma unroll 1
-          for (int i = 0; i < n; ++i, ++vc) {
-            const uint32_t v_st = vc & 1;
-            w.dbg = (it_n << 20) | (qn << 8) | (vc & 0xff) | 0x80000000u;
-            w.wait(bar(V_FULL + v_st), (vc >> 1) & 1);
-            w.wait(bar(V_PEER + v_st), (vc >> 1) & 1);
-            if (i == n - 1 && vfix) { w.wait(bar(V_FIX), (ph >> 5) & 1); ph ^= 32u; }
-            bool k_waited = false;
-#pragma unroll 1
-            for (int x = 0; x < 2; ++x) {
-              const int nx = x ? nx1 : n;
-              const bool do_pv = i < nx, do_qk = i + 1 < nx;
-              if (do_pv) {
-                w.wait(bar(P_FULL + x), (ph >> x) & 1); ph ^= 1u << x;
-                if (i == 0) { w.wait(bar(O_FREE + x), ((ph >> (2 + x)) & 1) ^ 1); ph ^= 4u << x; }
-              }
-              tc_fence_after();
-              if (do_pv && elect_one()) {
-                const uint32_t b_lo = v_lo + v_st * (kVTileBytes >> 4);
-#pragma unroll
-                for (int ks = 0; ks < BN / 16; ++ks)
-                  umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, b_lo + ks * (2 * kVGroupBytes >> 4), idesc_pv, (i > 0 || ks > 0));
-                if (i == nx - 1) tc_commit(bar(O_FULL + x));
-                TRACE(1, 20 + x);
-              }
-              __syncwarp();
-              // the next K tile is only needed now: the PV above is already running while this waits on the rotation
-              if (do_qk && !k_waited) { k_wait(i + 1); k_waited = true; tc_fence_after(); }
-              if (elect_one()) {
-                if (x == 1) tc_commit(bar(V_EMPTY + v_st));
-                if (do_qk) qk(x, i + 1);
-                if (x == 1 && i + 1 < n && last) tc_commit(bar(K_EMPTY + ((kbase + i + 1) & (kKStages - 1))));
-              }
-              __syncwarp();
-            }
-          }
+          tc_commit(bar(S_FULL + x));
+          TRACE(1, 10 + x);
+        };
+        w.wait(bar(Q_READY), (ph >> 4) & 1);   // tile A of Q is rotated; tile B follows while QK_A already runs
+        w.wait(bar(K_READY + k_st), k_ph);
+        tc_fence_after();
+        if (elect_one()) qk(0, k_st);
+        __syncwarp();
+        w.wait(bar(Q_READY + 1), (ph >> 4) & 1); ph ^= 16u;
+        tc_fence_after();
+        if (elect_one()) {
+          if (nx1 > 0) qk(1, k_st);
+          tc_commit(bar(K_EMPTY + k_st));
+          if (n == 1) tc_commit(bar(Q_EMPTY));
         }
-        kbase += n_kv_item;
+        __syncwarp();
+        if (++k_st == kKStages) { k_st = 0; k_ph ^= 1; }
+#pragma unroll 1
+        for (int i = 0; i < n; ++i) {
+          w.wait(bar(V_FULL + v_st), v_ph);
+          w.wait(bar(V_PEER + v_st), v_ph);
+          if (i == n - 1 && vfix) { w.wait(bar(V_FIX), (ph >> 5) & 1); ph ^= 32u; }
+          bool k_waited = false;
+#pragma unroll 1
+          for (int x = 0; x < 2; ++x) {
+            const int nx = x ? nx1 : n;
+            const bool do_pv = i < nx, do_qk = i + 1 < nx;
+            if (do_pv) {
+              w.wait(bar(P_FULL + x), (ph >> x) & 1); ph ^= 1u << x;
+              if (i == 0) { w.wait(bar(O_FREE + x), ((ph >> (2 + x)) & 1) ^ 1); ph ^= 4u << x; }
+            }
+            tc_fence_after();
+            if (do_pv && elect_one()) {
+              const uint32_t b_lo = v_lo + v_st * (kVTileBytes >> 4);
+#pragma unroll
+              for (int ks = 0; ks < BN / 16; ++ks)
+                umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, b_lo + ks * (2 * kVGroupBytes >> 4), idesc_pv, (i > 0 || ks > 0));
+              if (i == nx - 1) tc_commit(bar(O_FULL + x));
+              TRACE(1, 20 + x);
+            }
+            __syncwarp();
+            // the next K tile is only needed now: the PV above is already running while this waits on the rotation
+            if (do_qk && !k_waited) { w.wait(bar(K_READY + k_st), k_ph); k_waited = true; tc_fence_after(); }
+            if (elect_one()) {
+              if (x == 1) tc_commit(bar(V_EMPTY + v_st));
+              if (do_qk) qk(x, k_st);
+              if (x == 1 && i + 1 < n) {
+                tc_commit(bar(K_EMPTY + k_st));
+                if (i + 1 == n - 1) tc_commit(bar(Q_EMPTY));
+              }
+            }
+            __syncwarp();
+          }
+          if (++v_st == kVStages) { v_st = 0; v_ph ^= 1; }
+          if (i + 1 < n) { if (++k_st == kKStages) { k_st = 0; k_ph ^= 1; } }
+        }
       }
     }
   } else if (warp >= 8) {
-    // ============================================================ rotation warps (a3, a5): per sub-item, in the order the MMA
-    // issuer needs them, Q (64 of the CTA's 256 rows per warp, rotated one sub-item AHEAD of the softmax warps) and then
-    // this CTA's 64 keys of every K tile the sub-item is the first to see (16 rows per warp)
+    // ============================================================ rotation warps: this CTA's 64 keys of every K tile (a5)
+    // NOTE on code shape: the kernel is instruction-cache bound (four roles with different code share an SM), so only the
+    // per-tile K path is unrolled.  The once-per-item Q rotation (a3) lives in the softmax warps as a rolled loop.
     reg_dec<kRegsRot>();
     const int rw = warp - 8, rot_tid = threadIdx.x - 256;
     const int rsub = lane >> 3, ch = lane & 7;
     Rot8 rot;
-    const uint32_t finc_addr = smem_u32(sm.finc) + 64 * ch, step1_addr = smem_u32(sm.step1) + 64 * ch;
-    const uint32_t step4_addr = smem_u32(sm.step4) + 64 * ch;
+    uint64_t c4[4], s4[4], ns4[4];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+      const float2 u0 = prm.step4[8 * ch + 2 * e], u1 = prm.step4[8 * ch + 2 * e + 1];
+      c4[e] = pk2(u0.x, u1.x); s4[e] = pk2(u0.y, u1.y); ns4[e] = pk2(-u0.y, -u1.y);
+    }
+    const uint32_t finc_addr = smem_u32(sm.finc) + 64 * ch;
     // byte offset of the lane's 16-byte chunk in row (4k + rsub) of a 16-row stretch: even k / odd k (SWIZZLE_128B)
     const uint32_t off_e = (uint32_t)(rsub * 128 + ((ch ^ rsub) << 4));
     const uint32_t off_o = (uint32_t)((4 + rsub) * 128 + ((ch ^ (4 + rsub)) << 4));
-    const bool k_prerot = (prm.flags & MINIPIC_K_PREROTATED) != 0, q_prerot = (prm.flags & MINIPIC_Q_PREROTATED) != 0;
-    constexpr int RW = kKeysCta / 4;   // 16 K tile rows (= 2 row groups) per rotation warp
-    constexpr int NTW = (32 / G) > 0 ? (32 / G) : 1;   // Q tokens in a 32-row chunk
-    auto load_step = [&](uint32_t addr, uint64_t (&cd)[4], uint64_t (&sd)[4], uint64_t (&nsd)[4]) {
-#pragma unroll
-      for (int e = 0; e < 4; ++e) {
-        const uint4 u = lds128(addr + 16 * e);   // (cos, sin) of frequencies 2e, 2e + 1 of this lane
-        cd[e] = pk2(__uint_as_float(u.x), __uint_as_float(u.z));
-        sd[e] = pk2(__uint_as_float(u.y), __uint_as_float(u.w));
-        nsd[e] = pk2(-__uint_as_float(u.y), -__uint_as_float(u.w));
-      }
-    };
-    uint32_t kbase = 0, vc = 0, qn = 0;
+    const bool k_prerot = (prm.flags & MINIPIC_K_PREROTATED) != 0;
+    constexpr int RW = kKeysCta / 4;   // 16 tile rows (= 2 row groups) per rotation warp
+    uint32_t kc = 0, vc = 0;
     for (uint32_t it_n = 0;; ++it_n) {
       const int slot = it_n & (kRing - 1);
       w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
       if (w.dead || sm.ring[slot].t0 < 0) break;
-      const Item it = load_item<TOK>(sm.ring[slot]);
-      const int item_kv_hi = sm.ring[slot].kv_hi;
+      const Item it = load_item<TOK>(sm.ring[slot], rank);
       __syncwarp();
       if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
+      if (it.n_kv == 0) continue;
       const int* pos = a.kv_positions + it.kv_off;
-      int n_prev = 0;
-      for (int q = 0; q < it.nsub; ++q, ++qn) {
-        const Sub sb = load_sub<TOK>(it, q, rank);
-        {
-          // ---- a3: Q rows of the sub-item, in place: row = token * G + head-in-group, the G rows of a token share one
-          //      position.  This warp: tile x = rw / 2, rows [64 (rw & 1), + 64) as two 32-row chunks.  Exact restart at
-          //      the first row of a chunk, one-position steps while the positions are consecutive.
-          const int b = qn & 1, x = rw >> 1;
-          const int ntok_x = sb.ntok_x(x);
-          const int tile_idx0 = sb.idx0 + sb.tb + x * TOK;      // sequence index of the tile's first token
-          int qpx[2];
+      const int jw = it.kv_lo + rank * kKeysCta + RW * rw;   // first key of this warp's rows in tile 0
+      // lane l (< 16) holds the position of key jw + i * 128 + l (fetched one tile early)
+      int myp = __ldg(pos + min(jw + (lane & (RW - 1)), it.kv_len - 1));
+      for (int i = 0; i < it.n_kv; ++i) {
+        const int st = kc % kKStages;
+        const int j0 = jw + i * BN;
+        const int myp_next = (i + 1 < it.n_kv) ? __ldg(pos + min(j0 + BN + (lane & (RW - 1)), it.kv_len - 1)) : 0;
+        const int nrow = it.kv_hi - j0;                   // rows of this warp's chunk that hold visible keys
+        const bool work = !k_prerot && nrow > 0;
+        const int p0 = __shfl_sync(0xffffffffu, myp, 0);
+        // consecutive positions (every workload the paper describes): one exact restart, then 4-position steps
+        const bool contig = __all_sync(0xffffffffu, (lane & (RW - 1)) >= nrow || myp == p0 + (lane & (RW - 1)));
+        if (work && contig) rot.restart(p0 + rsub, finc_addr);          // before the wait: overlaps the TMA latency
+        w.wait(bar(K_FULL + st), (kc / kKStages) & 1);
+        if (rw == 0) TRACE_L0(2, 30);
+        if (work) {
+          const uint32_t kt = smem_u32(sm.k[st]) + (uint32_t)rw * (2 * kGroupBytes);
+          auto row_addr = [&](int k) { return kt + (k >> 1) * kGroupBytes + ((k & 1) ? off_o : off_e); };
+          if (contig) {
+            uint4 lo = lds128(row_addr(0)), hi = lds128(row_addr(0) + kKvHalfOff);
 #pragma unroll
-          for (int c = 0; c < 2; ++c) {
-            const int tk0 = (64 * (rw & 1) + 32 * c) / G;       // first token of the chunk within the tile
-            const int tk = min(tk0 + min(lane, NTW - 1), max(ntok_x - 1, 0));
-            qpx[c] = (!q_prerot && ntok_x > tk0) ? __ldg(pos + min(tile_idx0 + tk, it.kv_len - 1)) : 0;
-          }
-          w.wait(bar(Q_FULL + b), (qn >> 1) & 1);
-          if (!q_prerot) {
-            uint64_t c1[4], s1[4], ns1[4];
-            load_step(step1_addr, c1, s1, ns1);
+            for (int k = 0; k < RW / 4; ++k) {
+              uint4 lo_n = lo, hi_n = hi;
+              if (k < RW / 4 - 1) { lo_n = lds128(row_addr(k + 1)); hi_n = lds128(row_addr(k + 1) + kKvHalfOff); }
+              rot.rotate_store(row_addr(k), kKvHalfOff, lo, hi);
+              if (k < RW / 4 - 1) rot.advance(c4, s4, ns4);
+              lo = lo_n; hi = hi_n;
+            }
+          } else {
 #pragma unroll 1
-            for (int c = 0; c < 2; ++c) {
-              const int row0 = 64 * (rw & 1) + 32 * c;
-              const int ntw = ntok_x - row0 / G;                // tokens of the tile at or after this chunk's first row
-              if (ntw <= 0) break;
-              const uint32_t qt = smem_u32(sm.q[b][x]) + (uint32_t)(row0 / 8) * 1024;
-              int prev = 0;
-#pragma unroll 2
-              for (int k = 0; k < 8; ++k) {
-                if ((4 * k) / G >= ntw) break;
-                const uint32_t addr = qt + (k >> 1) * 1024 + ((k & 1) ? off_o : off_e);
-                const uint4 lo = lds128(addr), hi = lds128(addr + kHalfBytes);
-                const int p = __shfl_sync(0xffffffffu, qpx[c], (row0 % G + 4 * k + rsub) / G);
-                if (k > 0 && p == prev + 1) rot.advance(c1, s1, ns1);
-                else if (k == 0 || p != prev) rot.restart(p, finc_addr);
-                prev = p;
-                rot.rotate_store(addr, kHalfBytes, lo, hi);
-              }
+            for (int k = 0; k < RW / 4; ++k) {
+              if (4 * k >= nrow) break;
+              rot.restart(__shfl_sync(0xffffffffu, myp, 4 * k + rsub), finc_addr);
+              const uint4 lo = lds128(row_addr(k)), hi = lds128(row_addr(k) + kKvHalfOff);
+              rot.rotate_store(row_addr(k), kKvHalfOff, lo, hi);
             }
           }
-          fence_proxy_async();
-          __syncwarp();
-          if (lane == 0) mbar_arrive_cl(lbar(Q_READY + b));
-          if (rw == 0) TRACE_L0(2, 32);
         }
-        // ---- a5: K tiles [n_prev, sb.n) of the item (ring uses kbase + i)
-        if (sb.n > n_prev) {
-          uint64_t c4[4], s4[4], ns4[4];
-          load_step(step4_addr, c4, s4, ns4);
-          const int jw = it.kv_lo + rank * kKeysCta + RW * rw;   // first key of this warp's rows in tile 0
-          // lane l (< 16) holds the position of key jw + i * 128 + l (fetched one tile early)
-          int myp = __ldg(pos + min(jw + n_prev * BN + (lane & (RW - 1)), it.kv_len - 1));
-          for (int i = n_prev; i < sb.n; ++i) {
-            const uint32_t u = kbase + i;
-            const int st = u & (kKStages - 1);
-            const int j0 = jw + i * BN;
-            const int myp_next = (i + 1 < sb.n) ? __ldg(pos + min(j0 + BN + (lane & (RW - 1)), it.kv_len - 1)) : 0;
-            const int nrow = item_kv_hi - j0;                  // rows of this warp's chunk that hold visible keys
-            const bool work = !k_prerot && nrow > 0;
-            const int p0 = __shfl_sync(0xffffffffu, myp, 0);
-            // consecutive positions (every workload the paper describes): one exact restart, then 4-position steps
-            const bool contig = __all_sync(0xffffffffu, (lane & (RW - 1)) >= nrow || myp == p0 + (lane & (RW - 1)));
-            if (work && contig) rot.restart(p0 + rsub, finc_addr);          // before the wait: overlaps the TMA latency
-            w.wait(bar(K_FULL + st), (u / kKStages) & 1);
-            if (rw == 0) TRACE_L0(2, 30);
-            if (work) {
-              const uint32_t kt = smem_u32(sm.k[st]) + (uint32_t)rw * (2 * kGroupBytes);
-              auto row_addr = [&](int k) { return kt + (k >> 1) * kGroupBytes + ((k & 1) ? off_o : off_e); };
-              if (contig) {
-                uint4 lo = lds128(row_addr(0)), hi = lds128(row_addr(0) + kKvHalfOff);
-#pragma unroll
-                for (int k = 0; k < RW / 4; ++k) {
-                  uint4 lo_n = lo, hi_n = hi;
-                  if (k < RW / 4 - 1) { lo_n = lds128(row_addr(k + 1)); hi_n = lds128(row_addr(k + 1) + kKvHalfOff); }
-                  rot.rotate_store(row_addr(k), kKvHalfOff, lo, hi);
-                  if (k < RW / 4 - 1) rot.advance(c4, s4, ns4);
-                  lo = lo_n; hi = hi_n;
-                }
-              } else {
-#pragma unroll 1
-                for (int k = 0; k < RW / 4; ++k) {
-                  if (4 * k >= nrow) break;
-                  rot.restart(__shfl_sync(0xffffffffu, myp, 4 * k + rsub), finc_addr);
-                  const uint4 lo = lds128(row_addr(k)), hi = lds128(row_addr(k) + kKvHalfOff);
-                  rot.rotate_store(row_addr(k), kKvHalfOff, lo, hi);
-                }
-              }
-            }
-            fence_proxy_async();
-            __syncwarp();
-            if (lane == 0) mbar_arrive_cl(lbar(K_READY + st));
-            if (rw == 0) TRACE_L0(2, 31);
-            myp = myp_next;
-          }
-          n_prev = sb.n;
-        }
-        // ---- V: rows at or beyond kv_hi inside the last gathered block of the sub-item's last tile may hold anything
-        //      (never written cache slots); their P is 0, make sure 0 * (those bits) is not NaN
-        if (sb.n > 0 && (sb.kv_hi & (kBlock - 1)) != 0) {
-          const uint32_t uv = vc + sb.n - 1;
-          const int vs = uv & 1;
-          w.wait(bar(V_FULL + vs), (uv >> 1) & 1);
-          const int first = sb.kv_hi - (it.kv_lo + (sb.n - 1) * BN), last = (first + kBlock - 1) & ~(kBlock - 1);
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cl(lbar(K_READY + st));
+        if (rw == 0) TRACE_L0(2, 31);
+        ++kc;
+        myp = myp_next;
+        // ---- V tile i: rows at or beyond kv_hi inside the last gathered block may hold anything (never written
+        //      cache slots); their P is 0, make sure 0 * (those bits) is not NaN
+        if (i == it.n_kv - 1 && (it.kv_hi & (kBlock - 1)) != 0) {
+          const int vs = (vc + i) % kVStages;
+          w.wait(bar(V_FULL + vs), ((vc + i) / kVStages) & 1);
+          const int first = it.kv_hi - (it.kv_lo + i * BN), last = (first + kBlock - 1) & ~(kBlock - 1);
           if (rot_tid >= first && rot_tid < last) {
             const uint32_t vrow = smem_u32(sm.v[vs]) + (rot_tid >> 3) * kVGroupBytes + (rot_tid & 7) * 128;
 #pragma unroll
@@ -955,9 +868,8 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           fence_proxy_async();
           mbar_arrive(bar(V_FIX));
         }
-        vc += sb.n;
       }
-      kbase += it.n_kv;
+      vc += it.n_kv;
     }
   } else {
     // ============================================================ softmax + epilogue warps (a7, a9): thread = row
@@ -967,43 +879,33 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
     const uint32_t t_lane = tmem + ((uint32_t)((warp & 3) * 32) << 16);
     const uint32_t t_s = t_lane + x * BN, t_o = t_lane + (2 + x) * BN;
     const int tok_in = row / G, hg = row % G;
-    uint32_t sc = 0, oc = 0, qn = 0;
-    struct { bool valid; int b, qpar, t0, kvh, ntok_x, n; float l, m; } pe;
+    uint32_t sc = 0, oc = 0, qc = 0;
+    struct { bool valid; int t0, kvh, ntok_x, n; float l, m; } pe;
     pe.valid = false;
     auto epilogue = [&]() {
-      // ---- epilogue (a9) of the PREVIOUS sub-item: O / l -> out, LSE = ln sum exp of the scaled scores.  A thread owns a
-      //      row in TMEM, but a row is 256 B in global memory: the warp transposes 64 columns at a time through its 32 rows
-      //      of the sub-item's own (no longer needed) Q tile so that every store instruction writes full 128-byte lines
+      // ---- epilogue (a9): O / l -> out, LSE = ln sum exp of the scaled scores.  A thread owns a row in TMEM, but a row
+      //      is 256 B in global memory: the warp transposes 64 columns at a time through its 4 KB staging buffer so
+      //      that every store instruction writes four full 128-byte lines instead of 32 scattered 16-byte pieces
       const float inv = pe.l > 0.f ? 1.f / pe.l : 0.f;
-      // A warp whose tile slot is idle (tile B of a short item, n = 0) has nothing to wait for and would run sub-items
-      // ahead of the others: it must not hand the buffer back (Q_EMPTY collects all 8 softmax warps of the CTA) before
-      // the sub-item's Q has even arrived, or it could arrive twice within one phase of the barrier.
-      w.wait(bar(Q_FULL + pe.b), pe.qpar);
       if (pe.n > 0) { w.wait(bar(O_FULL + x), oc & 1); ++oc; tc_fence_after(); }
       if ((warp & 3) == 0) TRACE_L0(3 + x, 42);
-      if (pe.ntok_x <= 0) {   // this CTA owns no row of the tile (the peer does): only release O and the Q buffer
-        if (pe.n > 0) tc_fence_before();
-        __syncwarp();
-        if (lane == 0) {
-          if (pe.n > 0) mbar_arrive_cl(lbar(O_FREE + x));
-          mbar_arrive(bar(Q_EMPTY + pe.b));
-        }
+      if (pe.ntok_x <= 0) {   // this CTA owns no row of the tile (the peer does): only release O
+        if (pe.n > 0) { tc_fence_before(); __syncwarp(); if (lane == 0) mbar_arrive_cl(lbar(O_FREE + x)); }
         return;
       }
       {
-        const uint32_t stg0 = smem_u32(sm.q[pe.b][x]) + (uint32_t)(warp & 3) * 4096;
+        const uint32_t stg = smem_u32(sm.ostage[warp]);
         const int rr = lane >> 3, cc = lane & 7;
         const bool whole = pe.ntok_x == TOK;   // every row of the tile is a real query row: the warp's 32 rows go out
                                                   // as one TMA tensor store per pass (box = 64 columns x G heads x 32/G tokens)
         __nv_bfloat16* obase = (__nv_bfloat16*)a.out + ((size_t)pe.t0 * prm.hq + pe.kvh * G) * D + cc * 8;
 #pragma unroll 1
         for (int pass = 0; pass < 2; ++pass) {
-          const uint32_t stg = stg0 + pass * kHalfBytes;
           float o[64];
           if (pe.n > 0) {
             tmem_ld32(t_o + pass * 64, o); tmem_ld32(t_o + pass * 64 + 32, o + 32);
             tmem_wait_ld();
-            if (pass == 1) {   // O is in registers: the next sub-item may start
+            if (pass == 1) {   // O is in registers: the next item may start
               tc_fence_before(); __syncwarp();
               if (lane == 0) mbar_arrive_cl(lbar(O_FREE + x));
             }
@@ -1011,6 +913,8 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
 #pragma unroll
             for (int e = 0; e < 64; ++e) o[e] = 0.f;
           }
+          if (lane == 0) tma_store_wait_read();   // the previous store out of this staging buffer has been read
+          __syncwarp();
 #pragma unroll
           for (int c = 0; c < 8; ++c) {
             uint4 v;
@@ -1034,12 +938,8 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
               if (rowg / G < pe.ntok_x)
                 *reinterpret_cast<uint4*>(obase + ((size_t)(rowg / G) * prm.hq + rowg % G) * D + pass * 64) = v;
             }
+            __syncwarp();
           }
-        }
-        __syncwarp();
-        if (lane == 0) {
-          tma_store_wait_read();              // the tensor stores have read the staging rows: the Q buffer may be reloaded
-          mbar_arrive(bar(Q_EMPTY + pe.b));
         }
       }
       if ((warp & 3) == 0) TRACE_L0(3 + x, 43);
@@ -1047,116 +947,159 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         a.lse[(size_t)(pe.t0 + tok_in) * prm.hq + pe.kvh * G + hg] =
             pe.l > 0.f ? (pe.m + log2f(pe.l)) * 0.6931471805599453f : -INFINITY;
         };
+    // Q rotation (a3) state of this lane: same row / chunk mapping as the K rotation lanes
+    const int rw = warp & 3, rsub = lane >> 3, ch = lane & 7;
+    const uint32_t finc_addr = smem_u32(sm.finc) + 64 * ch, step1_addr = smem_u32(sm.step1) + 64 * ch;
+    const uint32_t off_e = (uint32_t)(rsub * 128 + ((ch ^ rsub) << 4));
+    const uint32_t off_o = (uint32_t)((4 + rsub) * 128 + ((ch ^ (4 + rsub)) << 4));
+    const bool q_prerot = (prm.flags & MINIPIC_Q_PREROTATED) != 0;
+    constexpr int NTW = (32 / G) > 0 ? (32 / G) : 1;   // Q tokens per warp per tile
     for (uint32_t it_n = 0;; ++it_n) {
       const int slot = it_n & (kRing - 1);
       w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
-      if (w.dead || sm.ring[slot].t0 < 0) break;
-      const Item it = load_item<TOK>(sm.ring[slot]);
+      const bool stop = w.dead || sm.ring[slot].t0 < 0;   // one more trip for the deferred epilogue, then out
+      const Item it = load_item<TOK>(sm.ring[slot], rank);
       __syncwarp();
-      if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
-#pragma unroll 1
-      for (int q = 0; q < it.nsub; ++q, ++qn) {
-        const Sub sb = load_sub<TOK>(it, q, rank);
-        if (pe.valid) epilogue();   // previous sub-item of this tile slot
-        const int n = sb.n_x(x);                  // KV tiles this tile slot runs (the same in both CTAs)
-        const int tile_t = sb.tb + x * TOK;       // first token (within the sub-item) of this CTA's tile x
-        const bool row_ok = tok_in < sb.ntok_x(x);
-        const int idx_first = sb.idx0 + tile_t;                               // lowest query index of this tile
-        const int idx_row = min(sb.idx0 + tile_t + tok_in, it.kv_len - 1);    // highest visible key of this row
-        float m_used = -INFINITY, l_run = 0.f;   // m in log2 units (score * scale * log2 e)
-        for (int i = 0; i < n; ++i, ++sc) {
-          w.dbg = (it_n << 20) | (qn << 8) | (uint32_t)i | (sc << 28);
-          const int j0 = it.kv_lo + i * BN;
-          float s[BN];
-          w.wait(bar(S_FULL + x), sc & 1);
-          if ((warp & 3) == 0) TRACE_L0(3 + x, 40);
-          tc_fence_after();
-#pragma unroll
-          for (int c = 0; c < 4; ++c) tmem_ld32(t_s + c * 32, s + c * 32);
-          tmem_wait_ld();
-          if ((warp & 3) == 0) TRACE_L0(3 + x, 44);
-          // mask at 32-column chunk granularity (all bounds but c_hi are warp-uniform): a chunk that every row of the
-          // tile sees needs no mask code, a chunk no row sees (above the causal diagonal) skips max / exp altogether
-          const int c_lo = it.lo - j0;
-          const int c_hi = row_ok ? idx_row - j0 : -1;
-          const int c_hi_max = min(idx_first + TOK - 1, it.kv_len - 1) - j0;   // highest row of the tile (warp-uniform)
-          if (j0 + BN - 1 > min(idx_first, it.kv_len - 1)) {   // tile reaches past the lowest row's last visible key
-#pragma unroll
-            for (int c = 0; c < BN; ++c) s[c] = (c <= c_hi) ? s[c] : -INFINITY;
-          }
-          if (c_lo > 0) {   // vis_lo inside the first gathered 16-token block (kv_lo = floor16(vis_lo)): c_lo < 16
-#pragma unroll
-            for (int c = 0; c < kBlock; ++c) s[c] = (c >= c_lo) ? s[c] : -INFINITY;
-          }
-          float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
-#pragma unroll
-          for (int c = 0; c < BN; c += 8) {
-            mx0 = max3(mx0, s[c], s[c + 1]); mx1 = max3(mx1, s[c + 2], s[c + 3]);
-            mx2 = max3(mx2, s[c + 4], s[c + 5]); mx3 = max3(mx3, s[c + 6], s[c + 7]);
-          }
-          const float m_new = fmaxf(m_used, fmaxf(max3(mx0, mx1, mx2), mx3) * prm.scale_log2);
-          if ((warp & 3) == 0) TRACE_L0(3 + x, 45);
-          if (i == 0) {
-            m_used = m_new;
-          } else {
-            const bool grow = m_new > m_used + 8.f;   // lazy rescale: P may exceed 1 by up to 2^8 before O, l are rescaled
-            if (__any_sync(0xffffffffu, grow)) {
-              // S_FULL(i) was committed after PV(i-1): O is stable until this thread publishes P(i)
-              const float corr = grow ? fast_exp2(m_used - m_new) : 1.f;
-              if (grow) { l_run *= corr; m_used = m_new; }
-#pragma unroll 1
-              for (int c = 0; c < 8; ++c) {
-                float o[16];
-                tmem_ld16(t_o + c * 16, o);
-                tmem_wait_ld();
-#pragma unroll
-                for (int e = 0; e < 16; ++e) o[e] *= corr;
-                tmem_st16(t_o + c * 16, reinterpret_cast<const uint32_t*>(o));
-              }
-            }
-          }
-          const float m_sub = (m_used == -INFINITY) ? 0.f : m_used;
-          const uint64_t sc2 = pk2(prm.scale_log2, prm.scale_log2), nm2 = pk2(-m_sub, -m_sub);
-          uint64_t lsum0 = pk2(0.f, 0.f), lsum1 = lsum0;
-#pragma unroll
-          for (int h = 0; h < 4; ++h) {
-            uint32_t pk[16];
-            if (32 * h > c_hi_max) {   // keys above the causal diagonal for every row of the tile: P = 0, no exp
-#pragma unroll
-              for (int c = 0; c < 16; ++c) pk[c] = 0u;
-              tmem_st16(t_s + 16 * h, pk);
-              continue;
-            }
-#pragma unroll
-            for (int c = 0; c < 16; ++c) {
-              float x0, x1, p0, p1;
-              upk2(fma2(pk2(s[32 * h + 2 * c], s[32 * h + 2 * c + 1]), sc2, nm2), x0, x1);
-              p0 = fast_exp2(x0); p1 = fast_exp2(x1);
-              if (c & 1) lsum1 = add2(lsum1, pk2(p0, p1)); else lsum0 = add2(lsum0, pk2(p0, p1));
-              pk[c] = pack_bf16(p0, p1);
-            }
-            tmem_st16(t_s + 16 * h, pk);
-          }
-          {
-            float a0, a1;
-            upk2(add2(lsum0, lsum1), a0, a1);
-            l_run += a0 + a1;
-          }
-          if ((warp & 3) == 0) TRACE_L0(3 + x, 46);
-          tmem_wait_st();
-          tc_fence_before();
-          __syncwarp();
-          if (lane == 0) mbar_arrive_cl(lbar(P_FULL + x));
-          if ((warp & 3) == 0) TRACE_L0(3 + x, 41);
+      if (!stop && lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
+      const int n = stop ? 0 : it.n_x(x);      // KV tiles this tile slot runs (the same in both CTAs)
+      const int tile_t = it.tb + x * TOK;      // first token (within the item) of this CTA's tile x
+      if (!stop && it.n_kv > 0) {
+        // ---- a3: rotate this warp's 32 rows of Q tile x in place: row = token * G + head-in-group, the G rows of a token
+        //      share one position.  Exact restart at the first row, one-position steps while the positions are consecutive.
+        //      The eight softmax warps do this (not the four K rotation warps): they would otherwise idle at the item
+        //      boundary while K0, Q_A, Q_B queue up on the rotation warps.  Rolled loop: see the note on code size there.
+        const int ntw = it.ntok_x(x) - (32 * rw) / G;   // tokens of this tile that this warp rotates
+        int qpx = 0;
+        if (!q_prerot && ntw > 0) {
+          const int tk = min((32 * rw) / G + min(lane, NTW - 1), it.ntok_x(x) - 1);
+          qpx = __ldg(a.kv_positions + it.kv_off + min(it.idx0 + tile_t + tk, it.kv_len - 1));
         }
-        // the epilogue of a sub-item is DEFERRED to the start of the next one (the MMA issuer is then already running the
-        // next sub-item's first QK^T); pe = what it needs.  Every sub-item has one: it also hands the Q buffer back.
-        pe.valid = true; pe.b = qn & 1; pe.qpar = (qn >> 1) & 1; pe.t0 = it.t0 + sb.t_off + tile_t; pe.kvh = it.kvh; pe.ntok_x = sb.ntok_x(x); pe.n = n;
-        pe.l = l_run; pe.m = m_used;
+        w.wait(bar(Q_FULL), qc & 1); ++qc;
+        if (!q_prerot && ntw > 0) {
+          Rot8 rot;
+          uint64_t c1[4], s1[4], ns1[4];
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const uint4 u = lds128(step1_addr + 16 * e);   // (cos, sin) of frequencies 2e, 2e + 1 of this lane
+            c1[e] = pk2(__uint_as_float(u.x), __uint_as_float(u.z));
+            s1[e] = pk2(__uint_as_float(u.y), __uint_as_float(u.w));
+            ns1[e] = pk2(-__uint_as_float(u.y), -__uint_as_float(u.w));
+          }
+          const uint32_t qt = smem_u32(sm.q[x]) + (uint32_t)rw * 4096;
+          int prev = 0;
+#pragma unroll 1
+          for (int k = 0; k < 8; ++k) {
+            if ((4 * k) / G >= ntw) break;
+            const uint32_t addr = qt + (k >> 1) * 1024 + ((k & 1) ? off_o : off_e);
+            const uint4 lo = lds128(addr), hi = lds128(addr + kHalfBytes);
+            const int p = __shfl_sync(0xffffffffu, qpx, ((32 * rw) % G + 4 * k + rsub) / G);
+            if (k > 0 && p == prev + 1) rot.advance(c1, s1, ns1);
+            else if (k == 0 || p != prev) rot.restart(p, finc_addr);
+            prev = p;
+            rot.rotate_store(addr, kHalfBytes, lo, hi);
+          }
+        }
+        fence_proxy_async();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cl(lbar(Q_READY + x));
       }
+      if (pe.valid) epilogue();   // previous item of this tile
+      if (stop) break;
+      const bool row_ok = tok_in < it.ntok_x(x);
+      const int idx_first = it.idx0 + tile_t;                               // lowest query index of this tile
+      const int idx_row = min(it.idx0 + tile_t + tok_in, it.kv_len - 1);    // highest visible key of this row
+      float m_used = -INFINITY, l_run = 0.f;   // m in log2 units (score * scale * log2 e)
+      for (int i = 0; i < n; ++i, ++sc) {
+        const int j0 = it.kv_lo + i * BN;
+        float s[BN];
+        w.wait(bar(S_FULL + x), sc & 1);
+        if ((warp & 3) == 0) TRACE_L0(3 + x, 40);
+        tc_fence_after();
+#pragma unroll
+        for (int c = 0; c < 4; ++c) tmem_ld32(t_s + c * 32, s + c * 32);
+        tmem_wait_ld();
+        if ((warp & 3) == 0) TRACE_L0(3 + x, 44);
+        // mask at 32-column chunk granularity (all bounds but c_hi are warp-uniform): a chunk that every row of the
+        // tile sees needs no mask code, a chunk no row sees (above the causal diagonal) skips max / exp altogether
+        const int c_lo = it.lo - j0;
+        const int c_hi = row_ok ? idx_row - j0 : -1;
+        const int c_hi_max = min(idx_first + TOK - 1, it.kv_len - 1) - j0;   // highest row of the tile (warp-uniform)
+        if (j0 + BN - 1 > min(idx_first, it.kv_len - 1)) {   // tile reaches past the lowest row's last visible key
+#pragma unroll
+          for (int c = 0; c < BN; ++c) s[c] = (c <= c_hi) ? s[c] : -INFINITY;
+        }
+        if (c_lo > 0) {   // vis_lo inside the first gathered 16-token block (kv_lo = floor16(vis_lo)): c_lo < 16
+#pragma unroll
+          for (int c = 0; c < kBlock; ++c) s[c] = (c >= c_lo) ? s[c] : -INFINITY;
+        }
+        float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+#pragma unroll
+        for (int c = 0; c < BN; c += 8) {
+          mx0 = max3(mx0, s[c], s[c + 1]); mx1 = max3(mx1, s[c + 2], s[c + 3]);
+          mx2 = max3(mx2, s[c + 4], s[c + 5]); mx3 = max3(mx3, s[c + 6], s[c + 7]);
+        }
+        const float m_new = fmaxf(m_used, fmaxf(max3(mx0, mx1, mx2), mx3) * prm.scale_log2);
+        if ((warp & 3) == 0) TRACE_L0(3 + x, 45);
+        if (i == 0) {
+          m_used = m_new;
+        } else {
+          const bool grow = m_new > m_used + 8.f;   // lazy rescale: P may exceed 1 by up to 2^8 before O, l are rescaled
+          if (__any_sync(0xffffffffu, grow)) {
+            // S_FULL(i) was committed after PV(i-1): O is stable until this thread publishes P(i)
+            const float corr = grow ? fast_exp2(m_used - m_new) : 1.f;
+            if (grow) { l_run *= corr; m_used = m_new; }
+#pragma unroll 1
+            for (int c = 0; c < 8; ++c) {
+              float o[16];
+              tmem_ld16(t_o + c * 16, o);
+              tmem_wait_ld();
+#pragma unroll
+              for (int e = 0; e < 16; ++e) o[e] *= corr;
+              tmem_st16(t_o + c * 16, reinterpret_cast<const uint32_t*>(o));
+            }
+          }
+        }
+        const float m_sub = (m_used == -INFINITY) ? 0.f : m_used;
+        const uint64_t sc2 = pk2(prm.scale_log2, prm.scale_log2), nm2 = pk2(-m_sub, -m_sub);
+        uint64_t lsum0 = pk2(0.f, 0.f), lsum1 = lsum0;
+#pragma unroll
+        for (int h = 0; h < 4; ++h) {
+          uint32_t pk[16];
+          if (32 * h > c_hi_max) {   // keys above the causal diagonal for every row of the tile: P = 0, no exp
+#pragma unroll
+            for (int c = 0; c < 16; ++c) pk[c] = 0u;
+            tmem_st16(t_s + 16 * h, pk);
+            continue;
+          }
+#pragma unroll
+          for (int c = 0; c < 16; ++c) {
+            float x0, x1, p0, p1;
+            upk2(fma2(pk2(s[32 * h + 2 * c], s[32 * h + 2 * c + 1]), sc2, nm2), x0, x1);
+            p0 = fast_exp2(x0); p1 = fast_exp2(x1);
+            if (c & 1) lsum1 = add2(lsum1, pk2(p0, p1)); else lsum0 = add2(lsum0, pk2(p0, p1));
+            pk[c] = pack_bf16(p0, p1);
+          }
+          tmem_st16(t_s + 16 * h, pk);
+        }
+        {
+          float a0, a1;
+          upk2(add2(lsum0, lsum1), a0, a1);
+          l_run += a0 + a1;
+        }
+        if ((warp & 3) == 0) TRACE_L0(3 + x, 46);
+        tmem_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cl(lbar(P_FULL + x));
+        if ((warp & 3) == 0) TRACE_L0(3 + x, 41);
+      }
+      // the epilogue of an item is DEFERRED until this tile's Q rows of the next item are rotated (below), so that QK of the
+      // next item starts ~3 K cycles earlier; pe = what it needs.  A tile slot that ran KV tiles for the peer's rows only
+      // (ntok_x = 0, n > 0) still has to consume O_FULL and release O.
+      pe.valid = it.ntok_x(x) > 0 || n > 0; pe.t0 = it.t0 + tile_t; pe.kvh = it.kvh; pe.ntok_x = it.ntok_x(x); pe.n = n;
+      pe.l = l_run; pe.m = m_used;
     }
-    if (pe.valid) epilogue();
-    if (lane == 0) tma_store_wait_all();   // the staging rows must outlive the last tensor stores
+    if (lane == 0) tma_store_wait_all();   // the staging buffers must outlive the last tensor stores
   }
   tc_fence_before();
   cluster_sync_all();   // no CTA may exit (or free TMEM) while its peer can still arrive on its barriers / run MMAs on it
@@ -1281,18 +1224,12 @@ bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
   PlanHeader* hdr = (PlanHeader*)a.workspace;
   TileDesc* sorted = (TileDesc*)((char*)a.workspace + sizeof(PlanHeader));
   TileDesc* tmp = sorted + (a.num_q_tokens + 1);
-  const int t4 = 4 * BM / c.group;   // query tokens per sub-item: two 128-row tiles in each CTA of a pair
-  // resident items (several sub-items over K tiles rotated once) trade parallelism for less K work: allow them only when
-  // there are enough query tokens to keep every CTA pair busy with items of that size
-  const int pairs = max(current_sm_count() / 2, 1);
-  int cap = t4;
-  while (cap * 2 <= kResKeys && (long long)a.num_q_tokens * c.hkv >= 4LL * pairs * (cap * 2)) cap *= 2;
-  if (const char* e = getenv("MINIPIC_DEBUG_CAP")) cap = max(t4, min(atoi(e) / t4 * t4, kResKeys));
+  const int tok2 = 4 * BM / c.group;   // query tokens per work item: two 128-row tiles in each CTA of a pair
   if (cudaMemsetAsync(hdr, 0, sizeof(PlanHeader), c.stream) != cudaSuccess) return false;
-  plan_mark_kernel<<<(a.num_q_tokens + 255) / 256, 256, 0, c.stream>>>(a, t4, cap, hdr, tmp);
-  plan_scan_kernel<<<1, 1024, 0, c.stream>>>(hdr);
-  plan_scatter_kernel<<<(a.num_q_tokens + 255) / 256, 256, 0, c.stream>>>(hdr, tmp, sorted);
-  note_launch(3);
+  if (a.num_q_tokens > 0) {
+    plan_kernel<<<(a.num_q_tokens + kPlanThreads - 1) / kPlanThreads, kPlanThreads, 0, c.stream>>>(a, tok2, hdr, tmp, sorted);
+    note_launch(1);
+  }
   Params prm;
   prm.a = a; prm.hq = c.hq; prm.hkv = c.hkv; prm.scale_log2 = c.scale_log2; prm.flags = c.flags;
   prm.hdr = hdr; prm.tiles = sorted;
