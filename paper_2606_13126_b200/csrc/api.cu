@@ -229,7 +229,7 @@ int minipic_decode_attention(const minipic_config* cfg, const void* q, const voi
                num_seqs, max_kv_len, out, lse, workspace, workspace_bytes};
   if (!(c.flags & MINIPIC_FORCE_SIMT) && decode_mma_supported(c)) {
     g_variant = "decode_mma";
-    launch_decode_mma(c, a, sp, o_part, lse_part);
+    if (!launch_decode_mma(c, a, sp, o_part, lse_part)) return MINIPIC_ERR_CUDA;
   } else {
     g_variant = "decode_simt";
     launch_decode_simt(c, a, sp, o_part, lse_part);

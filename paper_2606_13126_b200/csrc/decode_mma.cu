@@ -1,24 +1,27 @@
 // a10: split-KV decode partial kernel (bf16, head_dim 128, GQA group <= 8), HBM-bound.
 //
-// One warp owns one (sequence, KV head, split): it streams the split's 16-token blocks straight from the paged
-// cache into registers with coalesced 16-byte loads (every 32-byte sector it touches is fully used), rotates K in
-// registers at the request's logical positions (Eq. 2), and runs both contractions on the
-// register-operand tensor path (mma.sync m16n8k16, bf16 x bf16 -> fp32) so that the CUDA cores are left for the
-// bf16->fp32 conversion and the two FMAs per K element.  The G query heads of the group share the
-// rotated K tile.  Online softmax uses warp shuffles across the 4 lanes that hold one head's scores.
-// Partials (o_s normalised over the split, lse_s) go to the workspace; lse_merge_kernel (a11) combines them.
-// The W warps of a CTA are W KV heads of the SAME (sequence, split): they share the (cos, sin) tile of every 16-key block
-// through a small shared-memory ring instead of each recomputing it (see "cos/sin ring" below).
+// One warp owns one (sequence, KV head, split).  It is its own producer and consumer: lane 0 keeps a ring of kStages
+// 16-token blocks in flight with cp.async.bulk.tensor (one 4 KB box of K and one of V per physical block, looked up in the
+// block table; SWIZZLE_128B, so the fragment reads below are bank-conflict free), the whole warp then rotates K in
+// registers at the request's logical positions (Eq. 2) and runs both contractions on the register-operand
+// tensor path (mma.sync m16n8k16, bf16 x bf16 -> fp32), so the CUDA cores are left for the bf16->fp32 conversion and the two
+// FMAs per K element.  Staging through shared memory (instead of streaming straight into registers, the
+// round-1 kernel) takes the HBM latency off the warp's critical path: with the loads decoupled the rotation's ~500 extra
+// instructions per block overlap the stream instead of adding to it.  The G query heads of the group share the rotated K
+// tile.  Online softmax uses warp shuffles across the 4 lanes that hold one head's scores.  Partials (o_s normalised over
+// the split, lse_s) go to the workspace; lse_merge_kernel (a11) combines them.
 //
 // Fragment trick: the dot products are sums over head_dim (QK^T) and over keys (PV), so any permutation of the
 // summation index is legal as long as both operands use it.  That lets each lane feed the MMA fragments from
 // whole 16-byte vectors:
 //   QK^T as S^T[head, key] = Q'[head, d] K'^T[d, key]:  A = Q' (row g = head), B = K' (col g = key), and the lane
-//     (g, q) loads for key rows g and g+8 the 16-byte chunks q, q+4, q+8, q+12 - chunk c and c+8 hold the two
-//     halves of the rotate-half pairs, so the rotation is lane-local.
+//     (g, q) reads for key rows g and g+8 the 16-byte chunks 2q, 2q+1 of both halves of head_dim - chunk c of the low half
+//     and chunk c of the high half hold the two elements of the rotate-half pairs, so the rotation is lane-local.
 //   PV as O^T[d, head] = V^T[d, key] P[key, head]:  the S^T accumulator layout IS the B-fragment layout of P; the
-//     lane loads chunk g (and g+8) of V rows 2q, 2q+1, 2q+8, 2q+9 and two byte-permutes per register pair build
+//     lane reads chunk g of both halves of V rows 2q, 2q+1, 2q+8, 2q+9 and two byte-permutes per register pair build
 //     the A fragments.
+#include <cuda.h>
+
 #include "internal.h"
 
 namespace minipic {
@@ -62,24 +65,16 @@ __device__ __forceinline__ void rotate_chunks(uint4& lo, uint4& hi, const float 
   }
 }
 
-// ---- cos/sin ring shared by the warps (KV heads) of a CTA ------------------------------------------------------------
-// The warps of a CTA work on the SAME 16 key positions of the same (sequence, split); only the KV head differs.  The
-// (cos, sin) tile of a block - 16 positions x 64 frequencies - is therefore computed ONCE per CTA: every warp computes 1/W
-// of it for the block kLook iterations ahead (8 * 4/W exact evaluations per lane instead of 32), stores it to a ring of
-// kSlots tiles in shared memory, and picks up its own 32 pairs with 16 LDS.128.  Hand-off is two mbarriers per slot
-// (full / empty, one arrival per warp), so the warps stay loosely coupled (up to kLook blocks of skew) instead of running
-// in lock step.  Tile layout: row r (512 B) x 8 chunks of 8 frequencies (64 B) x 4 pieces of 16 B = (c0, c1, s0, s1) of two
-// neighbouring frequencies - the operand order of the packed f32x2 rotation; the piece index is XOR-swizzled with
-// ((r & 1) << 1 | (chunk >> 1) & 1) so that both the writers' and the readers' quarter-warps touch 32 distinct banks.
-constexpr int kSlots = 4, kLook = 2, kCsTileBytes = kBlock * 512;
+constexpr int kStages = MINIPIC_DECODE_STAGES;   // blocks in flight per warp (internal.h)
+constexpr int kStageBytes = 8192;                // K block (4 KB) | V block (4 KB) of one KV head
 constexpr unsigned kSpinLimit = 1u << 26;
 
 __device__ __forceinline__ uint32_t smem_addr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
 }
-__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
-  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
   unsigned spins = 0;
@@ -94,37 +89,32 @@ __device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
     if (++spins > kSpinLimit) __trap();   // a protocol bug must fail loudly instead of hanging the GPU
   }
 }
+__device__ __forceinline__ void tma_block(uint32_t dst, const CUtensorMap* tmap, uint32_t bar, int grp) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%3, %3, %3, %4}], [%2];"
+      ::"r"(dst), "l"(tmap), "r"(bar), "r"(0), "r"(grp) : "memory");
+}
 __device__ __forceinline__ uint4 lds128(uint32_t addr) {
   uint4 v;
   asm volatile("ld.shared.v4.b32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr) : "memory");
   return v;
 }
-__device__ __forceinline__ void sts128(uint32_t addr, float a, float b, float c, float d) {
-  asm volatile("st.shared.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
-}
-// rotate word w of a (lo, hi) chunk pair with the piece (c0, c1, s0, s1): packed f32x2 math, one RN to bf16
-__device__ __forceinline__ void rotate_word(unsigned& l, unsigned& h, const uint4& cs) {
-  const uint64_t a = pk2(bf16lo(l), bf16hi(l)), b = pk2(bf16lo(h), bf16hi(h));
-  const uint64_t c = ((uint64_t)cs.y << 32) | cs.x, s = ((uint64_t)cs.w << 32) | cs.z;
-  const uint64_t ns = mul2(s, pk2(-1.f, -1.f));
-  float x0, x1, y0, y1;
-  upk2(fma2(b, ns, mul2(a, c)), x0, x1);
-  upk2(fma2(a, s, mul2(b, c)), y0, y1);
-  l = pack_bf16(x0, x1);
-  h = pack_bf16(y0, y1);
-}
 
 template <bool kRotK, int W>
-__global__ void __launch_bounds__(32 * W, 16 / W)   // 16 warps / SM; 4-warp CTAs measured 6 % faster than 8-warp CTAs
-decode_mma_kernel(DecodeArgs a, int hq, int hkv, int group, float scale_log2, RopeParams rp, unsigned flags,
-                  int split_len, int max_splits, float* __restrict__ o_part, float* __restrict__ lse_part) {
+__global__ void __launch_bounds__(32 * W, MINIPIC_DECODE_WARPS_PER_SM / W)
+decode_mma_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v, DecodeArgs a,
+                  int hq, int hkv, int group, float scale_log2, RopeParams rp, unsigned flags, int split_len,
+                  int max_splits, float* __restrict__ o_part, float* __restrict__ lse_part) {
   constexpr int D = 128;
-  __shared__ unsigned long long finc[64];  // F_i: 64-bit fixed-point phase increments (turns per position)
-  __shared__ __align__(128) unsigned char cs_ring[kRotK ? kSlots * kCsTileBytes : 16];
-  __shared__ unsigned long long bars[2 * kSlots];
+  // dynamic shared memory only (the swizzled block images need a 1024-byte aligned base):
+  // [W warps][kStages][K 4 KB | V 4 KB] | F_i[64] | barriers[W * kStages]
+  extern __shared__ __align__(1024) unsigned char smem_raw[];
+  unsigned long long* finc = reinterpret_cast<unsigned long long*>(smem_raw + W * kStages * kStageBytes);  // 64-bit phase increments
+  unsigned long long* bars = finc + 64;
   for (int i = threadIdx.x; i < 64; i += 32 * W) finc[i] = rp.phase_inc[i];
-  if (kRotK && threadIdx.x == 0) {
-    for (int i = 0; i < 2 * kSlots; ++i) mbar_init(smem_addr(&bars[i]), W);
+  if (threadIdx.x == 0) {
+    if (smem_addr(smem_raw) & 1023u) __trap();
+    for (int i = 0; i < W * kStages; ++i) mbar_init(smem_addr(&bars[i]), 1);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -138,23 +128,22 @@ decode_mma_kernel(DecodeArgs a, int hq, int hkv, int group, float scale_log2, Ro
   const int j_begin = max(vis_lo, s * split_len), j_end = min(kv_len, (s + 1) * split_len);
   const int* __restrict__ pos = a.kv_positions + __ldg(a.cu_kv_lens + r);
   const int* __restrict__ bt = a.block_tables + (size_t)r * a.max_blocks;
-  const __nv_bfloat16* __restrict__ kc = (const __nv_bfloat16*)a.k_cache;
-  const __nv_bfloat16* __restrict__ vc = (const __nv_bfloat16*)a.v_cache;
 
-  // ---- Q' fragments (a3): head g of the group, chunks q4 + 4j, rotated at the query's logical position
+  // this lane's 16-byte chunks of a row: j = 0, 1 -> chunks 2 q4 + j of the low half, j = 2, 3 -> the same of the high half
+  // ---- Q' fragments (a3): head g of the group, rotated at the query's logical position
   unsigned qf[8][2];
   {
     uint4 ch[4];
     if (g < group) {
       const __nv_bfloat16* qrow = (const __nv_bfloat16*)a.q + ((size_t)r * hq + (size_t)kvh * group + g) * D;
 #pragma unroll
-      for (int j = 0; j < 4; ++j) ch[j] = __ldg(reinterpret_cast<const uint4*>(qrow + (q4 + 4 * j) * 8));
+      for (int j = 0; j < 4; ++j) ch[j] = __ldg(reinterpret_cast<const uint4*>(qrow + (2 * q4 + (j & 1) + 8 * (j >> 1)) * 8));
       if (!(flags & MINIPIC_Q_PREROTATED)) {
         const int qpos = __ldg(pos + kv_len - 1);
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
           float c[8], sn[8];
-          rope_cs8(finc, qpos, (q4 + 4 * j) * 8, c, sn);
+          rope_cs8(finc, qpos, (2 * q4 + j) * 8, c, sn);
           rotate_chunks(ch[j], ch[j + 2], c, sn);
         }
       }
@@ -174,67 +163,64 @@ decode_mma_kernel(DecodeArgs a, int hq, int hkv, int group, float scale_log2, Ro
   for (int i = 0; i < 8; ++i) { o[i][0] = o[i][1] = o[i][2] = o[i][3] = 0.f; }
   float m_run = -INFINITY, l_run = 0.f;
 
-  const int kb0 = j_begin / kBlock, kb1 = (j_end + kBlock - 1) / kBlock;
-
-  // ---- this lane's share of a (cos, sin) tile: rows prow0 + 4 i (i < 4 / W), frequency chunk pc
-  const int pc = (lane & 3) + 4 * ((lane >> 3) & 1);
-  const int prow0 = warp * (kBlock / W) + ((lane >> 2) & 1) + 2 * (lane >> 4);
-  const uint32_t ring0 = smem_addr(cs_ring), bar0 = smem_addr(bars);
-  const uint32_t psw = (uint32_t)((((lane >> 2) & 1) << 1) | ((pc >> 1) & 1));   // row parity of prow0 + 4 i = (lane >> 2) & 1
-  const uint32_t rsw = (uint32_t)(((g & 1) << 1) | (q4 >> 1));                   // reader: rows g, g + 8, chunks q4, q4 + 4
-  auto produce = [&](int n) {   // tile of block kb0 + n -> slot n % kSlots
-    const int slot = n % kSlots, kb = kb0 + n;
-    if (n >= kSlots) mbar_wait(bar0 + 8u * (kSlots + slot), ((n / kSlots) & 1) ^ 1);   // every warp is done with block n - kSlots
-    const uint32_t tile = ring0 + slot * kCsTileBytes;
-#pragma unroll
-    for (int i = 0; i < 4 / W; ++i) {
-      const int row = prow0 + 4 * i;
-      const int p = __ldg(pos + min(kb * kBlock + row, kv_len - 1));
-      float c[8], sn[8];
-      rope_cs8(finc, p, pc * 8, c, sn);
-      const uint32_t base = tile + row * 512 + pc * 64;
-#pragma unroll
-      for (int k = 0; k < 4; ++k) sts128(base + ((k ^ psw) << 4), c[2 * k], c[2 * k + 1], sn[2 * k], sn[2 * k + 1]);
-    }
-    __syncwarp();
-    if (lane == 0) mbar_arrive(bar0 + 8u * slot);
+  const int kb0 = j_begin / kBlock, kb1 = (j_end + kBlock - 1) / kBlock, nb = kb1 - kb0;
+  const uint32_t ring = smem_addr(smem_raw) + (uint32_t)warp * (kStages * kStageBytes);
+  const uint32_t bar0 = smem_addr(&bars[warp * kStages]);
+  // a4: block n of the split -> stage n % kStages (lane 0 only): one 4 KB box of K and one of V through the block table
+  auto issue = [&](int n) {
+    const int st = n % kStages;
+    const int grp = (__ldg(bt + kb0 + n) * hkv + kvh) * 2;   // row-group coordinate of (block, head) in the cache tensor map
+    mbar_expect_tx(bar0 + 8u * st, kStageBytes);
+    tma_block(ring + st * kStageBytes, &tmap_k, bar0 + 8u * st, grp);
+    tma_block(ring + st * kStageBytes + 4096, &tmap_v, bar0 + 8u * st, grp);
   };
-  if (kRotK) {
-#pragma unroll 1
-    for (int n = 0; n < kLook && kb0 + n < kb1; ++n) produce(n);
+  if (lane == 0)
+    for (int n = 0; n < kStages - 1 && n < nb; ++n) issue(n);
+
+  // swizzled offsets of this lane's chunks inside a 4 KB block image: [row group (2)][half (2)][8 rows x 128 B], SWIZZLE_128B
+  uint32_t koff[2];   // K rows g (group 0) and g + 8 (group 1) share the in-group offset: chunk 2 q4 + j of row g
+#pragma unroll
+  for (int j = 0; j < 2; ++j) koff[j] = (uint32_t)(g * 128 + (((2 * q4 + j) ^ g) << 4));
+  uint32_t voff[4];   // V rows 2 q4 + (i & 1) + 8 (i >> 1), chunk g
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const int row = 2 * q4 + (i & 1);
+    voff[i] = (uint32_t)((i >> 1) * 2048 + row * 128 + ((g ^ row) << 4));
   }
 
-  int blk = __ldg(bt + kb0);
 #pragma unroll 1
-  for (int kb = kb0; kb < kb1; ++kb) {
-    const int n = kb - kb0;
-    const size_t base = ((size_t)blk * hkv + kvh) * (kBlock * D);
-    if (kb + 1 < kb1) blk = __ldg(bt + kb + 1);
-    // ---- a4: K rows g and g+8, chunks q4 + 4j: 8 x 16-byte streaming loads
+  for (int n = 0; n < nb; ++n) {
+    const int kb = kb0 + n;
+    // every lane is done with the stage that block n + kStages - 1 reuses (it held block n - 1): refill it
+    __syncwarp();
+    if (lane == 0 && n + kStages - 1 < nb) issue(n + kStages - 1);
+    // a5 (first half): cos/sin of this lane's two rows, computed while the block is still in flight
+    float cs[2][2][8], sn[2][2][8];
+    // Measured and dropped: row g + 8 from row g by one angle-addition step with a (cos 8 f, sin 8 f) table in shared
+    // memory (-72 instructions per block): 1.14 -> 1.43 ms.  The loop is bound by dependent latency at 3 warps per
+    // scheduler, not by issue slots, and the second row's cos/sin then wait for the first row's MUFU results.
+    if (kRotK) {
+#pragma unroll
+      for (int t = 0; t < 2; ++t) {
+        const int p = __ldg(pos + min(kb * kBlock + g + 8 * t, kv_len - 1));
+#pragma unroll
+        for (int j = 0; j < 2; ++j) rope_cs8(finc, p, (2 * q4 + j) * 8, cs[t][j], sn[t][j]);
+      }
+    }
+    const uint32_t stg = ring + (n % kStages) * kStageBytes;
+    mbar_wait(bar0 + 8u * (n % kStages), (n / kStages) & 1);
+    // ---- K rows g and g+8: 8 x 16-byte conflict-free shared loads
     uint4 kr[2][4];
 #pragma unroll
     for (int t = 0; t < 2; ++t)
 #pragma unroll
-      for (int j = 0; j < 4; ++j) kr[t][j] = ldg_stream16(kc + base + (g + 8 * t) * D + (q4 + 4 * j) * 8);
-    // ---- a5: rotate in registers at pi_r(j); cos/sin from the CTA's shared tile (this warp's share of the tile kLook
-    //      blocks ahead is computed first, under the latency of the loads above)
+      for (int j = 0; j < 4; ++j) kr[t][j] = lds128(stg + t * 2048 + (j >> 1) * 1024 + koff[j & 1]);
+    // ---- a5: rotate in registers at pi_r(j)
     if (kRotK) {
-      if (kb + kLook < kb1) produce(n + kLook);
-      const int slot = n % kSlots;
-      mbar_wait(bar0 + 8u * slot, (n / kSlots) & 1);
-      const uint32_t tile = ring0 + slot * kCsTileBytes;
 #pragma unroll
       for (int t = 0; t < 2; ++t)
 #pragma unroll
-        for (int j = 0; j < 2; ++j) {
-          const uint32_t src = tile + (g + 8 * t) * 512 + (q4 + 4 * j) * 64;
-          unsigned* l = reinterpret_cast<unsigned*>(&kr[t][j]);
-          unsigned* h = reinterpret_cast<unsigned*>(&kr[t][j + 2]);
-#pragma unroll
-          for (int k = 0; k < 4; ++k) rotate_word(l[k], h[k], lds128(src + ((k ^ rsw) << 4)));
-        }
-      __syncwarp();
-      if (lane == 0) mbar_arrive(bar0 + 8u * (kSlots + slot));   // this warp no longer needs the tile
+        for (int j = 0; j < 2; ++j) rotate_chunks(kr[t][j], kr[t][j + 2], cs[t][j], sn[t][j]);
     }
     // ---- a6: S^T[head, key] for the two 8-key halves of the block
     float st[2][4];
@@ -247,16 +233,17 @@ decode_mma_kernel(DecodeArgs a, int hq, int hkv, int group, float scale_log2, Ro
         mma16816(st[t], qf[2 * j + 1][0], 0u, qf[2 * j + 1][1], 0u, kr[t][j].z, kr[t][j].w);
       }
     }
-    // ---- V rows 2q, 2q+1, 2q+8, 2q+9, chunks g and g+8 (issued now, consumed after the softmax)
+    // ---- V rows 2q, 2q+1, 2q+8, 2q+9, chunk g of both halves
     uint4 vr[4][2];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      const int row = 2 * q4 + (i & 1) + 8 * (i >> 1);
-      const int jrow = kb * kBlock + row;
+      const int jrow = kb * kBlock + 2 * q4 + (i & 1) + 8 * (i >> 1);
       const bool ok = jrow >= j_begin && jrow < j_end;  // never multiply P = 0 with uninitialised cache bits
 #pragma unroll
-      for (int hf = 0; hf < 2; ++hf)
-        vr[i][hf] = ok ? ldg_stream16(vc + base + row * D + (g + 8 * hf) * 8) : make_uint4(0, 0, 0, 0);
+      for (int hf = 0; hf < 2; ++hf) {
+        const uint4 v = lds128(stg + 4096 + hf * 1024 + voff[i]);
+        vr[i][hf] = ok ? v : make_uint4(0, 0, 0, 0);
+      }
     }
     // ---- a7: mask + online softmax (row = head g; its 16 scores live in 4 lanes x 4 registers)
     float sc[2][2];
@@ -328,28 +315,50 @@ decode_mma_kernel(DecodeArgs a, int hq, int hkv, int group, float scale_log2, Ro
   }
 }
 
-template <int W>
-void launch_w(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, float* o_part, float* lse_part) {
+template <bool kRotK, int W>
+bool launch_k(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, const CUtensorMap& mk, const CUtensorMap& mv,
+              float* o_part, float* lse_part) {
+  const size_t smem = (size_t)W * kStages * kStageBytes + 64 * 8 + (size_t)W * kStages * 8;
+  static bool attr_done[64] = {};   // per (function, device)
+  int dev = 0;
+  cudaGetDevice(&dev);
+  if (dev < 0 || dev >= 64 || !attr_done[dev]) {
+    if (cudaFuncSetAttribute(decode_mma_kernel<kRotK, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+      note_error("decode_mma: cudaFuncSetAttribute(MaxDynamicSharedMemorySize) failed");
+      return false;
+    }
+    if (dev >= 0 && dev < 64) attr_done[dev] = true;
+  }
   dim3 grid((unsigned)sp.max_splits * (unsigned)a.num_seqs, c.hkv / W);
-  if (c.flags & MINIPIC_K_PREROTATED)
-    decode_mma_kernel<false, W><<<grid, 32 * W, 0, c.stream>>>(a, c.hq, c.hkv, c.group, c.scale_log2, c.rope, c.flags,
-                                                               sp.split_len, sp.max_splits, o_part, lse_part);
-  else
-    decode_mma_kernel<true, W><<<grid, 32 * W, 0, c.stream>>>(a, c.hq, c.hkv, c.group, c.scale_log2, c.rope, c.flags,
-                                                              sp.split_len, sp.max_splits, o_part, lse_part);
+  decode_mma_kernel<kRotK, W><<<grid, 32 * W, smem, c.stream>>>(mk, mv, a, c.hq, c.hkv, c.group, c.scale_log2, c.rope,
+                                                               c.flags, sp.split_len, sp.max_splits, o_part, lse_part);
+  return true;
+}
+template <int W>
+bool launch_w(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, const CUtensorMap& mk, const CUtensorMap& mv,
+              float* o_part, float* lse_part) {
+  return (c.flags & MINIPIC_K_PREROTATED) ? launch_k<false, W>(c, a, sp, mk, mv, o_part, lse_part)
+                                          : launch_k<true, W>(c, a, sp, mk, mv, o_part, lse_part);
 }
 
 }  // namespace
 
 bool decode_mma_supported(const Ctx& c) { return c.dtype == MINIPIC_BF16 && c.d == 128 && c.group <= 8; }
 
-void launch_decode_mma(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, float* o_part, float* lse_part) {
-  if (a.num_seqs == 0) return;
-  // W warps = W KV heads of one (sequence, split) per CTA; they share the (cos, sin) tiles through shared memory
-  if (c.hkv % 4 == 0) launch_w<4>(c, a, sp, o_part, lse_part);
-  else if (c.hkv % 2 == 0) launch_w<2>(c, a, sp, o_part, lse_part);
-  else launch_w<1>(c, a, sp, o_part, lse_part);
-  note_launch();
+bool launch_decode_mma(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, float* o_part, float* lse_part) {
+  if (a.num_seqs == 0) return true;
+  CUtensorMap mk, mv;
+  if (!make_cache_tensor_map(&mk, a.k_cache, c.num_blocks, c.hkv, 2) || !make_cache_tensor_map(&mv, a.v_cache, c.num_blocks, c.hkv, 2)) {
+    note_error("decode_mma: cuTensorMapEncodeTiled failed (driver entry point missing or bad tensor geometry)");
+    return false;
+  }
+  // W warps = W KV heads of one (sequence, split) per CTA
+  bool ok;
+  if (c.hkv % 4 == 0) ok = launch_w<4>(c, a, sp, mk, mv, o_part, lse_part);
+  else if (c.hkv % 2 == 0) ok = launch_w<2>(c, a, sp, mk, mv, o_part, lse_part);
+  else ok = launch_w<1>(c, a, sp, mk, mv, o_part, lse_part);
+  if (ok) note_launch();
+  return ok;
 }
 
 }  // namespace minipic

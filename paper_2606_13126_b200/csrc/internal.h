@@ -1,6 +1,16 @@
 // Launcher declarations shared by the translation units of libminipic.so.
 #pragma once
+#include <cuda.h>
+
 #include "common.cuh"
+
+// decode (a10) launch shape: blocks in flight per warp and resident warps per SM (kStages * 8 KB of shared memory per warp)
+#ifndef MINIPIC_DECODE_STAGES
+#define MINIPIC_DECODE_STAGES 2
+#endif
+#ifndef MINIPIC_DECODE_WARPS_PER_SM
+#define MINIPIC_DECODE_WARPS_PER_SM 12
+#endif
 
 namespace minipic {
 
@@ -40,7 +50,10 @@ void launch_decode_simt(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, 
 void launch_lse_merge(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, const float* o_part, const float* lse_part);
 // a10 tensor-core (mma.sync, register operands) split-KV kernel: bf16, D=128, G<=8
 bool decode_mma_supported(const Ctx& c);
-void launch_decode_mma(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, float* o_part, float* lse_part);
+bool launch_decode_mma(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, float* o_part, float* lse_part);
+// the paged cache as a 4-D bf16 tensor map whose box is one (block, head): 16 tokens x 128 dims land as
+// [row group (2)][half of head_dim (halves)][8 rows x 128 B], SWIZZLE_128B (defined in prefill_sm100.cu)
+bool make_cache_tensor_map(CUtensorMap* m, const void* cache, int num_blocks, int hkv, int halves);
 // a2-a9 tcgen05 / TMEM / TMA prefill: bf16, D=128, G in {1,2,4,8}
 bool prefill_sm100_supported(const Ctx& c);
 size_t prefill_sm100_workspace_bytes(const Ctx& c, int num_reqs, int num_q_tokens);

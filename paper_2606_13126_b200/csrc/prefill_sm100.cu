@@ -1127,18 +1127,6 @@ EncodeTiledFn get_encode() {
 }
 // cache viewed as a 4-D bf16 tensor (64 columns, 8 rows of a group [256 B apart], 2 halves of head_dim [128 B apart],
 // row groups [2048 B apart]); box = (64, 8, 2, 2) = one (block, head) = 4 KB landing as [group][half][8 x 128 B], SWIZZLE_128B
-// halves = 2: K (both halves of head_dim, 4 KB per block); halves = 1: V (the CTA's half, chosen by the box coordinate, 2 KB)
-bool make_cache_map(CUtensorMap* m, const void* cache, int num_blocks, int hkv, int halves) {
-  EncodeTiledFn enc = get_encode();
-  if (!enc) return false;
-  cuuint64_t dims[4] = {64, 8, 2, (cuuint64_t)num_blocks * hkv * 2};
-  cuuint64_t strides[3] = {(cuuint64_t)D * 2, 128, (cuuint64_t)kGroupBytes};
-  cuuint32_t box[4] = {64, 8, (cuuint32_t)halves, 2};
-  cuuint32_t estr[4] = {1, 1, 1, 1};
-  return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(cache), dims, strides, box, estr,
-             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
-             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
 // q viewed as [Tq][Hq][128]; box = (128/G tokens) x (G heads) x 64 columns: one half of an MMA tile, rows (token, head)
 bool make_q_map(CUtensorMap* m, const void* q, int num_q_tokens, int hq, int group) {
   EncodeTiledFn enc = get_encode();
@@ -1185,6 +1173,18 @@ bool launch_g(const Ctx& c, const CUtensorMap& mq, const CUtensorMap& mk, const 
 
 }  // namespace
 
+// halves = 2: K (both halves of head_dim, 4 KB per block); halves = 1: V (the CTA's half, chosen by the box coordinate, 2 KB)
+bool make_cache_tensor_map(CUtensorMap* m, const void* cache, int num_blocks, int hkv, int halves) {
+  EncodeTiledFn enc = get_encode();
+  if (!enc) return false;
+  cuuint64_t dims[4] = {64, 8, 2, (cuuint64_t)num_blocks * hkv * 2};
+  cuuint64_t strides[3] = {(cuuint64_t)D * 2, 128, (cuuint64_t)kGroupBytes};
+  cuuint32_t box[4] = {64, 8, (cuuint32_t)halves, 2};
+  cuuint32_t estr[4] = {1, 1, 1, 1};
+  return enc(m, CU_TENSOR_MAP_DATA_TYPE_BFLOAT16, 4, const_cast<void*>(cache), dims, strides, box, estr,
+             CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
 #ifdef MINIPIC_TRACE
 extern "C" int minipic_debug_trace_copy(long long* host, int* counts) {
   cudaDeviceSynchronize();
@@ -1216,7 +1216,7 @@ size_t prefill_sm100_workspace_bytes(const Ctx&, int, int num_q_tokens) {
 
 bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
   CUtensorMap mq, mk, mv, mo;
-  if (!make_cache_map(&mk, a.k_cache, c.num_blocks, c.hkv, 2) || !make_cache_map(&mv, a.v_cache, c.num_blocks, c.hkv, 1) ||
+  if (!make_cache_tensor_map(&mk, a.k_cache, c.num_blocks, c.hkv, 2) || !make_cache_tensor_map(&mv, a.v_cache, c.num_blocks, c.hkv, 1) ||
       !make_q_map(&mq, a.q, a.num_q_tokens, c.hq, c.group) || !make_out_map(&mo, a.out, a.num_q_tokens, c.hq, c.group)) {
     note_error("prefill_sm100: cuTensorMapEncodeTiled failed (driver entry point missing or bad tensor geometry)");
     return false;
