@@ -134,17 +134,20 @@ def gather_kv(k_cache: np.ndarray, v_cache: np.ndarray, block_table_row: np.ndar
 
 
 # ----------------------------------------------------------------------------- a6-a9: attention
-def _attend_rows(qr: np.ndarray, k: np.ndarray, v: np.ndarray, idx: np.ndarray, vis_lo: np.ndarray, scale: float):
+def _attend_rows(qr: np.ndarray, k: np.ndarray, v: np.ndarray, idx: np.ndarray, vis_lo: np.ndarray, scale: float,
+                 key_ok: np.ndarray | None = None):
     """Masked softmax attention for a group of query rows of one (request, head).
 
     qr [n, D] rotated queries; k, v [kv_len, D] rotated keys / values; row i sees key j iff
-    vis_lo[i] <= j <= idx[i].  Returns out [n, D], lse [n].  A row with no visible key returns
-    out = 0, lse = -inf.
+    vis_lo[i] <= j <= idx[i] (and key_ok[j], when the key-masking variant is on: PAPER.md:294).
+    Returns out [n, D], lse [n].  A row with no visible key returns out = 0, lse = -inf.
     """
     kv_len = k.shape[0]
     s = (qr @ k.T) * scale                                   # Eq. 2 scores for every (row, key)
     j = np.arange(kv_len)[None, :]
     visible = (j >= vis_lo[:, None]) & (j <= idx[:, None])
+    if key_ok is not None:
+        visible = visible & np.asarray(key_ok, bool)[None, :]
     s = np.where(visible, s, -np.inf)
     m = s.max(axis=1) if kv_len else np.full(qr.shape[0], -np.inf)
     empty = ~np.isfinite(m)
@@ -161,7 +164,7 @@ def prefill_attention(*, q, k_cache, v_cache, block_tables, cu_q_lens, kv_lens, 
                       q_seq_idx, q_vis_lo, num_q_heads: int, dtype: str, rope_theta: float,
                       softmax_scale: float | None = None, mode: str = "F", q_prerotated: bool = False,
                       k_prerotated: bool = False, rows: np.ndarray | None = None,
-                      heads: np.ndarray | None = None, row_chunk: int = 512):
+                      heads: np.ndarray | None = None, row_chunk: int = 512, key_mask: bool = False):
     """Steps 2-6 of DESIGN.md "Oracle algorithm" for every query row (or for ``rows`` x ``heads``).
 
     Returns (out fp64 [Tq, Hq, D], lse fp64 [Tq, Hq]); entries outside ``rows`` x ``heads`` are NaN.
@@ -169,6 +172,8 @@ def prefill_attention(*, q, k_cache, v_cache, block_tables, cu_q_lens, kv_lens, 
     and before the scores (the conventional pre-rotated-cache arithmetic).
     Query rows are processed in chunks of ``row_chunk`` only to bound memory; rows are
     independent, so this changes no arithmetic.
+    ``key_mask`` (the "key-vector zeroing" of marker / padding tokens that PAPER.md:294 defers, taken as a
+    MASK variant): a key whose logical position is negative is invisible to every query row.
     """
     tq = q.shape[0]
     hq = num_q_heads
@@ -193,6 +198,7 @@ def prefill_attention(*, q, k_cache, v_cache, block_tables, cu_q_lens, kv_lens, 
         idx = np.asarray(q_seq_idx)[sel].astype(np.int64)
         lo = np.asarray(q_vis_lo)[sel].astype(np.int64)
         q_pos = pos[idx]                                           # pi_r(idx_t)
+        key_ok = (pos >= 0) if key_mask else None
         cache_kv = {}
         for h in head_list:
             g = h // group                                         # GQA: KV head of query head h
@@ -211,7 +217,8 @@ def prefill_attention(*, q, k_cache, v_cache, block_tables, cu_q_lens, kv_lens, 
                 c1 = min(c0 + row_chunk, sel.size)
                 # keys outside [min vis_lo, max idx] of the chunk are invisible to every row of it
                 klo, hi = max(int(lo[c0:c1].min()), 0), int(idx[c0:c1].max()) + 1
-                o, l = _attend_rows(qr[c0:c1], kk[klo:hi], vv[klo:hi], idx[c0:c1] - klo, lo[c0:c1] - klo, scale)  # steps 5-6
+                o, l = _attend_rows(qr[c0:c1], kk[klo:hi], vv[klo:hi], idx[c0:c1] - klo, lo[c0:c1] - klo, scale,
+                                    None if key_ok is None else key_ok[klo:hi])                                   # steps 5-6
                 out[sel[c0:c1], h, :] = o
                 lse[sel[c0:c1], h] = l
     return out, lse
@@ -220,7 +227,7 @@ def prefill_attention(*, q, k_cache, v_cache, block_tables, cu_q_lens, kv_lens, 
 def decode_attention(*, q, k_cache, v_cache, block_tables, kv_lens, cu_kv_lens, kv_positions, num_q_heads: int,
                      dtype: str, rope_theta: float, q_vis_lo=None, softmax_scale: float | None = None,
                      mode: str = "F", q_prerotated: bool = False, k_prerotated: bool = False,
-                     seqs: np.ndarray | None = None, heads: np.ndarray | None = None):
+                     seqs: np.ndarray | None = None, heads: np.ndarray | None = None, key_mask: bool = False):
     """Decode = the same definition with one query per sequence at idx = kv_len - 1 (step 7)."""
     n = len(kv_lens)
     idx = (np.asarray(kv_lens) - 1).astype(np.int32)
@@ -229,7 +236,8 @@ def decode_attention(*, q, k_cache, v_cache, block_tables, kv_lens, cu_kv_lens, 
                              cu_q_lens=np.arange(n + 1), kv_lens=kv_lens, cu_kv_lens=cu_kv_lens,
                              kv_positions=kv_positions, q_seq_idx=idx, q_vis_lo=lo, num_q_heads=num_q_heads,
                              dtype=dtype, rope_theta=rope_theta, softmax_scale=softmax_scale, mode=mode,
-                             q_prerotated=q_prerotated, k_prerotated=k_prerotated, rows=seqs, heads=heads)
+                             q_prerotated=q_prerotated, k_prerotated=k_prerotated, rows=seqs, heads=heads,
+                             key_mask=key_mask)
 
 
 # ----------------------------------------------------------------------------- a11: LSE merge
