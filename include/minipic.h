@@ -64,8 +64,14 @@ typedef enum { MINIPIC_BF16 = 0, MINIPIC_F32 = 1 } minipic_dtype;
 enum {
   MINIPIC_Q_PREROTATED = 1u, /* caller already applied R(pos) to Q (the paper's own flow) */
   MINIPIC_K_PREROTATED = 2u, /* CONTROL ONLY: the cache holds rotated K, kernels skip the K RoPE step   */
-  MINIPIC_FORCE_SIMT   = 4u  /* DEBUG: run the generic fp32 CUDA-core attention kernels instead of the  */
+  MINIPIC_FORCE_SIMT   = 4u, /* DEBUG: run the generic fp32 CUDA-core attention kernels instead of the  */
                              /* tensor-core ones (bf16, head_dim 128 normally take the latter)          */
+  MINIPIC_KEY_MASK     = 8u  /* mask variant for marker / padding tokens (the "key-vector zeroing" that */
+                             /* PAPER.md:294 defers): a key with kv_positions[...] < 0 is invisible to  */
+                             /* EVERY query row of its request (as if it were deleted from the sequence; */
+                             /* sequence indices, q_seq_idx and q_vis_lo are unchanged).  Without the    */
+                             /* flag positions must be >= 0.  A row that queries AT a masked index has   */
+                             /* undefined output (such rows are discarded by the caller).               */
 };
 
 typedef struct {
@@ -106,6 +112,29 @@ int minipic_cache_write(const minipic_config* cfg,
                         const int64_t* slot_mapping,            /* [num_tokens], block*B + offset  */
                         int32_t num_tokens,
                         void* k_cache, void* v_cache, void* cuda_stream);
+
+/* ---- f1: fused pre-attention step ("rotated once by the model's RotaryEmbedding layer ... stores
+ * unrotated key vectors"; Table 2 row rotary_embedding/base.py) ---------------------------------
+ * ONE pass over the QKV-projection output of the new tokens, qkv [num_tokens, Hq + 2 Hkv, D] (heads [0, Hq) = Q,
+ * [Hq, Hq + Hkv) = K, the rest V), instead of a rotary kernel over Q plus minipic_cache_write:
+ *   k_cache / v_cache[slot / B, h, slot % B, :] = K / V rows of token t, raw byte copy (bit exact, slot < 0: skipped);
+ *   q_out[t, h] = R(positions[t]) q[t, h], rotated in fp32 and rounded ONCE to the I/O dtype - the paper's own flow:
+ *                 pass q_out to the attention calls with MINIPIC_Q_PREROTATED.  If cfg->flags has
+ *                 MINIPIC_Q_PREROTATED the rows are copied unrotated.
+ * positions: int32 [num_tokens], the tokens' logical positions (>= 0).  q_out: [num_tokens, Hq, D], must not overlap qkv. */
+int minipic_preattn_fused(const minipic_config* cfg, const void* qkv, const int64_t* slot_mapping,
+                          const int32_t* positions, int32_t num_tokens, void* q_out,
+                          void* k_cache, void* v_cache, void* cuda_stream);
+
+/* ---- f4: copy-and-re-rotate CONTROL ("block-by-block copy and repositioning"; App. A :284-286) ------
+ * What a POSITION-DEPENDENT cache must do to reuse a span at another offset; MiniPIC never needs it (its blocks hold
+ * unrotated keys) - it exists to measure the HBM traffic the position-free layout avoids.  For every i < num_pairs:
+ *   k_cache[dst_blocks[i]] = R(delta[i]) k_cache[src_blocks[i]]  (all heads, all 16 rows; fp32 rotation, one RN),
+ *   v_cache[dst_blocks[i]] = v_cache[src_blocks[i]]               (bit exact).
+ * delta may be negative.  No block id may appear both as a source and as a destination in one call, destinations must
+ * be distinct. */
+int minipic_block_rerotate(const minipic_config* cfg, void* k_cache, void* v_cache, const int32_t* src_blocks,
+                           const int32_t* dst_blocks, const int32_t* delta, int32_t num_pairs, void* cuda_stream);
 
 /* ---- a2-a9: prefill attention (PAPER.md:100-113, Eq. 2; mask :57, :90, :123-128, :143) ---------
  * For every query row t of request r (rows cu_q_lens[r] .. cu_q_lens[r+1]) and head h:

@@ -22,7 +22,7 @@ MINIPIC_ERR_UNSUPPORTED = 2
 MINIPIC_ERR_WORKSPACE_TOO_SMALL = 3
 MINIPIC_ERR_CUDA = 4
 MINIPIC_BF16, MINIPIC_F32 = 0, 1
-MINIPIC_Q_PREROTATED, MINIPIC_K_PREROTATED, MINIPIC_FORCE_SIMT = 1, 2, 4
+MINIPIC_Q_PREROTATED, MINIPIC_K_PREROTATED, MINIPIC_FORCE_SIMT, MINIPIC_KEY_MASK = 1, 2, 4, 8
 
 # every symbol include/minipic.h declares (tests check the library exports all of them)
 EXPORTS = [
@@ -32,7 +32,7 @@ EXPORTS = [
     "minipic_prefill_host_arena_bytes", "minipic_prefill_step_host",
     "minipic_decode_host_arena_bytes", "minipic_decode_step_host",
     "minipic_status_string", "minipic_last_cuda_error", "minipic_launch_count", "minipic_last_variant",
-    "minipic_prefill_status",
+    "minipic_prefill_status", "minipic_preattn_fused", "minipic_block_rerotate",
 ]
 
 
@@ -87,6 +87,10 @@ def lib() -> C.CDLL:
     L.minipic_last_variant.restype = C.c_char_p
     L.minipic_prefill_status.restype = C.c_int
     L.minipic_prefill_status.argtypes = [VP, VP]
+    L.minipic_preattn_fused.restype = C.c_int
+    L.minipic_preattn_fused.argtypes = [P, VP, VP, VP, I32, VP, VP, VP, VP]
+    L.minipic_block_rerotate.restype = C.c_int
+    L.minipic_block_rerotate.argtypes = [P, VP, VP, VP, VP, VP, I32, VP]
     _lib = L
     return L
 
@@ -143,6 +147,16 @@ def minipic_rope_table_build(cfg, num_positions: int, table, stream=None) -> Non
 def minipic_cache_write(cfg, k_new, v_new, slot_mapping, num_tokens, k_cache, v_cache, stream=None) -> None:
     _check(lib().minipic_cache_write(C.byref(cfg), _ptr(k_new), _ptr(v_new), _ptr(slot_mapping), num_tokens,
                                      _ptr(k_cache), _ptr(v_cache), _stream(stream)))
+
+
+def minipic_preattn_fused(cfg, qkv, slot_mapping, positions, num_tokens, q_out, k_cache, v_cache, stream=None) -> None:
+    _check(lib().minipic_preattn_fused(C.byref(cfg), _ptr(qkv), _ptr(slot_mapping), _ptr(positions), num_tokens,
+                                       _ptr(q_out), _ptr(k_cache), _ptr(v_cache), _stream(stream)))
+
+
+def minipic_block_rerotate(cfg, k_cache, v_cache, src_blocks, dst_blocks, delta, num_pairs, stream=None) -> None:
+    _check(lib().minipic_block_rerotate(C.byref(cfg), _ptr(k_cache), _ptr(v_cache), _ptr(src_blocks), _ptr(dst_blocks),
+                                        _ptr(delta), num_pairs, _stream(stream)))
 
 
 def minipic_prefill_workspace_bytes(cfg, num_reqs: int, num_q_tokens: int) -> int:

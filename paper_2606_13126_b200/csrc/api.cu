@@ -158,6 +158,32 @@ int minipic_cache_write(const minipic_config* cfg, const void* k_new, const void
   return check_launch("cache_write") ? MINIPIC_OK : MINIPIC_ERR_CUDA;
 }
 
+int minipic_preattn_fused(const minipic_config* cfg, const void* qkv, const int64_t* slot_mapping, const int32_t* positions,
+                          int32_t num_tokens, void* q_out, void* k_cache, void* v_cache, void* cuda_stream) {
+  int st = validate_cfg(cfg);
+  if (st != MINIPIC_OK) return st;
+  if (num_tokens < 0) return MINIPIC_ERR_INVALID_ARG;
+  if (num_tokens == 0) return MINIPIC_OK;
+  if (!qkv || !slot_mapping || !positions || !q_out || !k_cache || !v_cache) return MINIPIC_ERR_INVALID_ARG;
+  if (((uintptr_t)qkv | (uintptr_t)q_out | (uintptr_t)k_cache | (uintptr_t)v_cache) & 15) return MINIPIC_ERR_INVALID_ARG;
+  Ctx c; make_ctx(cfg, cuda_stream, &c);
+  launch_preattn_fused(c, qkv, slot_mapping, positions, num_tokens, q_out, k_cache, v_cache);
+  return check_launch("preattn_fused") ? MINIPIC_OK : MINIPIC_ERR_CUDA;
+}
+
+int minipic_block_rerotate(const minipic_config* cfg, void* k_cache, void* v_cache, const int32_t* src_blocks,
+                           const int32_t* dst_blocks, const int32_t* delta, int32_t num_pairs, void* cuda_stream) {
+  int st = validate_cfg(cfg);
+  if (st != MINIPIC_OK) return st;
+  if (num_pairs < 0) return MINIPIC_ERR_INVALID_ARG;
+  if (num_pairs == 0) return MINIPIC_OK;
+  if (!k_cache || !v_cache || !src_blocks || !dst_blocks || !delta) return MINIPIC_ERR_INVALID_ARG;
+  if (((uintptr_t)k_cache | (uintptr_t)v_cache) & 15) return MINIPIC_ERR_INVALID_ARG;
+  Ctx c; make_ctx(cfg, cuda_stream, &c);
+  launch_block_rerotate(c, k_cache, v_cache, src_blocks, dst_blocks, delta, num_pairs);
+  return check_launch("block_rerotate") ? MINIPIC_OK : MINIPIC_ERR_CUDA;
+}
+
 size_t minipic_prefill_workspace_bytes(const minipic_config* cfg, int32_t num_reqs, int32_t num_q_tokens) {
   if (validate_cfg(cfg) != MINIPIC_OK || num_reqs < 0 || num_q_tokens < 0) return 0;
   Ctx c; make_ctx(cfg, nullptr, &c);

@@ -33,8 +33,10 @@ struct WarpAttn {
 
   // keys j in [j0, j1) of request with block table `bt`, positions `pos` (both already offset to the request)
   __device__ __forceinline__ void run(const T* kc, const T* vc, const int* bt, const int* pos, int hkv, int g,
-                                      int j0, int j1, float scale, const RopeParams& rp, bool k_prerot, int lane) {
+                                      int j0, int j1, float scale, const RopeParams& rp, bool k_prerot, bool key_mask,
+                                      int lane) {
     for (int j = j0; j < j1; ++j) {
+      if (key_mask && __ldg(pos + j) < 0) continue;   // MINIPIC_KEY_MASK: invisible to every row
       const int blk = __ldg(bt + j / kBlock);
       const size_t row = (((size_t)blk * hkv + g) * kBlock + (j % kBlock)) * D;
       float k[E], v[E];
@@ -91,7 +93,7 @@ __global__ void __launch_bounds__(128) prefill_simt_kernel(PrefillArgs a, int hq
   wa.init((const T*)a.q + ((size_t)t * hq + h) * D, rp, __ldg(pos + idx), flags & MINIPIC_Q_PREROTATED, lane);
   const int hi = min(idx + 1, __ldg(a.kv_lens + r));
   wa.run((const T*)a.k_cache, (const T*)a.v_cache, bt, pos, hkv, h / (hq / hkv), lo, hi, scale, rp,
-         flags & MINIPIC_K_PREROTATED, lane);
+         flags & MINIPIC_K_PREROTATED, flags & MINIPIC_KEY_MASK, lane);
   T* o = (T*)a.out + ((size_t)t * hq + h) * D;
   const float inv = wa.l_run > 0.f ? 1.f / wa.l_run : 0.f;
 #pragma unroll
@@ -115,7 +117,7 @@ __global__ void __launch_bounds__(32) decode_simt_kernel(DecodeArgs a, int hq, i
   wa.init((const T*)a.q + ((size_t)r * hq + h) * D, rp, __ldg(pos + idx), flags & MINIPIC_Q_PREROTATED, lane);
   const int j0 = max(lo, s * split_len), j1 = min(kv_len, (s + 1) * split_len);
   wa.run((const T*)a.k_cache, (const T*)a.v_cache, bt, pos, hkv, h / (hq / hkv), j0, j1, scale, rp,
-         flags & MINIPIC_K_PREROTATED, lane);
+         flags & MINIPIC_K_PREROTATED, flags & MINIPIC_KEY_MASK, lane);
   const size_t pr = ((size_t)r * hq + h) * max_splits + s;
   const float inv = wa.l_run > 0.f ? 1.f / wa.l_run : 0.f;
 #pragma unroll

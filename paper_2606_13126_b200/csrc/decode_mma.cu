@@ -100,7 +100,7 @@ __device__ __forceinline__ uint4 lds128(uint32_t addr) {
   return v;
 }
 
-template <bool kRotK, int W>
+template <bool kRotK, bool kKeyMask, int W>
 __global__ void __launch_bounds__(32 * W, MINIPIC_DECODE_WARPS_PER_SM / W)
 decode_mma_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_constant__ CUtensorMap tmap_v, DecodeArgs a,
                   int hq, int hkv, int group, float scale_log2, RopeParams rp, unsigned flags, int split_len,
@@ -253,7 +253,9 @@ decode_mma_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_const
 #pragma unroll
       for (int e = 0; e < 2; ++e) {
         const int j = kb * kBlock + 8 * t + 2 * q4 + e;
-        sc[t][e] = (j >= j_begin && j < j_end) ? st[t][e] * scale_log2 : -INFINITY;
+        bool vis = j >= j_begin && j < j_end;
+        if (kKeyMask && vis) vis = __ldg(pos + j) >= 0;   // MINIPIC_KEY_MASK: invisible to every row
+        sc[t][e] = vis ? st[t][e] * scale_log2 : -INFINITY;
         m_blk = fmaxf(m_blk, sc[t][e]);
       }
     m_blk = fmaxf(m_blk, __shfl_xor_sync(0xffffffffu, m_blk, 1));
@@ -315,7 +317,7 @@ decode_mma_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_const
   }
 }
 
-template <bool kRotK, int W>
+template <bool kRotK, bool kKeyMask, int W>
 bool launch_k(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, const CUtensorMap& mk, const CUtensorMap& mv,
               float* o_part, float* lse_part) {
   const size_t smem = (size_t)W * kStages * kStageBytes + 64 * 8 + (size_t)W * kStages * 8;
@@ -323,22 +325,25 @@ bool launch_k(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, const CUte
   int dev = 0;
   cudaGetDevice(&dev);
   if (dev < 0 || dev >= 64 || !attr_done[dev]) {
-    if (cudaFuncSetAttribute(decode_mma_kernel<kRotK, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+    if (cudaFuncSetAttribute(decode_mma_kernel<kRotK, kKeyMask, W>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
       note_error("decode_mma: cudaFuncSetAttribute(MaxDynamicSharedMemorySize) failed");
       return false;
     }
     if (dev >= 0 && dev < 64) attr_done[dev] = true;
   }
   dim3 grid((unsigned)sp.max_splits * (unsigned)a.num_seqs, c.hkv / W);
-  decode_mma_kernel<kRotK, W><<<grid, 32 * W, smem, c.stream>>>(mk, mv, a, c.hq, c.hkv, c.group, c.scale_log2, c.rope,
+  decode_mma_kernel<kRotK, kKeyMask, W><<<grid, 32 * W, smem, c.stream>>>(mk, mv, a, c.hq, c.hkv, c.group, c.scale_log2, c.rope,
                                                                c.flags, sp.split_len, sp.max_splits, o_part, lse_part);
   return true;
 }
 template <int W>
 bool launch_w(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, const CUtensorMap& mk, const CUtensorMap& mv,
               float* o_part, float* lse_part) {
-  return (c.flags & MINIPIC_K_PREROTATED) ? launch_k<false, W>(c, a, sp, mk, mv, o_part, lse_part)
-                                          : launch_k<true, W>(c, a, sp, mk, mv, o_part, lse_part);
+  if (c.flags & MINIPIC_KEY_MASK)
+    return (c.flags & MINIPIC_K_PREROTATED) ? launch_k<false, true, W>(c, a, sp, mk, mv, o_part, lse_part)
+                                            : launch_k<true, true, W>(c, a, sp, mk, mv, o_part, lse_part);
+  return (c.flags & MINIPIC_K_PREROTATED) ? launch_k<false, false, W>(c, a, sp, mk, mv, o_part, lse_part)
+                                          : launch_k<true, false, W>(c, a, sp, mk, mv, o_part, lse_part);
 }
 
 }  // namespace

@@ -20,6 +20,12 @@ void launch_rope_table(const RopeParams& rp, int num_positions, float2* table, c
 void launch_cache_write(int itemsize, int hkv, int d, const void* k_new, const void* v_new, const int64_t* slots,
                         int num_tokens, void* k_cache, void* v_cache, cudaStream_t s);
 
+// f1 / f4 (preattn.cu)
+void launch_preattn_fused(const Ctx& c, const void* qkv, const int64_t* slots, const int* positions, int num_tokens,
+                          void* q_out, void* k_cache, void* v_cache);
+void launch_block_rerotate(const Ctx& c, void* k_cache, void* v_cache, const int* src, const int* dst, const int* delta,
+                           int num_pairs);
+
 struct PrefillArgs {
   const void* q; const void* k_cache; const void* v_cache;
   const int* block_tables; int max_blocks;

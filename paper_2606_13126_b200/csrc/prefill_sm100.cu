@@ -521,7 +521,7 @@ struct Rot8 {
   }
 };
 
-template <int G>
+template <int G, bool kKeyMask>   // kKeyMask: MINIPIC_KEY_MASK variant (its own instantiation: the common path pays nothing)
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
                      const __grid_constant__ CUtensorMap tmap_v, const __grid_constant__ CUtensorMap tmap_o,
@@ -1012,6 +1012,18 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       for (int i = 0; i < n; ++i, ++sc) {
         const int j0 = it.kv_lo + i * BN;
         float s[BN];
+        // MINIPIC_KEY_MASK: keys with a negative logical position are invisible to every row.  Lane l looks
+        // at the positions of columns l, l + 32, l + 64, l + 96 (fetched before the wait); four ballots give the tile's
+        // 128-bit mask, warp-uniform, and tiles without a masked key (nearly all) pay nothing more.
+        unsigned dead0 = 0, dead1 = 0, dead2 = 0, dead3 = 0;
+        if (kKeyMask) {
+          const int* pos = a.kv_positions + it.kv_off;
+          const int jl = j0 + lane;
+          dead0 = __ballot_sync(0xffffffffu, jl < it.kv_len && __ldg(pos + jl) < 0);
+          dead1 = __ballot_sync(0xffffffffu, jl + 32 < it.kv_len && __ldg(pos + jl + 32) < 0);
+          dead2 = __ballot_sync(0xffffffffu, jl + 64 < it.kv_len && __ldg(pos + jl + 64) < 0);
+          dead3 = __ballot_sync(0xffffffffu, jl + 96 < it.kv_len && __ldg(pos + jl + 96) < 0);
+        }
         w.wait(bar(S_FULL + x), sc & 1);
         if ((warp & 3) == 0) TRACE_L0(3 + x, 40);
         tc_fence_after();
@@ -1027,6 +1039,15 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         if (j0 + BN - 1 > min(idx_first, it.kv_len - 1)) {   // tile reaches past the lowest row's last visible key
 #pragma unroll
           for (int c = 0; c < BN; ++c) s[c] = (c <= c_hi) ? s[c] : -INFINITY;
+        }
+        if (kKeyMask && (dead0 | dead1 | dead2 | dead3)) {
+#pragma unroll
+          for (int c = 0; c < 32; ++c) {
+            if ((dead0 >> c) & 1u) s[c] = -INFINITY;
+            if ((dead1 >> c) & 1u) s[32 + c] = -INFINITY;
+            if ((dead2 >> c) & 1u) s[64 + c] = -INFINITY;
+            if ((dead3 >> c) & 1u) s[96 + c] = -INFINITY;
+          }
         }
         if (c_lo > 0) {   // vis_lo inside the first gathered 16-token block (kv_lo = floor16(vis_lo)): c_lo < 16
 #pragma unroll
@@ -1152,23 +1173,29 @@ bool make_out_map(CUtensorMap* m, void* out, int num_q_tokens, int hq, int group
              CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int G>
-bool launch_g(const Ctx& c, const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mo,
+template <int G, bool kKeyMask>
+bool launch_gk(const Ctx& c, const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mo,
               const Params& prm, int sms) {
   const size_t smem = sizeof(Smem);
   static bool attr_done[64] = {};   // the attribute is per (function, device): track it per device ordinal
   int dev = 0;
   cudaGetDevice(&dev);
   if (dev < 0 || dev >= 64 || !attr_done[dev]) {
-    if (cudaFuncSetAttribute(prefill_sm100_kernel<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+    if (cudaFuncSetAttribute(prefill_sm100_kernel<G, kKeyMask>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
       note_error("prefill_sm100: cudaFuncSetAttribute(MaxDynamicSharedMemorySize) failed");
       return false;
     }
     if (dev >= 0 && dev < 64) attr_done[dev] = true;
   }
-  prefill_sm100_kernel<G><<<sms, kThreads, smem, c.stream>>>(mq, mk, mv, mo, prm);
+  prefill_sm100_kernel<G, kKeyMask><<<sms, kThreads, smem, c.stream>>>(mq, mk, mv, mo, prm);
   note_launch();
   return true;
+}
+
+template <int G>
+bool launch_g(const Ctx& c, const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mo,
+              const Params& prm, int sms) {
+  return (c.flags & MINIPIC_KEY_MASK) ? launch_gk<G, true>(c, mq, mk, mv, mo, prm, sms) : launch_gk<G, false>(c, mq, mk, mv, mo, prm, sms);
 }
 
 }  // namespace

@@ -17,7 +17,7 @@ All arrays are numpy.  bf16 tensors are carried as ``uint16`` bit patterns.
 """
 from __future__ import annotations
 
-from dataclasses import dataclass, field
+from dataclasses import dataclass, field, replace
 from typing import List, Optional, Sequence, Tuple
 
 import numpy as np
@@ -285,6 +285,65 @@ def rag_partial_prefill(*, name: str = "c3_rag_partial_prefill", seed: int = 2, 
 
 def config3(seed: int = 2) -> Workload:
     return rag_partial_prefill(seed=seed)
+
+
+def epic_linked_prefill(*, name: str = "epic_linked_prefill", seed: int = 6, hq: int = 32, hkv: int = 8, d: int = 128,
+                        theta: float = 5e5, dtype: str = "bf16", sigma: float = 1.0, pool_spans: int = 200,
+                        span_min: int = 128, span_max: int = 512, num_reqs: int = 32, spans_per_req: int = 10,
+                        prefix_len: int = 32, suffix_len: int = 64, link_tokens: int = 16) -> Workload:
+    """EPIC / LegoLink through the same descriptor: every document is cached except its
+    first ``link_tokens`` tokens (a block multiple: "with block-level granularity, k rounds to a block multiple"), which
+    hash-depend on the preceding context and are RECOMPUTED inside the final prompt - they are queries that see everything
+    before them (vis_lo = 0) and their fresh K/V go to private blocks; the rest of each document cache-hits from the shared
+    pool.  Queries = the link tokens of every document + the question suffix."""
+    if link_tokens % BLOCK:
+        raise ValueError("link_tokens must be a block multiple")
+    rng = np.random.default_rng(seed)
+    lens = [max(_round_up(int(x)), link_tokens + BLOCK) for x in rng.integers(span_min, span_max + 1, size=pool_spans)]
+    new_tokens = num_reqs * (spans_per_req * link_tokens + suffix_len)
+    num_blocks = (sum(lens) + _round_up(prefix_len) + new_tokens) // BLOCK + 64
+    c = _Composer(rng, num_blocks, hkv, d, dtype, sigma)
+    prefix_blocks = c.tokens(prefix_len, resident=True, tag="prefix") if prefix_len else None
+    pool = [c.tokens(L, resident=True, tag=f"span{i}") for i, L in enumerate(lens)]
+    reqs = []
+    for r in range(num_reqs):
+        pick = rng.choice(pool_spans, size=spans_per_req, replace=False)
+        segs = []
+        if prefix_len:
+            segs.append(_Seg(prefix_blocks, prefix_len, local=False, query=False))
+        for sp in pick:
+            L = lens[int(sp)]
+            segs.append(_Seg(c.tokens(link_tokens, resident=False), link_tokens, local=False, query=True))
+            segs.append(_Seg(pool[int(sp)][link_tokens // BLOCK:], L - link_tokens, local=True, query=False))
+        segs.append(_Seg(c.tokens(suffix_len, resident=False), suffix_len, local=False, query=True))
+        reqs.append(segs)
+    lay = _layout(reqs)
+    q = _draw(rng, (int(lay["cu_q_lens"][-1]), hq, d), sigma, dtype)
+    return Workload(name=name, kind="prefill", num_q_heads=hq, num_kv_heads=hkv, head_dim=d,
+                    num_blocks=num_blocks, dtype=dtype, rope_theta=theta, resident=c.resident,
+                    new=c.new_batch(), q=q, seed=seed, notes=dict(pool_span_lens=lens, link_tokens=link_tokens), **lay)
+
+
+def with_masked_keys(w: Workload, seed: int = 0, frac: float = 0.06) -> Workload:
+    """Key-masking variant (minipic.h MINIPIC_KEY_MASK): a copy of ``w`` in which a random ``frac`` of the
+    keys that are NOT query tokens - plus, per request, one whole 16-token block and sequence index 0 when they are not
+    queries - carry logical position -1 (marker / padding tokens).  Run it with flags = MINIPIC_KEY_MASK."""
+    rng = np.random.default_rng(seed)
+    pos = w.kv_positions.copy()
+    for r in range(w.num_reqs):
+        n, o = int(w.kv_lens[r]), int(w.cu_kv_lens[r])
+        is_q = np.zeros(n, bool)
+        if w.kind == "prefill":
+            is_q[w.q_seq_idx[int(w.cu_q_lens[r]):int(w.cu_q_lens[r + 1])]] = True
+        else:
+            is_q[n - 1] = True
+        dead = (rng.random(n) < frac)
+        b = int(rng.integers(0, max(n // BLOCK, 1))) * BLOCK
+        dead[b:b + BLOCK] = True
+        dead[0] = True
+        dead &= ~is_q
+        pos[o:o + n][dead] = -1
+    return replace(w, name=w.name + "_keymask", kv_positions=pos, notes=dict(w.notes, key_mask=True))
 
 
 # --------------------------------------------------------------------------- config 4

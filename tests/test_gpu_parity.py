@@ -30,6 +30,7 @@ import numpy as np
 import pytest
 import torch
 
+from oracle import minipic_next as N
 from oracle import minipic_oracle as O
 from paper_2606_13126_b200 import binding as mp
 from paper_2606_13126_b200 import workloads as W
@@ -87,11 +88,11 @@ def _record(stats, w):
             f.write(json.dumps({"workload": w.name, **stats}) + "\n")
 
 
-def compare(dw, rows=None, heads=None, oracle_cache=None, expect_variant=None, k_prerot=False):
+def compare(dw, rows=None, heads=None, oracle_cache=None, expect_variant=None, k_prerot=False, key_mask=False):
     w = dw.w
     dw.check_health()   # no hand-off barrier of the prefill pipeline timed out
     kc, vc = oracle_cache if oracle_cache is not None else O.build_cache(w)
-    of, lf = O.run_workload(w, kc, vc, mode="F", rows=rows, heads=heads, k_prerotated=k_prerot)
+    of, lf = O.run_workload(w, kc, vc, mode="F", rows=rows, heads=heads, k_prerotated=k_prerot, key_mask=key_mask)
     variant = mp.minipic_last_variant()
     if expect_variant:
         assert variant == expect_variant, variant
@@ -112,7 +113,7 @@ def compare(dw, rows=None, heads=None, oracle_cache=None, expect_variant=None, k
         assert dl.max() <= LSE_TOL, stats
         _record(stats, w)
         return stats
-    _, lq = O.run_workload(w, kc, vc, mode="Q", rows=rows, heads=heads, k_prerotated=k_prerot)
+    _, lq = O.run_workload(w, kc, vc, mode="Q", rows=rows, heads=heads, k_prerotated=k_prerot, key_mask=key_mask)
     dq_full = np.where(sel, np.abs(gl - lq), 0.0)                    # [Tq, Hq]
     dq = dq_full[sel]
     row_ids, nvis = _visible_counts(w, None)
@@ -475,3 +476,114 @@ def test_midsize_many_items_per_cta_full_compare():
     dw.step(); torch.cuda.synchronize()
     st = compare(dw, expect_variant="prefill_sm100_tcgen05")
     assert st["entries"] == w.num_q_tokens * w.num_q_heads
+
+
+# --------------------------------------------------------------------------- the steps next to the path
+@pytest.mark.parametrize("which", [1, 2, 3])
+@pytest.mark.parametrize("force_simt", [False, True])
+def test_key_mask_variant(which, force_simt):
+    """MINIPIC_KEY_MASK: keys with a negative logical position are invisible to every row - prefill
+    (tcgen05 and CUDA-core kernels) and split-KV decode against the oracle's key_mask."""
+    w = W.with_masked_keys(W.small_variants()[which], seed=which)
+    assert (w.kv_positions < 0).sum() > 16
+    dw = DeviceWorkload(w, flags=mp.MINIPIC_KEY_MASK | (mp.MINIPIC_FORCE_SIMT if force_simt else 0))
+    dw.step(); torch.cuda.synchronize()
+    compare(dw, key_mask=True)
+    if which == 3 and not force_simt:   # the flag, not the data, turns the mask on: same inputs without it differ
+        d0 = DeviceWorkload(w); d0.step(); torch.cuda.synchronize()
+        assert np.abs(d0.out_f64() - dw.out_f64()).max() > 1e-2
+
+
+def test_epic_linked_workload():
+    """EPIC / LegoLink as a workload: link tokens of every document are recomputed queries (vis_lo = 0,
+    fresh K/V in private blocks), the rest of each document cache-hits from shared blocks."""
+    w = W.epic_linked_prefill(hq=8, hkv=2, pool_spans=12, span_min=96, span_max=400, num_reqs=5, spans_per_req=4,
+                              link_tokens=32, seed=21)
+    dw = DeviceWorkload(w); dw.step(); torch.cuda.synchronize()
+    st = compare(dw, expect_variant="prefill_sm100_tcgen05")
+    assert st["entries"] == w.num_q_tokens * w.num_q_heads
+
+
+def _assert_rotated_bf16(got_bits, want_f64, src_f64):
+    """A rotated value computed in fp32 and rounded once to bf16, against the oracle's (fp64 rotation, one rounding):
+    the fp32 result is within ~5e-7 * sqrt(a^2 + b^2) of the exact one (a, b = the rotate-half pair it comes from), so the
+    two roundings agree except where the exact value sits that close to a bf16 rounding boundary - then they are
+    neighbours.  |got - want| <= ulp_bf16(want) + 5e-7 * pair norm, and mismatches are rare."""
+    got = O.bf16_bits_to_f64(got_bits)
+    h = src_f64.shape[-1] // 2
+    pn = np.sqrt(src_f64[..., :h] ** 2 + src_f64[..., h:] ** 2)
+    pn = np.concatenate([pn, pn], axis=-1)
+    ulp = 2.0 ** (np.floor(np.log2(np.maximum(np.abs(want_f64), 2.0 ** -126))) - 7)
+    err = np.abs(got - want_f64)
+    assert np.all(err <= ulp + 5e-7 * pn), float((err - ulp - 5e-7 * pn).max())
+    assert (err > 0).mean() < 2e-3, float((err > 0).mean())
+
+
+@pytest.mark.parametrize("which", ["s2", "c1"])
+def test_preattn_fused(which):
+    """f1 (Table 2 :207): one launch writes K, V unrotated (bit exact) and Q rotated once; attention on the
+    result with MINIPIC_Q_PREROTATED meets the usual gates."""
+    w = W.small_variants()[0] if which == "s2" else W.config1()
+    nb = w.new[0]
+    T, hq, hkv = w.num_q_tokens, w.num_q_heads, w.num_kv_heads
+    assert nb.k.shape[0] == T and w.num_reqs == 1                     # every token is new and is a query, in order
+    assert np.array_equal(nb.slots, w.block_tables[0][w.q_seq_idx // 16].astype(np.int64) * 16 + w.q_seq_idx % 16)
+    qkv = np.concatenate([w.q, nb.k, nb.v], axis=1)
+    pos = w.kv_positions[w.q_seq_idx]
+    fill = 0x7FC1 if w.dtype == "bf16" else np.float32(np.nan)        # unwritten slots hold NaN patterns
+    kc = O.new_cache(w.num_blocks, hkv, 16, w.head_dim, w.dtype, fill); vc = O.new_cache(w.num_blocks, hkv, 16, w.head_dim, w.dtype, fill)
+    q_want = N.preattn_fused(qkv, nb.slots, pos, kc, vc, num_q_heads=hq, num_kv_heads=hkv, dtype=w.dtype, rope_theta=w.rope_theta)
+    dw = DeviceWorkload(w, cache_fill=(0x7FC1 if w.dtype == "bf16" else float("nan")), upload_resident=True)
+    to_dev = lambda a: torch.from_numpy(a.view(np.int16) if a.dtype == np.uint16 else a).cuda()
+    q_out = torch.zeros_like(dw.q)
+    mp.minipic_preattn_fused(dw.cfg, to_dev(qkv), to_dev(nb.slots), to_dev(pos.astype(np.int32)), T, q_out, dw.k_cache, dw.v_cache)
+    torch.cuda.synchronize()
+    gk, gv = dw.cache_bits()
+    assert gk.tobytes() == kc.tobytes() and gv.tobytes() == vc.tobytes()          # K, V: bit exact incl. untouched slots
+    if w.dtype == "bf16":
+        _assert_rotated_bf16(q_out.cpu().numpy().view(np.uint16), q_want, O.to_f64(w.q, w.dtype))
+    else:
+        assert np.abs(q_out.cpu().numpy().astype(np.float64) - q_want).max() <= 2e-6
+    dw.q = q_out
+    dw.set_flags(mp.MINIPIC_Q_PREROTATED)
+    dw.attention(); torch.cuda.synchronize()
+    compare(dw, oracle_cache=(kc, vc))
+    # under MINIPIC_Q_PREROTATED the fused step copies Q unrotated
+    q_copy = torch.zeros_like(dw.q)
+    mp.minipic_preattn_fused(dw.cfg, to_dev(qkv), to_dev(nb.slots), to_dev(pos.astype(np.int32)), T, q_copy, dw.k_cache, dw.v_cache)
+    torch.cuda.synchronize()
+    assert q_copy.cpu().numpy().tobytes() == (w.q.view(np.int16) if w.dtype == "bf16" else w.q).tobytes()
+
+
+@pytest.mark.parametrize("dtype", ["bf16", "f32"])
+def test_block_rerotate_control(dtype):
+    """f4: dst block <- R(delta) src block for K (one rounding), plain copy for V."""
+    rng = np.random.default_rng(17)
+    hkv, d, nblk, theta = 8, 128, 48, 5e5
+    raw_k = rng.standard_normal((nblk, hkv, 16, d)).astype(np.float32); raw_v = rng.standard_normal((nblk, hkv, 16, d)).astype(np.float32)
+    if dtype == "bf16":
+        kc, vc = W.f32_to_bf16_bits(raw_k), W.f32_to_bf16_bits(raw_v)
+    else:
+        kc, vc = raw_k.copy(), raw_v.copy()
+    perm = rng.permutation(nblk)
+    src, dst = perm[:20].astype(np.int32), perm[20:40].astype(np.int32)
+    src[5] = src[4]                                                   # one source feeds two destinations
+    delta = rng.integers(-40000, 40000, 20).astype(np.int32); delta[0] = 0; delta[1] = 1; delta[2] = -1
+    to_dev = lambda a: torch.from_numpy(a.view(np.int16) if a.dtype == np.uint16 else a).cuda()
+    gk, gv = to_dev(kc), to_dev(vc)
+    cfg = mp.make_config(num_q_heads=32, num_kv_heads=hkv, head_dim=d, num_blocks=nblk, dtype=dtype, rope_theta=theta)
+    mp.minipic_block_rerotate(cfg, gk, gv, to_dev(src), to_dev(dst), to_dev(delta), 20)
+    torch.cuda.synchronize()
+    k_before = kc.copy()
+    N.block_rerotate(kc, vc, src, dst, delta, dtype=dtype, rope_theta=theta)
+    hk, hv = gk.cpu().numpy(), gv.cpu().numpy()
+    if dtype == "bf16":
+        hk, hv = hk.view(np.uint16), hv.view(np.uint16)
+        assert hv.tobytes() == vc.tobytes()
+        _assert_rotated_bf16(hk[dst], O.bf16_bits_to_f64(kc[dst]), O.bf16_bits_to_f64(k_before[src]))
+        untouched = np.setdiff1d(np.arange(nblk), dst)
+        assert hk[untouched].tobytes() == kc[untouched].tobytes()
+        assert hk[dst[0]].tobytes() == kc[src[0]].tobytes()           # delta 0: bit-exact copy
+    else:
+        assert hv.tobytes() == vc.tobytes()
+        assert np.abs(hk.astype(np.float64) - kc.astype(np.float64)).max() <= 4e-6
