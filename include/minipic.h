@@ -219,6 +219,34 @@ int minipic_decode_step_host(const minipic_config* cfg,
  * Optional: the attention calls themselves stay asynchronous. */
 int minipic_prefill_status(const void* workspace, void* cuda_stream);
 
+/* ---- f3: HOST-side block hasher and block pool (Eq. 1; request procedure :123-128) ----------------
+ * The step before block tables exist.  Pure host code: every pointer below is a HOST pointer, nothing touches the GPU.
+ *   h_i = H(h_0, x_i)      if block i STARTS WITH ssep_id   (SSEP: detached - the span hashes the same anywhere)
+ *         H(h_0, x_{<=i})  if block i STARTS WITH pdep_id   (PDEP: depends on the whole prompt so far)
+ *         H(h_{i-1}, x_i)  otherwise                        (the engine's ordinary chain; h_{-1} = h_0)
+ * H = SHA-256(parent digest || tokens as little-endian int32), h_0 = SHA-256(seed as 8 little-endian bytes).
+ * Only full blocks have a hash: hashes_out_host receives (num_tokens / block_size) digests of 32 bytes. */
+int minipic_block_hashes(const int32_t* tokens_host, int32_t num_tokens, int32_t block_size, int32_t ssep_id,
+                         int32_t pdep_id, uint64_t seed, uint8_t* hashes_out_host);
+
+/* Block pool keyed by those digests (opaque host object, not thread safe; NULL on bad arguments). */
+typedef struct minipic_pool minipic_pool;
+minipic_pool* minipic_pool_create(int32_t num_blocks, int32_t block_size, int32_t ssep_id, int32_t pdep_id, uint64_t seed);
+void minipic_pool_destroy(minipic_pool* pool);
+/* Admit one request (a token stream, padded by the caller: PAPER.md:79).  For each of its ceil(n / B) blocks:
+ *   a cached digest  -> block_table_out[i] = that block, hit_out[i] = 1, slot_mapping_out = -1 for its tokens;
+ *   otherwise        -> a fresh block (free list in increasing id order, then the least recently released unreferenced
+ *                       block, whose digest is forgotten), hit_out[i] = 0, slot_mapping_out[t] = block * B + offset -
+ *                       exactly what minipic_cache_write / minipic_preattn_fused take for the tokens to be computed.
+ * A trailing partial block is never cached.  q_vis_lo_out[t] is the visibility descriptor of the attention calls
+ * (span token: first index of its SSEP block chain; before the first marker and from a PDEP block on: 0).
+ * Every block of the table holds one reference until minipic_pool_release.  MINIPIC_ERR_WORKSPACE_TOO_SMALL if the pool
+ * has no block left (the request's references are undone). */
+int minipic_pool_admit(minipic_pool* pool, const int32_t* tokens_host, int32_t num_tokens, int32_t* block_table_out,
+                       uint8_t* hit_out, int64_t* slot_mapping_out, int32_t* q_vis_lo_out, int32_t* num_new_tokens_out);
+int minipic_pool_release(minipic_pool* pool, const int32_t* block_table_host, int32_t num_blocks);
+void minipic_pool_stats(const minipic_pool* pool, uint64_t* hits, uint64_t* misses, uint64_t* evictions, int32_t* free_blocks);
+
 /* ---- misc ---------------------------------------------------------------------------------------*/
 const char* minipic_status_string(int status);
 /* Text of the last CUDA error seen by this thread inside the library ("" if none). */

@@ -33,6 +33,8 @@ EXPORTS = [
     "minipic_decode_host_arena_bytes", "minipic_decode_step_host",
     "minipic_status_string", "minipic_last_cuda_error", "minipic_launch_count", "minipic_last_variant",
     "minipic_prefill_status", "minipic_preattn_fused", "minipic_block_rerotate",
+    "minipic_block_hashes", "minipic_pool_create", "minipic_pool_destroy", "minipic_pool_admit", "minipic_pool_release",
+    "minipic_pool_stats",
 ]
 
 
@@ -91,6 +93,18 @@ def lib() -> C.CDLL:
     L.minipic_preattn_fused.argtypes = [P, VP, VP, VP, I32, VP, VP, VP, VP]
     L.minipic_block_rerotate.restype = C.c_int
     L.minipic_block_rerotate.argtypes = [P, VP, VP, VP, VP, VP, I32, VP]
+    L.minipic_block_hashes.restype = C.c_int
+    L.minipic_block_hashes.argtypes = [VP, I32, I32, I32, I32, C.c_uint64, VP]
+    L.minipic_pool_create.restype = VP
+    L.minipic_pool_create.argtypes = [I32, I32, I32, I32, C.c_uint64]
+    L.minipic_pool_destroy.restype = None
+    L.minipic_pool_destroy.argtypes = [VP]
+    L.minipic_pool_admit.restype = C.c_int
+    L.minipic_pool_admit.argtypes = [VP, VP, I32, VP, VP, VP, VP, VP]
+    L.minipic_pool_release.restype = C.c_int
+    L.minipic_pool_release.argtypes = [VP, VP, I32]
+    L.minipic_pool_stats.restype = None
+    L.minipic_pool_stats.argtypes = [VP, VP, VP, VP, VP]
     _lib = L
     return L
 
@@ -232,3 +246,57 @@ def minipic_last_variant() -> str:
 def minipic_prefill_status(workspace, stream=None) -> None:
     """Synchronises the stream and raises if the last tcgen05 prefill call on `workspace` recorded a barrier timeout."""
     _check(lib().minipic_prefill_status(_ptr(workspace), _stream(stream)))
+
+
+# ---- f3: host-side block hasher / pool (numpy arrays in host memory; argument marshalling only)
+def _np_ptr(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def minipic_block_hashes(tokens, block_size: int, ssep_id: int, pdep_id: int, seed: int = 0):
+    import numpy as np
+    tokens = np.ascontiguousarray(tokens, dtype=np.int32)
+    out = np.zeros((len(tokens) // block_size, 32), np.uint8)
+    _check(lib().minipic_block_hashes(_np_ptr(tokens), len(tokens), block_size, ssep_id, pdep_id, seed, _np_ptr(out)))
+    return out
+
+
+class Pool:
+    """Thin handle on a minipic_pool (Eq. 1 block pool); all logic lives in csrc/hasher.cu."""
+
+    def __init__(self, num_blocks: int, block_size: int, ssep_id: int, pdep_id: int, seed: int = 0):
+        self.block_size = block_size
+        self.h = lib().minipic_pool_create(num_blocks, block_size, ssep_id, pdep_id, seed)
+        if not self.h:
+            raise MinipicError(1)
+
+    def admit(self, tokens):
+        import numpy as np
+        tokens = np.ascontiguousarray(tokens, dtype=np.int32)
+        n, nb = len(tokens), -(-len(tokens) // self.block_size)
+        table, hit = np.zeros(nb, np.int32), np.zeros(nb, np.uint8)
+        slots, lo, n_new = np.zeros(n, np.int64), np.zeros(n, np.int32), C.c_int32(0)
+        _check(lib().minipic_pool_admit(self.h, _np_ptr(tokens), n, _np_ptr(table), _np_ptr(hit), _np_ptr(slots), _np_ptr(lo),
+                                        C.byref(n_new)))
+        return table, hit, slots, lo, int(n_new.value)
+
+    def release(self, table):
+        import numpy as np
+        table = np.ascontiguousarray(table, dtype=np.int32)
+        _check(lib().minipic_pool_release(self.h, _np_ptr(table), len(table)))
+
+    def stats(self):
+        h, m, e, f = C.c_uint64(0), C.c_uint64(0), C.c_uint64(0), C.c_int32(0)
+        lib().minipic_pool_stats(self.h, C.byref(h), C.byref(m), C.byref(e), C.byref(f))
+        return dict(hits=h.value, misses=m.value, evictions=e.value, free_blocks=f.value)
+
+    def close(self):
+        if self.h:
+            lib().minipic_pool_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -587,3 +587,60 @@ def test_block_rerotate_control(dtype):
     else:
         assert hv.tobytes() == vc.tobytes()
         assert np.abs(hk.astype(np.float64) - kc.astype(np.float64)).max() <= 4e-6
+
+
+def test_pool_derived_tables_end_to_end():
+    """f3 + f1 + the hot path, the paper's own procedure: documents are prefilled ONCE as separate
+    requests at positions 0.., final prompts in different orders cache-hit their unrotated blocks at other offsets.  Block
+    tables, slot mappings and q_vis_lo come from the C++ pool (GPU side) / the oracle pool (CPU side)."""
+    from paper_2606_13126_b200 import isps
+    rng = np.random.default_rng(31)
+    B, hq, hkv, d, theta, SSEP, PDEP, PAD = 16, 8, 2, 128, 5e5, 128001, 128002, 128000
+    system = rng.integers(0, 1000, 40)
+    corpus = [rng.integers(0, 1000, int(rng.integers(150, 420))) for _ in range(5)]
+    batches = [[(system, [corpus[i] for i in order], rng.integers(0, 1000, 37)) for order in ([0, 1, 2, 3], [3, 1, 4, 0], [2, 0, 1, 4])]]
+    ordered = isps.isps_order(batches, B, SSEP, PDEP, PAD)
+    nblk = 256
+    gpool, cpool = mp.Pool(nblk, B, SSEP, PDEP), N.Pool(nblk, B, SSEP, PDEP)
+    cfg = mp.make_config(num_q_heads=hq, num_kv_heads=hkv, head_dim=d, num_blocks=nblk, dtype="bf16", rope_theta=theta,
+                         flags=mp.MINIPIC_Q_PREROTATED)
+    gk = torch.full((nblk, hkv, 16, d), 0x7FC1, dtype=torch.int16, device="cuda"); gv = gk.clone()
+    kc = O.new_cache(nblk, hkv, 16, d, "bf16", 0x7FC1); vc = O.new_cache(nblk, hkv, 16, d, "bf16", 0x7FC1)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int16) if a.dtype == np.uint16 else np.ascontiguousarray(a)).cuda()
+    hits_in_finals = 0
+    for kind, toks in ordered:
+        n = len(toks)
+        table, hit, slots, lo, n_new = gpool.admit(toks)
+        t2, hit2, slots2, lo2 = cpool.admit(toks)
+        assert np.array_equal(table, t2) and np.array_equal(slots, slots2) and np.array_equal(lo, lo2)
+        new = np.flatnonzero(slots >= 0)
+        assert len(new) == n_new
+        if kind == "span":
+            assert n_new == n                                            # a span alone: everything is computed, once
+        else:
+            hits_in_finals += int(hit.sum())
+            assert n_new == 38 and hit[:-3].all() and not hit[-3:].any()  # only [PDEP, task] (38 tokens) is computed
+        qkv = W.f32_to_bf16_bits(rng.standard_normal((n_new, hq + 2 * hkv, d)).astype(np.float32))
+        pos = np.arange(n, dtype=np.int32)
+        # ---- GPU: fused pre-attention step, then prefill attention over the request's block table
+        q_rot = torch.zeros((n_new, hq, d), dtype=torch.int16, device="cuda")
+        cfg_rot = mp.make_config(num_q_heads=hq, num_kv_heads=hkv, head_dim=d, num_blocks=nblk, dtype="bf16", rope_theta=theta)
+        mp.minipic_preattn_fused(cfg_rot, dev(qkv), dev(slots[new]), dev(pos[new]), n_new, q_rot, gk, gv)
+        out = torch.zeros_like(q_rot); lse = torch.zeros((n_new, hq), dtype=torch.float32, device="cuda")
+        ws_bytes = mp.minipic_prefill_workspace_bytes(cfg, 1, n_new)
+        ws = torch.empty(max(ws_bytes, 256), dtype=torch.uint8, device="cuda")
+        mp.minipic_prefill_attention(cfg, q_rot, gk, gv, dev(table[None, :]), len(table), dev(np.array([0, n_new], np.int32)),
+                                     dev(np.array([n], np.int32)), dev(np.array([0, n], np.int32)), dev(pos),
+                                     dev(new.astype(np.int32)), dev(lo[new]), 1, n_new, n, out, lse, ws, ws_bytes)
+        torch.cuda.synchronize()
+        mp.minipic_prefill_status(ws)
+        # ---- oracle: scalar cache write + fp64 attention with in-attention rotation of the raw q
+        O.cache_write(kc, vc, qkv[:, hq:hq + hkv], qkv[:, hq + hkv:], slots[new])
+        of, lf = O.prefill_attention(q=qkv[:, :hq], k_cache=kc, v_cache=vc, block_tables=table[None, :],
+                                     cu_q_lens=np.array([0, n_new]), kv_lens=np.array([n]), cu_kv_lens=np.array([0, n]),
+                                     kv_positions=pos, q_seq_idx=new.astype(np.int32), q_vis_lo=lo[new], num_q_heads=hq,
+                                     dtype="bf16", rope_theta=theta)
+        do = np.abs(out.view(torch.bfloat16).double().cpu().numpy() - of); dl = np.abs(lse.double().cpu().numpy() - lf)
+        assert do.max() <= OUT_MAX and do.mean() <= OUT_MEAN and dl.mean() <= LSE_TOL, (kind, float(do.max()), float(dl.mean()))
+    assert gk.cpu().numpy().view(np.uint16).tobytes() == kc.tobytes() and gv.cpu().numpy().view(np.uint16).tobytes() == vc.tobytes()
+    assert hits_in_finals > 100
