@@ -164,6 +164,100 @@ def run_reference(args):
     return 0
 
 
+# ------------------------------------------------------------------------------------------- SURVEY 8(f) rows
+def next_rows_extras(torch, mp, W, DeviceWorkload, dev, peaks, time_calls):
+    """Measurements of the rows next to the hot path: f1 fused pre-attention step, f2 EPIC / LegoLink workload and the
+    key-masking variant, f3 ISPS replay through the C++ pool (host only), f4 copy-and-re-rotate control."""
+    ex = {}
+    to_dev = lambda a: torch.from_numpy(np.ascontiguousarray(a).view(np.int16) if a.dtype == np.uint16 else np.ascontiguousarray(a)).to(dev)
+    # ---- f1 on config 5's new tokens (every query token of config 5 is a new token): qkv [T, Hq + 2 Hkv, D]
+    w5 = W.config5()
+    nb = w5.new[0]
+    T, hq, hkv, d = w5.num_q_tokens, w5.num_q_heads, w5.num_kv_heads, w5.head_dim
+    assert nb.k.shape[0] == T
+    qkv = to_dev(np.concatenate([w5.q, nb.k, nb.v], axis=1)); del nb
+    pos = to_dev(np.concatenate([w5.kv_positions[int(w5.cu_kv_lens[r]):int(w5.cu_kv_lens[r + 1])][
+        w5.q_seq_idx[int(w5.cu_q_lens[r]):int(w5.cu_q_lens[r + 1])]] for r in range(w5.num_reqs)]).astype(np.int32))
+    d5 = DeviceWorkload(w5, device=dev)
+    slots = d5.new_dev[0][2]
+    q_out = torch.empty_like(d5.q)
+    f = lambda: mp.minipic_preattn_fused(d5.cfg, qkv, slots, pos, T, q_out, d5.k_cache, d5.v_cache)
+    t_f = time_calls(f, 20, 3, torch)
+    bytes_f = 2 * T * (hq + 2 * hkv) * d * 2                    # read qkv once, write q' + K + V once
+    t_w = time_calls(d5.write_new, 20, 3, torch)
+    t_a = time_calls(d5.attention, 10, 2, torch)
+    d5.q = q_out; d5.set_flags(mp.MINIPIC_Q_PREROTATED)
+    t_aq = time_calls(d5.attention, 10, 2, torch)
+    ex["f1_preattn_fused_c5"] = {"ms": t_f[0], "gbs": bytes_f / t_f[0] / 1e6, "frac_hbm_measured": bytes_f / t_f[0] / 1e6 / peaks["hbm_gbs"],
+                                 "algorithmic_bytes": bytes_f, "step_ms_cache_write_plus_inkernel_q_rope": t_w[0] + t_a[0],
+                                 "step_ms_fused_plus_q_prerotated": t_f[0] + t_aq[0],
+                                 "note": "the fused step also moves Q (read + write 2.2 GB); the paper's flow has that pass anyway (rotary layer)"}
+    del d5, qkv, q_out
+    w2 = W.config2()
+    nb2 = w2.new[0]
+    d2 = DeviceWorkload(w2, device=dev)
+    qkv2 = to_dev(np.concatenate([w2.q, nb2.k, nb2.v], axis=1)); pos2 = to_dev(w2.kv_positions[w2.q_seq_idx].astype(np.int32))
+    q2 = torch.empty_like(d2.q)
+    def step_plain():
+        d2.write_new(); d2.attention()
+    t_plain = time_calls(step_plain, 50, 5, torch)
+    q_raw = d2.q
+    def step_fused():
+        mp.minipic_preattn_fused(d2.cfg_rot, qkv2, d2.new_dev[0][2], pos2, w2.num_q_tokens, q2, d2.k_cache, d2.v_cache)
+        d2.attention()
+    d2.cfg_rot = d2.cfg
+    d2.q = q2; d2.set_flags(mp.MINIPIC_Q_PREROTATED)
+    t_fused = time_calls(step_fused, 50, 5, torch)
+    ex["f1_config2_step"] = {"ms_cache_write_then_prefill": t_plain[0], "ms_fused_preattn_then_prefill_q_prerotated": t_fused[0]}
+    del d2
+    # ---- f2: EPIC / LegoLink workload (link tokens of every document recomputed) and the key-masking variant on config 3
+    we = W.epic_linked_prefill()
+    de = DeviceWorkload(we, device=dev); de.step(); torch.cuda.synchronize()
+    te = time_calls(de.attention, 30, 3, torch); de.check_health()
+    ex["f2_epic_linked"] = {"ms": te[0], "query_tokens": we.num_q_tokens, "tokens_per_s": we.num_q_tokens / te[0] * 1e3,
+                            "tflops": we.attention_flops() / te[0] / 1e9, "link_tokens_per_document": 16}
+    del de
+    w3 = W.config3(); w3m = W.with_masked_keys(w3)
+    d3 = DeviceWorkload(w3m, device=dev, flags=mp.MINIPIC_KEY_MASK); d3.step(); torch.cuda.synchronize()
+    tm = time_calls(d3.attention, 30, 3, torch); d3.check_health()
+    d3.set_flags(0); t0 = time_calls(d3.attention, 30, 3, torch)
+    ex["f2_key_mask_c3"] = {"ms_masked": tm[0], "ms_same_input_flag_off": t0[0], "masked_keys": int((w3m.kv_positions < 0).sum())}
+    # ---- f4: what a position-dependent cache would have to do for config 3's cache hits: copy + re-rotate every cached block
+    nblk_hit = sum(int(w3.kv_lens[r]) for r in range(w3.num_reqs)) // 16 - w3.written_tokens() // 16
+    k2 = torch.randint(-20000, 20000, (2 * nblk_hit, w3.num_kv_heads, 16, w3.head_dim), dtype=torch.int16, device=dev)
+    v2 = torch.randint(-20000, 20000, (2 * nblk_hit, w3.num_kv_heads, 16, w3.head_dim), dtype=torch.int16, device=dev)
+    cfg2 = mp.make_config(num_q_heads=w3.num_q_heads, num_kv_heads=w3.num_kv_heads, head_dim=w3.head_dim, num_blocks=2 * nblk_hit,
+                          dtype="bf16", rope_theta=w3.rope_theta)
+    src = torch.randperm(nblk_hit, device=dev).to(torch.int32)                          # sources and destinations disjoint
+    dstb = (torch.randperm(nblk_hit, device=dev) + nblk_hit).to(torch.int32)
+    delta = torch.randint(-3000, 3000, (nblk_hit,), dtype=torch.int32, device=dev)
+    fr = lambda: mp.minipic_block_rerotate(cfg2, k2, v2, src, dstb, delta, nblk_hit)
+    tr = time_calls(fr, 20, 3, torch)
+    bytes_r = nblk_hit * w3.num_kv_heads * 16 * w3.head_dim * 2 * 2 * 2      # K and V, read + write
+    ex["f4_copy_and_rerotate_c3_hits"] = {"ms": tr[0], "gbs": bytes_r / tr[0] / 1e6, "frac_hbm_measured": bytes_r / tr[0] / 1e6 / peaks["hbm_gbs"],
+                                          "blocks": int(nblk_hit), "hbm_bytes_a_position_dependent_cache_adds": int(bytes_r),
+                                          "hbm_bytes_minipic_adds": 0, "c3_prefill_ms_for_scale": t0[0]}
+    del d3, k2, v2
+    # ---- f3: engine-less ISPS replay through the C++ pool (host only): what has to be prefilled with / without the markers
+    from paper_2606_13126_b200 import isps
+    rng = np.random.default_rng(7)
+    SSEP, PDEP, PAD, B = 128001, 128002, 128000, 16
+    system = rng.integers(0, 100000, 32)
+    corpus = [rng.integers(0, 100000, int(rng.integers(128, 512))) for _ in range(200)]
+    batches = [[(system, [corpus[i] for i in rng.choice(200, 10, replace=False)], rng.integers(0, 100000, 63)) for _ in range(32)]
+               for _ in range(4)]
+    tic = time.perf_counter()
+    ordered = isps.isps_order(batches, B, SSEP, PDEP, PAD)
+    st = isps.replay(mp.Pool(1 << 16, B, SSEP, PDEP), ordered, keep=32)
+    sec = time.perf_counter() - tic
+    plain = [(k, np.where((t == SSEP) | (t == PDEP), PAD, t).astype(np.int32)) for k, t in ordered if k == "final"]
+    st0 = isps.replay(mp.Pool(1 << 16, B, SSEP, PDEP), plain, keep=32)
+    ex["f3_isps_replay"] = {"requests": st["requests"], "tokens": st["tokens"], "prefilled_with_ssep_pdep": st["prefilled_tokens"],
+                            "prefilled_prefix_caching_only": st0["prefilled_tokens"], "final_prompt_prefilled": st["final_prompt_prefilled"],
+                            "host_seconds_hash_and_admit": sec, "host_tokens_per_s": st["tokens"] / sec}
+    return ex
+
+
 # ------------------------------------------------------------------------------------------- CUDA leg
 def time_calls(fn, iters, warmup, torch):
     for _ in range(warmup):
@@ -272,7 +366,7 @@ def run_ours(args):
             "scaling": "weak", "vs_baseline": None, "dtype": "bf16", "data": "synthetic",
             "config": {"workload": WORKLOAD, "parallelism": f"replicas x{world}" if world > 1 else "single GPU",
                        "l2": "inputs larger than L2: each step touches ~3.5 GB (Q/O 2.2 GB) between repeats of any kernel",
-                       "rope": "in-kernel K and Q rotation; cos/sin from an exact 64-bit fixed-point phase + MUFU (prefill adds an angle-addition recurrence; decode shares one (cos, sin) tile per 16-key block between the KV heads of a CTA)",
+                       "rope": "in-kernel K and Q rotation; cos/sin from an exact 64-bit fixed-point phase + MUFU (prefill adds an angle-addition recurrence; decode stages K / V blocks through per-warp TMA rings and rotates in registers)",
                        "tokens_per_step": tokens_per_step},
             "roofline": roofline, "roofline_decode": roofline_decode, "roofline_cache_write": roofline_cache_write,
             "kernels_ms": {"c5_cache_write": seg_mean[0], "c5_prefill": seg_mean[1], "c4_cache_write": seg_mean[2],
@@ -349,6 +443,7 @@ def run_ours(args):
                                          "resident_kv_bytes": wp.logical_kv_bytes(), "ms_prerotated": tpp[0],
                                          "rope_overhead": tp[0] / tpp[0] - 1.0}
             del dp, flush
+            extras.update(next_rows_extras(torch, mp, W, DeviceWorkload, dev, peaks, time_calls))
         except Exception as e:  # extras never break the contract line
             extras["error"] = repr(e)
         line["extras"] = extras
