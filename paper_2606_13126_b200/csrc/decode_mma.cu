@@ -40,11 +40,14 @@ __device__ __forceinline__ void mma16816(float (&d)[4], unsigned a0, unsigned a1
 // (common.cuh) -> signed half-turns -> MUFU sin/cos on the reduced angle in [-pi, pi) (|err| < 1e-6, far below the
 // bf16 rounding of the rotated operand).  No global-memory traffic: in this HBM-bound kernel a cos/sin table lookup
 // from global memory costs as many L1 wavefronts as the KV stream itself (ncu: l1tex 92% with the table).
-__device__ __forceinline__ void rope_cs8(const unsigned long long* __restrict__ finc, int p, int i0, float (&c)[8],
+// finc is PADDED: the 8 increments of frequency chunk c start at finc + 10 c (80 bytes apart), so that the four lane groups
+// of a warp (chunks 2 q4 + j) read four different bank groups instead of the same one (ncu: 4-way conflict otherwise).
+constexpr int kFincStride = 10;
+__device__ __forceinline__ void rope_cs8(const unsigned long long* __restrict__ finc, int p, int chunk, float (&c)[8],
                                          float (&s)[8]) {
 #pragma unroll
   for (int e = 0; e < 8; ++e) {
-    const unsigned long long ph = (unsigned long long)(unsigned)p * finc[i0 + e];
+    const unsigned long long ph = (unsigned long long)(unsigned)p * finc[chunk * kFincStride + e];
     const float a = (float)(int)(ph >> 32) * 1.4629180792671596e-9f;  // * pi * 2^-31 -> radians in [-pi, pi)
     c[e] = __cosf(a);
     s[e] = __sinf(a);
@@ -110,8 +113,8 @@ decode_mma_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_const
   // [W warps][kStages][K 4 KB | V 4 KB] | F_i[64] | barriers[W * kStages]
   extern __shared__ __align__(1024) unsigned char smem_raw[];
   unsigned long long* finc = reinterpret_cast<unsigned long long*>(smem_raw + W * kStages * kStageBytes);  // 64-bit phase increments
-  unsigned long long* bars = finc + 64;
-  for (int i = threadIdx.x; i < 64; i += 32 * W) finc[i] = rp.phase_inc[i];
+  unsigned long long* bars = finc + 8 * kFincStride;
+  for (int i = threadIdx.x; i < 64; i += 32 * W) finc[(i >> 3) * kFincStride + (i & 7)] = rp.phase_inc[i];
   if (threadIdx.x == 0) {
     if (smem_addr(smem_raw) & 1023u) __trap();
     for (int i = 0; i < W * kStages; ++i) mbar_init(smem_addr(&bars[i]), 1);
@@ -143,7 +146,7 @@ decode_mma_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_const
 #pragma unroll
         for (int j = 0; j < 2; ++j) {
           float c[8], sn[8];
-          rope_cs8(finc, qpos, (2 * q4 + j) * 8, c, sn);
+          rope_cs8(finc, qpos, 2 * q4 + j, c, sn);
           rotate_chunks(ch[j], ch[j + 2], c, sn);
         }
       }
@@ -167,15 +170,18 @@ decode_mma_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_const
   const uint32_t ring = smem_addr(smem_raw) + (uint32_t)warp * (kStages * kStageBytes);
   const uint32_t bar0 = smem_addr(&bars[warp * kStages]);
   // a4: block n of the split -> stage n % kStages (lane 0 only): one 4 KB box of K and one of V through the block table
-  auto issue = [&](int n) {
+  auto issue = [&](int n, int blk) {
     const int st = n % kStages;
-    const int grp = (__ldg(bt + kb0 + n) * hkv + kvh) * 2;   // row-group coordinate of (block, head) in the cache tensor map
+    const int grp = (blk * hkv + kvh) * 2;   // row-group coordinate of (block, head) in the cache tensor map
     mbar_expect_tx(bar0 + 8u * st, kStageBytes);
     tma_block(ring + st * kStageBytes, &tmap_k, bar0 + 8u * st, grp);
     tma_block(ring + st * kStageBytes + 4096, &tmap_v, bar0 + 8u * st, grp);
   };
-  if (lane == 0)
-    for (int n = 0; n < kStages - 1 && n < nb; ++n) issue(n);
+  int blk_next = 0;   // lane 0: physical block of the next block to issue, read from the block table one iteration early
+  if (lane == 0) {
+    for (int n = 0; n < kStages - 1 && n < nb; ++n) issue(n, __ldg(bt + kb0 + n));
+    if (kStages - 1 < nb) blk_next = __ldg(bt + kb0 + kStages - 1);
+  }
 
   // swizzled offsets of this lane's chunks inside a 4 KB block image: [row group (2)][half (2)][8 rows x 128 B], SWIZZLE_128B
   uint32_t koff[2];   // K rows g (group 0) and g + 8 (group 1) share the in-group offset: chunk 2 q4 + j of row g
@@ -188,12 +194,20 @@ decode_mma_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_const
     voff[i] = (uint32_t)((i >> 1) * 2048 + row * 128 + ((g ^ row) << 4));
   }
 
+  int pcur[2] = {0, 0};   // logical positions of this lane's rows g, g + 8 of the current block
+  if (kRotK) {
+#pragma unroll
+    for (int t = 0; t < 2; ++t) pcur[t] = __ldg(pos + min(kb0 * kBlock + g + 8 * t, kv_len - 1));
+  }
 #pragma unroll 1
   for (int n = 0; n < nb; ++n) {
     const int kb = kb0 + n;
     // every lane is done with the stage that block n + kStages - 1 reuses (it held block n - 1): refill it
     __syncwarp();
-    if (lane == 0 && n + kStages - 1 < nb) issue(n + kStages - 1);
+    if (lane == 0 && n + kStages - 1 < nb) {
+      issue(n + kStages - 1, blk_next);
+      if (n + kStages < nb) blk_next = __ldg(bt + kb0 + n + kStages);
+    }
     // a5 (first half): cos/sin of this lane's two rows, computed while the block is still in flight
     float cs[2][2][8], sn[2][2][8];
     // Measured and dropped: row g + 8 from row g by one angle-addition step with a (cos 8 f, sin 8 f) table in shared
@@ -202,10 +216,13 @@ decode_mma_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_const
     if (kRotK) {
 #pragma unroll
       for (int t = 0; t < 2; ++t) {
-        const int p = __ldg(pos + min(kb * kBlock + g + 8 * t, kv_len - 1));
 #pragma unroll
-        for (int j = 0; j < 2; ++j) rope_cs8(finc, p, (2 * q4 + j) * 8, cs[t][j], sn[t][j]);
+        for (int j = 0; j < 2; ++j) rope_cs8(finc, pcur[t], 2 * q4 + j, cs[t][j], sn[t][j]);
       }
+      // positions of the NEXT block's two rows: a global load whose latency would otherwise sit at the top of every
+      // iteration (ncu: 12 % of the stall samples were long-scoreboard waits on it)
+#pragma unroll
+      for (int t = 0; t < 2; ++t) pcur[t] = __ldg(pos + min((kb + 1) * kBlock + g + 8 * t, kv_len - 1));
     }
     const uint32_t stg = ring + (n % kStages) * kStageBytes;
     mbar_wait(bar0 + 8u * (n % kStages), (n / kStages) & 1);
@@ -320,7 +337,7 @@ decode_mma_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_const
 template <bool kRotK, bool kKeyMask, int W>
 bool launch_k(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, const CUtensorMap& mk, const CUtensorMap& mv,
               float* o_part, float* lse_part) {
-  const size_t smem = (size_t)W * kStages * kStageBytes + 64 * 8 + (size_t)W * kStages * 8;
+  const size_t smem = (size_t)W * kStages * kStageBytes + 8 * kFincStride * 8 + (size_t)W * kStages * 8;
   static bool attr_done[64] = {};   // per (function, device)
   int dev = 0;
   cudaGetDevice(&dev);
