@@ -39,7 +39,13 @@ constexpr int kHalfBytes = kTileBytes / 2;   // [half of head_dim][128 rows][128
 constexpr int kKeysCta = BN / 2;
 constexpr int kKTileBytes = kKeysCta * D * 2;    // 8 row groups of [half (2)][8 rows x 128 B]
 constexpr int kVTileBytes = BN * (D / 2) * 2;    // 16 row groups of [8 rows x 128 B] (this CTA's half of head_dim)
-constexpr int kKStages = 3, kVStages = 3, kRing = 4;
+#ifndef MINIPIC_KSTAGES
+#define MINIPIC_KSTAGES 3
+#endif
+#ifndef MINIPIC_VSTAGES
+#define MINIPIC_VSTAGES 3
+#endif
+constexpr int kKStages = MINIPIC_KSTAGES, kVStages = MINIPIC_VSTAGES, kRing = 4;
 // Measured and dropped (config 5, in-kernel RoPE; the kept version runs 2.24 ms):
 //  * a ring of three Q tile slots (next item's tile A loaded + rotated during the current item, epilogue staged in the
 //    finishing item's tile-B slot): parity-green, dense +3 %, but span items -7 % (2.30 ms): the four rotation warps are
