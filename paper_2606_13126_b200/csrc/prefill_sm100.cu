@@ -62,6 +62,17 @@ constexpr int kKStages = MINIPIC_KSTAGES, kVStages = MINIPIC_VSTAGES, kRing = 4;
 //    separate max pass saves;  second half of S loaded from TMEM under the first half's max: no change;
 //  * mbarrier.try_wait with a suspend-time hint (500 / 4000 ns) to take the wait loops (44 % of the issued instructions)
 //    off the issue slots: no change on dense tiles, 2 % slower on config 5 - try_wait already sleeps in hardware.
+// Measured and dropped on the CTA-pair kernel (config 5 at 2.04 ms, all parity-green):
+//  * Q double buffer + Q rotation by the rotation warps one item ahead + epilogue staged in the finished item's Q buffer +
+//    "resident" items (several 64-token sub-items over K tiles gathered and rotated once): 2.27 ms.  Four rotation warps
+//    need ~7.5 K cycles for the 256 Q rows of a sub-item (latency-bound at ~470 cycles per 4-row step whether rolled or
+//    unrolled), longer than a short sub-item lasts, and with Q and K both pre-rotated the structure still ran 2.04 ms;
+//  * P in shared memory (SS-mode PV) so that QK^T of tile i + 1 is issued as soon as S(i) is in registers and runs under the
+//    softmax of tile i: 2.05 ms, dense causal input 1058 -> 1025 TFLOP/s.  The softmax warps then wait for PV(i) (P buffer,
+//    O rescale) instead of for S(i + 1): the two tile slots run in phase and share the scheduler's MUFU / issue rate, which
+//    is what bounds the period, not the dependency chain;
+//  * named-barrier ping-pong that makes the tile-A and tile-B warps of a scheduler take turns in the exp phase: 2.09 ms;
+//  * 2, 3 or 4 K / V stages: 2.034 - 2.048 ms (no effect).
 // Two restructurings of the softmax were measured on config 5 (2.38 ms at the time) and dropped:
 //  * every 2nd / 3rd / 4th exp2 pair on the FMA pipe (Cody-Waite + cubic minimax) instead of MUFU: 2.59 / 2.56 / 2.45 ms -
 //    the softmax warps are issue / latency bound, not MUFU bound, at this tile period;
