@@ -219,10 +219,6 @@ decode_mma_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_const
 #pragma unroll
         for (int j = 0; j < 2; ++j) rope_cs8(finc, pcur[t], 2 * q4 + j, cs[t][j], sn[t][j]);
       }
-      // positions of the NEXT block's two rows: a global load whose latency would otherwise sit at the top of every
-      // iteration (ncu: 12 % of the stall samples were long-scoreboard waits on it)
-#pragma unroll
-      for (int t = 0; t < 2; ++t) pcur[t] = __ldg(pos + min((kb + 1) * kBlock + g + 8 * t, kv_len - 1));
     }
     const uint32_t stg = ring + (n % kStages) * kStageBytes;
     mbar_wait(bar0 + 8u * (n % kStages), (n / kStages) & 1);
@@ -239,6 +235,13 @@ decode_mma_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_const
 #pragma unroll
         for (int j = 0; j < 2; ++j) rotate_chunks(kr[t][j], kr[t][j + 2], cs[t][j], sn[t][j]);
     }
+    // positions of the NEXT block's two rows: a global load whose latency would otherwise sit at the top of every iteration
+    // (ncu: 12 % of the stall samples were long-scoreboard waits on it).  Issued here, where the cos / sin registers are dead
+    // (issued before the rotation it spilled to local memory).
+    if (kRotK) {
+#pragma unroll
+      for (int t = 0; t < 2; ++t) pcur[t] = __ldg(pos + min((kb + 1) * kBlock + g + 8 * t, kv_len - 1));
+    }
     // ---- a6: S^T[head, key] for the two 8-key halves of the block
     float st[2][4];
 #pragma unroll
@@ -253,13 +256,14 @@ decode_mma_kernel(const __grid_constant__ CUtensorMap tmap_k, const __grid_const
     // ---- V rows 2q, 2q+1, 2q+8, 2q+9, chunk g of both halves
     uint4 vr[4][2];
 #pragma unroll
-    for (int i = 0; i < 4; ++i) {
-      const int jrow = kb * kBlock + 2 * q4 + (i & 1) + 8 * (i >> 1);
-      const bool ok = jrow >= j_begin && jrow < j_end;  // never multiply P = 0 with uninitialised cache bits
+    for (int i = 0; i < 4; ++i)
 #pragma unroll
-      for (int hf = 0; hf < 2; ++hf) {
-        const uint4 v = lds128(stg + 4096 + hf * 1024 + voff[i]);
-        vr[i][hf] = ok ? v : make_uint4(0, 0, 0, 0);
+      for (int hf = 0; hf < 2; ++hf) vr[i][hf] = lds128(stg + 4096 + hf * 1024 + voff[i]);
+    if (kb * kBlock < j_begin || (kb + 1) * kBlock > j_end) {   // only the first / last block of a split (warp-uniform):
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {                              // never multiply P = 0 with uninitialised cache bits
+        const int jrow = kb * kBlock + 2 * q4 + (i & 1) + 8 * (i >> 1);
+        if (jrow < j_begin || jrow >= j_end) { vr[i][0] = make_uint4(0, 0, 0, 0); vr[i][1] = make_uint4(0, 0, 0, 0); }
       }
     }
     // ---- a7: mask + online softmax (row = head g; its 16 scores live in 4 lanes x 4 registers)
