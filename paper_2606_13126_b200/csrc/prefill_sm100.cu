@@ -40,10 +40,10 @@ constexpr int kKeysCta = BN / 2;
 constexpr int kKTileBytes = kKeysCta * D * 2;    // 8 row groups of [half (2)][8 rows x 128 B]
 constexpr int kVTileBytes = BN * (D / 2) * 2;    // 16 row groups of [8 rows x 128 B] (this CTA's half of head_dim)
 #ifndef MINIPIC_KSTAGES
-#define MINIPIC_KSTAGES 3
+#define MINIPIC_KSTAGES 2
 #endif
 #ifndef MINIPIC_VSTAGES
-#define MINIPIC_VSTAGES 3
+#define MINIPIC_VSTAGES 2
 #endif
 constexpr int kKStages = MINIPIC_KSTAGES, kVStages = MINIPIC_VSTAGES, kRing = 4;
 // Measured and dropped (config 5, in-kernel RoPE; the kept version runs 2.24 ms):
@@ -90,6 +90,7 @@ constexpr int kThreads = 512;
 constexpr int kRegsSoftmax = 184, kRegsRot = 96, kRegsCtl = 48;
 static_assert(256 * kRegsSoftmax + 128 * kRegsRot + 128 * kRegsCtl <= 65536, "setmaxnreg split exceeds the CTA register pool");
 constexpr int kMaxBins = 4096;
+constexpr int kDualMinTiles = 4;   // a "dual" item (see struct Item) needs at least this many KV tiles
 constexpr unsigned kWaitMaxSpins = 1u << 26;   // x (>= 30 cycles per failed try_wait) = seconds
 
 struct TileDesc { int t0, ntok, r, idx0, lo, n_kv, kv_hi, kv_len, kv_off, pad; };   // kv_off = cu_kv_lens[r]
@@ -328,7 +329,8 @@ __device__ __forceinline__ bool tile_starts(const PrefillArgs& a, int t, int r, 
 // to finish (ticket) turns the histogram into offsets in DESCENDING cost order and scatters the descriptors: a counting
 // sort, longest item first, that the persistent kernel's atomic work counter then walks.
 constexpr int kPlanThreads = 256, kPlanMaxTok = 512;   // tok = 4 * 128 / G <= 512
-__global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, int tok, PlanHeader* hdr, TileDesc* tmp, TileDesc* sorted) {
+__device__ __forceinline__ int tile_cost(const TileDesc& td) { return td.pad ? (td.n_kv + 1) >> 1 : td.n_kv; }   // tile steps
+__global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, int tok, int dual_ok, PlanHeader* hdr, TileDesc* tmp, TileDesc* sorted) {
   constexpr int kWords = (kPlanThreads + kPlanMaxTok) / 32;
   __shared__ unsigned sflag[kWords];
   __shared__ int s_last;
@@ -370,12 +372,13 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, int t
     TileDesc td;
     td.t0 = t; td.ntok = n; td.r = r; td.idx0 = __ldg(a.q_seq_idx + t); td.lo = max(__ldg(a.q_vis_lo + t), 0);
     td.kv_len = __ldg(a.kv_lens + r);
-    td.kv_off = __ldg(a.cu_kv_lens + r); td.pad = 0;
+    td.kv_off = __ldg(a.cu_kv_lens + r);
     const int kv_lo = td.lo & ~(kBlock - 1);
     td.kv_hi = min(td.idx0 + n, td.kv_len);
     td.n_kv = td.kv_hi > kv_lo ? (td.kv_hi - kv_lo + BN - 1) / BN : 0;
+    td.pad = (dual_ok && 2 * n <= tok && td.n_kv >= kDualMinTiles) ? 1 : 0;   // dual item: at most 2 TOK tokens over a long KV range
     tmp[atomicAdd(&hdr->n_tiles, 1)] = td;
-    atomicAdd(&hdr->hist[min(td.n_kv, kMaxBins - 1)], 1);
+    atomicAdd(&hdr->hist[min(tile_cost(td), kMaxBins - 1)], 1);
   }
   // ---- last block: counting sort of all descriptors, longest first
   __threadfence();
@@ -411,7 +414,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, int t
 #pragma unroll
       for (int e = 0; e < (int)(sizeof(TileDesc) / sizeof(int)); ++e) dst[e] = __ldcg(src + e);
     }
-    sorted[atomicAdd(&hdr->hist[min(td.n_kv, kMaxBins - 1)], 1)] = td;
+    sorted[atomicAdd(&hdr->hist[min(tile_cost(td), kMaxBins - 1)], 1)] = td;
   }
 }
 
@@ -421,7 +424,9 @@ struct Smem {
   alignas(1024) unsigned char k[kKStages][kKTileBytes];
   alignas(1024) unsigned char v[kVStages][kVTileBytes];
   alignas(1024) unsigned char ostage[8][kStageBytes];
-  unsigned long long bars[48];
+  alignas(1024) float xchg[BM][D];                    // dual items: O_B rows (fp32) on their way to the A warps, 16-byte chunks XOR-swizzled by row
+  float2 xml[BM];                                     // ... and (m_B, l_B)
+  unsigned long long bars[36];
   alignas(16) ItemInfo ring[kRing];
   alignas(16) unsigned long long finc[64];   // F_i (common.cuh), read by the rotation lanes at every exact restart
   alignas(16) float2 step1[64];              // (cos f_i, sin f_i): one-position step, used by the Q rotation
@@ -448,9 +453,10 @@ enum Bar {
   P_FULL = S_FULL + 2,                  // [2] leader, 4 softmax warps per CTA
   O_FULL = P_FULL + 2,                  // [2] multicast
   O_FREE = O_FULL + 2,                  // [2] leader, 4 softmax warps per CTA
-  NUM_BARS = O_FREE + 2
+  XCHG = O_FREE + 2,                    // local, 128 tile-B softmax threads: (O_B, m_B, l_B) of a dual item are in shared memory
+  NUM_BARS
 };
-static_assert(NUM_BARS <= 48, "barrier array too small");
+static_assert(NUM_BARS <= 36, "barrier array too small");
 static_assert(sizeof(Smem) <= 232448, "shared memory budget");
 static_assert(sizeof(ItemInfo) == 48, "ring entries are copied to the peer CTA as three 16-byte stores");
 
@@ -462,6 +468,7 @@ struct Params {
   PlanHeader* hdr;
   const TileDesc* tiles;
   int oob_grp;                       // first row-group coordinate beyond the cache tensor map: TMA zero-fills
+  int dual_ok;                       // the plan may make dual items (host decision from scalars: small grids only)
   unsigned long long phase_inc[64];  // F_i (common.cuh)
   float2 step1[64];                  // (cos f_i, sin f_i)
   float2 step4[64];                  // (cos 4 f_i, sin 4 f_i): the four-position RoPE step of the rotation lanes
@@ -470,22 +477,38 @@ struct Params {
 // A work item as one CTA of the pair sees it.  The item covers up to 4 * TOK query tokens (TOK = 128 / G tokens fill one
 // 128-row MMA tile): CTA rank c owns tokens [2 c TOK, 2 c TOK + 2 TOK) of it, tile A the first TOK of those, tile B the rest.
 // Both CTAs run the SAME number of KV tiles for a tile slot (the MMA covers both); rows a CTA does not own are masked.
+// DUAL items (short Q, long KV: ntok <= 2 TOK and n_kv >= kDualMinTiles, chosen by the plan): the two tile slots of a CTA hold
+// the SAME query rows (CTA rank c owns tokens [c TOK, c TOK + TOK)) and split the KV range - slot A runs tiles [0, n_a), slot B
+// tiles [n_a, n_kv) - so a 64-token suffix over a long context takes half as many tile steps and keeps both CTAs busy.  The
+// K / V "uses" are interleaved in the order the MMA issuer consumes them: use u = 2 j + x is tile j of slot x.  At the end
+// the B warps hand (O_B, m_B, l_B) to the A warps through shared memory and those merge the two partial softmaxes.
 struct Item {
   int t0, ntok, r, idx0, lo, kvh, n_kv, kv_hi, kv_len, kv_off;
-  int kv_lo, tb, ntok_a, ntok_b, n_b;
+  int kv_lo, tb, ntok_a, ntok_b, n_a, n_b;
+  bool dual;
   __device__ __forceinline__ int ntok_x(int x) const { return x ? ntok_b : ntok_a; }
-  __device__ __forceinline__ int n_x(int x) const { return x ? n_b : n_kv; }   // tile B is skipped by the whole pair if empty
+  __device__ __forceinline__ int n_x(int x) const { return x ? n_b : n_a; }   // KV tiles slot x runs (0: the pair skips the slot)
+  __device__ __forceinline__ int tile_x(int x, int i) const { return (dual && x) ? n_a + i : i; }      // i-th KV tile of slot x
+  __device__ __forceinline__ int tile_of_use(int u) const { return dual ? ((u & 1) ? n_a + (u >> 1) : (u >> 1)) : u; }
+  __device__ __forceinline__ int tok_x(int x, int tok_per_tile) const { return dual ? tb : tb + x * tok_per_tile; }   // first token of slot x
 };
-template <int TOK>
+template <int TOK, bool kDual>
 __device__ __forceinline__ Item load_item(const ItemInfo& ii, int rank) {
   Item it;
   it.t0 = ii.t0; it.ntok = ii.ntok; it.r = ii.r; it.idx0 = ii.idx0; it.lo = ii.lo; it.kvh = ii.kvh; it.n_kv = ii.n_kv;
   it.kv_hi = ii.kv_hi; it.kv_len = ii.kv_len; it.kv_off = ii.kv_off;
   it.kv_lo = it.lo & ~(kBlock - 1);
-  it.tb = rank * 2 * TOK;
-  const int mine = min(max(it.ntok - it.tb, 0), 2 * TOK);
-  it.ntok_a = min(mine, TOK); it.ntok_b = mine - it.ntok_a;
-  it.n_b = it.ntok > TOK ? it.n_kv : 0;
+  it.dual = kDual && ii.pad[0] != 0;   // kDual = false: a compile-time constant, every dual branch folds away
+  if (it.dual) {
+    it.tb = rank * TOK;
+    it.ntok_a = it.ntok_b = min(max(it.ntok - it.tb, 0), TOK);
+    it.n_a = (it.n_kv + 1) >> 1; it.n_b = it.n_kv - it.n_a;
+  } else {
+    it.tb = rank * 2 * TOK;
+    const int mine = min(max(it.ntok - it.tb, 0), 2 * TOK);
+    it.ntok_a = min(mine, TOK); it.ntok_b = mine - it.ntok_a;
+    it.n_a = it.n_kv; it.n_b = it.ntok > TOK ? it.n_kv : 0;
+  }
   return it;
 }
 
@@ -538,7 +561,9 @@ struct Rot8 {
   }
 };
 
-template <int G, bool kKeyMask>   // kKeyMask: MINIPIC_KEY_MASK variant (its own instantiation: the common path pays nothing)
+// kKeyMask: MINIPIC_KEY_MASK variant; kDual: dual items possible (the plan only makes them on small grids).  Both are their own
+// instantiations, so the common path (config 5) pays nothing for either.
+template <int G, bool kKeyMask, bool kDual>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kThreads, 1)
 prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_constant__ CUtensorMap tmap_k,
                      const __grid_constant__ CUtensorMap tmap_v, const __grid_constant__ CUtensorMap tmap_o,
@@ -570,6 +595,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
     for (int x = 0; x < 2; ++x) {
       mbar_init(bar(S_FULL + x), 1); mbar_init(bar(P_FULL + x), 8); mbar_init(bar(O_FULL + x), 1); mbar_init(bar(O_FREE + x), 8);
     }
+    mbar_init(bar(XCHG), 128);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   if (warp == 13) {  // TMEM: 512 columns = S_A | S_B | O_A | O_B, 128 each; P_X aliases the first 64 columns of S_X.
@@ -602,11 +628,12 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
             ii.kv_hi = td.kv_hi; ii.kv_len = td.kv_len; ii.kv_off = td.kv_off;
           }
           ii.pad[0] = ii.pad[1] = 0;
+          if (item < n_items) ii.pad[0] = prm.tiles[item / prm.hkv].pad;
           sm.ring[slot] = ii;
           const uint32_t dst = ring_p + (uint32_t)slot * (uint32_t)sizeof(ItemInfo);
           st_cluster_v4(dst, ii.t0, ii.ntok, ii.r, ii.idx0);
           st_cluster_v4(dst + 16, ii.lo, ii.kvh, ii.n_kv, ii.kv_hi);
-          st_cluster_v4(dst + 32, ii.kv_len, ii.kv_off, 0, 0);
+          st_cluster_v4(dst + 32, ii.kv_len, ii.kv_off, ii.pad[0], 0);
           mbar_arrive_cl_release(lbar(SCHED_FULL + slot));
           mbar_arrive_cl_release(full_p + 8u * (uint32_t)slot);
           TRACE(0, 1);
@@ -621,14 +648,15 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         const int slot = it_n & (kRing - 1);
         w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
         if (__any_sync(0xffffffffu, w.dead) || sm.ring[slot].t0 < 0) break;
-        const int n = sm.ring[slot].n_kv, kv_hi = sm.ring[slot].kv_hi;
+        const Item it = load_item<TOK, kDual>(sm.ring[slot], rank);
+        const int n = it.n_kv;
         __syncwarp();
         if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
-        const bool vfix = (kv_hi & (kBlock - 1)) != 0;
-        for (int i = 0; i < n; ++i, ++vc) {
+        const bool vfix = (it.kv_hi & (kBlock - 1)) != 0;
+        for (int i = 0; i < n; ++i, ++vc) {   // i = use index (see struct Item)
           const int st = vc % kVStages;
           w.wait(bar(V_FULL + st), (vc / kVStages) & 1);
-          if (i == n - 1 && vfix) { w.wait(bar(V_FIX), fixc & 1); ++fixc; }
+          if (it.tile_of_use(i) == n - 1 && vfix) { w.wait(bar(V_FIX), fixc & 1); ++fixc; }
           __syncwarp();
           if (lane == 0) mbar_arrive_cl(lbar(V_PEER + st));
         }
@@ -640,7 +668,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         const int slot = it_n & (kRing - 1);
         w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
         if (__any_sync(0xffffffffu, w.dead) || sm.ring[slot].t0 < 0) break;
-        const Item it = load_item<TOK>(sm.ring[slot], rank);
+        const Item it = load_item<TOK, kDual>(sm.ring[slot], rank);
         __syncwarp();
         if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
         if (it.n_kv == 0) continue;
@@ -650,10 +678,10 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           const int b = (it.kv_lo >> 4) + i * (BN / kBlock) + rank * (kKeysCta / kBlock) + lane;
           return (lane < kKeysCta / kBlock && b < nblk_total) ? (__ldg(bt + b) * prm.hkv + it.kvh) * 2 : prm.oob_grp;
         };
-        int y = block_grp(0);
-        for (int i = 0; i < it.n_kv; ++i) {
-          const int y_next = (i + 1 < it.n_kv) ? block_grp(i + 1) : 0;
-          {  // K tile i: one 4 KB box per physical block
+        int y = block_grp(it.tile_of_use(0));
+        for (int i = 0; i < it.n_kv; ++i) {   // i = use index: tile it.tile_of_use(i)
+          const int y_next = (i + 1 < it.n_kv) ? block_grp(it.tile_of_use(i + 1)) : 0;
+          {  // one K tile: one 4 KB box per physical block
             const int st = kc % kKStages;
             if (lane == 0) { w.wait(bar(K_EMPTY + st), ((kc / kKStages) & 1) ^ 1); if (!w.dead) mbar_expect_tx(bar(K_FULL + st), kKTileBytes); }
             if (__any_sync(0xffffffffu, w.dead)) break;   // a timed-out wait: stop issuing, let the kernel drain
@@ -662,7 +690,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
             TRACE_L0(0, 2);
           }
           if (i == 0) {  // this CTA's Q rows: (token, head-in-group), tile A then tile B
-            const int ntile = it.ntok_b > 0 ? 2 : (it.ntok_a > 0 ? 1 : 0);
+            const int ntile = it.dual ? (it.ntok_a > 0 ? 1 : 0) : (it.ntok_b > 0 ? 2 : (it.ntok_a > 0 ? 1 : 0));   // dual: both slots read tile 0
             if (lane == 0) { w.wait(bar(Q_EMPTY), (qc & 1) ^ 1); if (!w.dead) mbar_expect_tx(bar(Q_FULL), ntile * kTileBytes); }
             if (__any_sync(0xffffffffu, w.dead)) break;
             if (lane < 2 * ntile) {
@@ -683,6 +711,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
         if (__any_sync(0xffffffffu, w.dead) || sm.ring[slot].t0 < 0) break;
         const ItemInfo ii = sm.ring[slot];
+        const Item itv = load_item<TOK, kDual>(sm.ring[slot], rank);
         __syncwarp();
         if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
         if (ii.n_kv == 0) continue;
@@ -693,9 +722,9 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           const int b = (kv_lo >> 4) + i * (BN / kBlock) + lane;
           return (lane < BN / kBlock && b < nblk_total) ? (__ldg(bt + b) * prm.hkv + ii.kvh) * 2 : prm.oob_grp;
         };
-        int y = block_grp(0);
-        for (int i = 0; i < ii.n_kv; ++i) {
-          const int y_next = (i + 1 < ii.n_kv) ? block_grp(i + 1) : 0;
+        int y = block_grp(itv.tile_of_use(0));
+        for (int i = 0; i < ii.n_kv; ++i) {   // i = use index
+          const int y_next = (i + 1 < ii.n_kv) ? block_grp(itv.tile_of_use(i + 1)) : 0;
           const int st = vc % kVStages;
           if (lane == 0) { w.wait(bar(V_EMPTY + st), ((vc / kVStages) & 1) ^ 1); if (!w.dead) mbar_expect_tx(bar(V_FULL + st), kVTileBytes); }
           if (__any_sync(0xffffffffu, w.dead)) break;
@@ -721,19 +750,20 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         const int slot = it_n & (kRing - 1);
         w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
         if (__any_sync(0xffffffffu, w.dead) || sm.ring[slot].t0 < 0) break;
-        int n, nx1, kv_hi;
+        int n, nx1, kv_hi, dual;
         {
-          const Item it = load_item<TOK>(sm.ring[slot], 0);
+          const Item it = load_item<TOK, kDual>(sm.ring[slot], 0);
           n = __shfl_sync(0xffffffffu, it.n_kv, 0);
           nx1 = __shfl_sync(0xffffffffu, it.n_b, 0); kv_hi = __shfl_sync(0xffffffffu, it.kv_hi, 0);
+          dual = __shfl_sync(0xffffffffu, (int)it.dual, 0);
         }
         const bool vfix = (kv_hi & (kBlock - 1)) != 0;
         __syncwarp();
         if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
         if (n == 0) continue;
         // QK^T of tile x against K stage st: S_x = Q_x K'^T for both CTAs (elected lane only)
-        auto qk = [&](int x, uint32_t st) {
-          const uint32_t a_lo = q_lo + (uint32_t)x * (kTileBytes >> 4), b_lo = k_lo + st * (kKTileBytes >> 4);
+        auto qk = [&](int x, uint32_t st) {   // dual items: both slots read Q tile 0 (the same rows)
+          const uint32_t a_lo = q_lo + (uint32_t)(dual ? 0 : x) * (kTileBytes >> 4), b_lo = k_lo + st * (kKTileBytes >> 4);
 #pragma unroll
           for (int ks = 0; ks < D / 16; ++ks) {
             const uint32_t off_q = (ks >> 2) * (kHalfBytes >> 4) + (ks & 3) * 2, off_k = (ks >> 2) * (kKvHalfOff >> 4) + (ks & 3) * 2;
@@ -742,6 +772,52 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           tc_commit(bar(S_FULL + x));
           TRACE(1, 10 + x);
         };
+        if (dual) {
+          // ---- dual item: K / V uses alternate between the slots (use u = 2 j + x is tile j of slot x); n_a = n - nx1 >= nx1
+          const int n_a = n - nx1;
+          auto k_next = [&]() { if (++k_st == kKStages) { k_st = 0; k_ph ^= 1; } };
+          auto issue_qk = [&](int x, int u) {   // QK^T of slot x against K use u (the next one in the ring), then release it
+            w.wait(bar(K_READY + k_st), k_ph);
+            tc_fence_after();
+            if (elect_one()) {
+              qk(x, k_st);
+              tc_commit(bar(K_EMPTY + k_st));
+              if (u == n - 1) tc_commit(bar(Q_EMPTY));   // the item's last QK^T
+            }
+            __syncwarp();
+            k_next();
+          };
+          w.wait(bar(Q_READY), (ph >> 4) & 1);
+          w.wait(bar(Q_READY + 1), (ph >> 4) & 1); ph ^= 16u;
+          issue_qk(0, 0);
+          issue_qk(1, 1);
+#pragma unroll 1
+          for (int j = 0; j < n_a; ++j) {
+#pragma unroll 1
+            for (int x = 0; x < 2; ++x) {
+              if (x == 1 && j >= nx1) break;
+              const int u = 2 * j + x, nx = x ? nx1 : n_a;
+              w.wait(bar(V_FULL + v_st), v_ph);
+              w.wait(bar(V_PEER + v_st), v_ph);
+              if (vfix && (x ? n_a + j : j) == n - 1) { w.wait(bar(V_FIX), (ph >> 5) & 1); ph ^= 32u; }
+              w.wait(bar(P_FULL + x), (ph >> x) & 1); ph ^= 1u << x;
+              if (j == 0) { w.wait(bar(O_FREE + x), ((ph >> (2 + x)) & 1) ^ 1); ph ^= 4u << x; }
+              tc_fence_after();
+              if (elect_one()) {
+                const uint32_t b_lo = v_lo + v_st * (kVTileBytes >> 4);
+#pragma unroll
+                for (int ks = 0; ks < BN / 16; ++ks)
+                  umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, b_lo + ks * (2 * kVGroupBytes >> 4), idesc_pv, (j > 0 || ks > 0));
+                if (j == nx - 1) tc_commit(bar(O_FULL + x));
+                tc_commit(bar(V_EMPTY + v_st));
+              }
+              __syncwarp();
+              if (++v_st == kVStages) { v_st = 0; v_ph ^= 1; }
+              if (j + 1 < nx) issue_qk(x, u + 2);
+            }
+          }
+          continue;
+        }
         w.wait(bar(Q_READY), (ph >> 4) & 1);   // tile A of Q is rotated; tile B follows while QK_A already runs
         w.wait(bar(K_READY + k_st), k_ph);
         tc_fence_after();
@@ -822,18 +898,19 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       const int slot = it_n & (kRing - 1);
       w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
       if (w.dead || sm.ring[slot].t0 < 0) break;
-      const Item it = load_item<TOK>(sm.ring[slot], rank);
+      const Item it = load_item<TOK, kDual>(sm.ring[slot], rank);
       __syncwarp();
       if (lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
       if (it.n_kv == 0) continue;
       const int* pos = a.kv_positions + it.kv_off;
       const int jw = it.kv_lo + rank * kKeysCta + RW * rw;   // first key of this warp's rows in tile 0
       // lane l (< 16) holds the position of key jw + i * 128 + l (fetched one tile early)
-      int myp = __ldg(pos + min(jw + (lane & (RW - 1)), it.kv_len - 1));
-      for (int i = 0; i < it.n_kv; ++i) {
+      int myp = __ldg(pos + min(jw + it.tile_of_use(0) * BN + (lane & (RW - 1)), it.kv_len - 1));
+      for (int i = 0; i < it.n_kv; ++i) {   // i = use index: tile it.tile_of_use(i)
         const int st = kc % kKStages;
-        const int j0 = jw + i * BN;
-        const int myp_next = (i + 1 < it.n_kv) ? __ldg(pos + min(j0 + BN + (lane & (RW - 1)), it.kv_len - 1)) : 0;
+        const int tile = it.tile_of_use(i);
+        const int j0 = jw + tile * BN;
+        const int myp_next = (i + 1 < it.n_kv) ? __ldg(pos + min(jw + it.tile_of_use(i + 1) * BN + (lane & (RW - 1)), it.kv_len - 1)) : 0;
         const int nrow = it.kv_hi - j0;                   // rows of this warp's chunk that hold visible keys
         const bool work = !k_prerot && nrow > 0;
         const int p0 = __shfl_sync(0xffffffffu, myp, 0);
@@ -873,10 +950,10 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         myp = myp_next;
         // ---- V tile i: rows at or beyond kv_hi inside the last gathered block may hold anything (never written
         //      cache slots); their P is 0, make sure 0 * (those bits) is not NaN
-        if (i == it.n_kv - 1 && (it.kv_hi & (kBlock - 1)) != 0) {
+        if (tile == it.n_kv - 1 && (it.kv_hi & (kBlock - 1)) != 0) {
           const int vs = (vc + i) % kVStages;
           w.wait(bar(V_FULL + vs), ((vc + i) / kVStages) & 1);
-          const int first = it.kv_hi - (it.kv_lo + i * BN), last = (first + kBlock - 1) & ~(kBlock - 1);
+          const int first = it.kv_hi - (it.kv_lo + tile * BN), last = (first + kBlock - 1) & ~(kBlock - 1);
           if (rot_tid >= first && rot_tid < last) {
             const uint32_t vrow = smem_u32(sm.v[vs]) + (rot_tid >> 3) * kVGroupBytes + (rot_tid & 7) * 128;
 #pragma unroll
@@ -896,15 +973,28 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
     const uint32_t t_lane = tmem + ((uint32_t)((warp & 3) * 32) << 16);
     const uint32_t t_s = t_lane + x * BN, t_o = t_lane + (2 + x) * BN;
     const int tok_in = row / G, hg = row % G;
-    uint32_t sc = 0, oc = 0, qc = 0;
-    struct { bool valid; int t0, kvh, ntok_x, n; float l, m; } pe;
+    uint32_t sc = 0, oc = 0, qc = 0, xc = 0;
+    struct { bool valid, dual; int t0, kvh, ntok_x, n; float l, m; } pe;
     pe.valid = false;
     auto epilogue = [&]() {
       // ---- epilogue (a9): O / l -> out, LSE = ln sum exp of the scaled scores.  A thread owns a row in TMEM, but a row
       //      is 256 B in global memory: the warp transposes 64 columns at a time through its 4 KB staging buffer so
       //      that every store instruction writes four full 128-byte lines instead of 32 scattered 16-byte pieces
-      const float inv = pe.l > 0.f ? 1.f / pe.l : 0.f;
       if (pe.n > 0) { w.wait(bar(O_FULL + x), oc & 1); ++oc; tc_fence_after(); }
+      // dual item (tile A warps only get here with pe.dual): merge slot B's partial softmax over the other half of the KV
+      // range: m = max(m_A, m_B), O = O_A 2^(m_A - m) + O_B 2^(m_B - m), l likewise
+      float wa = 1.f, wb = 0.f;
+      const uint32_t xrow = smem_u32(sm.xchg[row]);
+      if (pe.dual) {
+        w.wait(bar(XCHG), xc & 1); ++xc;
+        const float2 ml = sm.xml[row];
+        const float m = fmaxf(pe.m, ml.x);
+        wa = (pe.m == -INFINITY) ? 0.f : fast_exp2(pe.m - m);
+        wb = (ml.x == -INFINITY) ? 0.f : fast_exp2(ml.x - m);
+        pe.l = pe.l * wa + ml.y * wb;
+        pe.m = m;
+      }
+      const float inv = pe.l > 0.f ? 1.f / pe.l : 0.f;
       if ((warp & 3) == 0) TRACE_L0(3 + x, 42);
       if (pe.ntok_x <= 0) {   // this CTA owns no row of the tile (the peer does): only release O
         if (pe.n > 0) { tc_fence_before(); __syncwarp(); if (lane == 0) mbar_arrive_cl(lbar(O_FREE + x)); }
@@ -929,6 +1019,14 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           } else {
 #pragma unroll
             for (int e = 0; e < 64; ++e) o[e] = 0.f;
+          }
+          if (pe.dual) {
+#pragma unroll
+            for (int c = 0; c < 16; ++c) {
+              const uint4 u = lds128(xrow + (uint32_t)(((16 * pass + c) ^ (row & 31)) << 4));
+              o[4 * c] = o[4 * c] * wa + __uint_as_float(u.x) * wb; o[4 * c + 1] = o[4 * c + 1] * wa + __uint_as_float(u.y) * wb;
+              o[4 * c + 2] = o[4 * c + 2] * wa + __uint_as_float(u.z) * wb; o[4 * c + 3] = o[4 * c + 3] * wa + __uint_as_float(u.w) * wb;
+            }
           }
           if (lane == 0) tma_store_wait_read();   // the previous store out of this staging buffer has been read
           __syncwarp();
@@ -975,11 +1073,11 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       const int slot = it_n & (kRing - 1);
       w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
       const bool stop = w.dead || sm.ring[slot].t0 < 0;   // one more trip for the deferred epilogue, then out
-      const Item it = load_item<TOK>(sm.ring[slot], rank);
+      const Item it = load_item<TOK, kDual>(sm.ring[slot], rank);
       __syncwarp();
       if (!stop && lane == 0) mbar_arrive_cl(lbar(SCHED_EMPTY + slot));
       const int n = stop ? 0 : it.n_x(x);      // KV tiles this tile slot runs (the same in both CTAs)
-      const int tile_t = it.tb + x * TOK;      // first token (within the item) of this CTA's tile x
+      const int tile_t = it.tok_x(x, TOK);     // first token (within the item) of this CTA's tile slot x
       if (!stop && it.n_kv > 0) {
         // ---- a3: rotate this warp's 32 rows of Q tile x in place: row = token * G + head-in-group, the G rows of a token
         //      share one position.  Exact restart at the first row, one-position steps while the positions are consecutive.
@@ -987,12 +1085,13 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         //      boundary while K0, Q_A, Q_B queue up on the rotation warps.  Rolled loop: see the note on code size there.
         const int ntw = it.ntok_x(x) - (32 * rw) / G;   // tokens of this tile that this warp rotates
         int qpx = 0;
-        if (!q_prerot && ntw > 0) {
+        const bool rot_q = !q_prerot && ntw > 0 && !(it.dual && x == 1);   // dual: slot B reads slot A's (rotated) Q tile
+        if (rot_q) {
           const int tk = min((32 * rw) / G + min(lane, NTW - 1), it.ntok_x(x) - 1);
           qpx = __ldg(a.kv_positions + it.kv_off + min(it.idx0 + tile_t + tk, it.kv_len - 1));
         }
         w.wait(bar(Q_FULL), qc & 1); ++qc;
-        if (!q_prerot && ntw > 0) {
+        if (rot_q) {
           Rot8 rot;
           uint64_t c1[4], s1[4], ns1[4];
 #pragma unroll
@@ -1027,7 +1126,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       const int idx_row = min(it.idx0 + tile_t + tok_in, it.kv_len - 1);    // highest visible key of this row
       float m_used = -INFINITY, l_run = 0.f;   // m in log2 units (score * scale * log2 e)
       for (int i = 0; i < n; ++i, ++sc) {
-        const int j0 = it.kv_lo + i * BN;
+        const int j0 = it.kv_lo + it.tile_x(x, i) * BN;
         float s[BN];
         // MINIPIC_KEY_MASK: keys with a negative logical position are invisible to every row.  Lane l looks
         // at the positions of columns l, l + 32, l + 64, l + 96 (fetched before the wait); four ballots give the tile's
@@ -1135,7 +1234,28 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       // next item starts ~3 K cycles earlier; pe = what it needs.  A tile slot that ran KV tiles for the peer's rows only
       // (ntok_x = 0, n > 0) still has to consume O_FULL and release O.
       pe.valid = it.ntok_x(x) > 0 || n > 0; pe.t0 = it.t0 + tile_t; pe.kvh = it.kvh; pe.ntok_x = it.ntok_x(x); pe.n = n;
-      pe.l = l_run; pe.m = m_used;
+      pe.l = l_run; pe.m = m_used; pe.dual = it.dual;
+      if (it.dual && x == 1) {
+        // ---- dual item, slot B: hand (O_B, m_B, l_B) to the tile-A warps of this CTA right away (not deferred)
+        w.wait(bar(O_FULL + 1), oc & 1); ++oc;
+        tc_fence_after();
+#pragma unroll 1
+        for (int c = 0; c < 4; ++c) {
+          float o[32];
+          tmem_ld32(t_o + 32 * c, o);
+          tmem_wait_ld();
+#pragma unroll
+          for (int q = 0; q < 8; ++q)
+            sts128(smem_u32(sm.xchg[row]) + (uint32_t)(((8 * c + q) ^ (row & 31)) << 4),
+                   make_uint4(__float_as_uint(o[4 * q]), __float_as_uint(o[4 * q + 1]), __float_as_uint(o[4 * q + 2]), __float_as_uint(o[4 * q + 3])));
+        }
+        sm.xml[row] = make_float2(m_used, l_run);
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cl(lbar(O_FREE + 1));
+        mbar_arrive(bar(XCHG));
+        pe.valid = false;
+      }
     }
     if (lane == 0) tma_store_wait_all();   // the staging buffers must outlive the last tensor stores
   }
@@ -1190,7 +1310,7 @@ bool make_out_map(CUtensorMap* m, void* out, int num_q_tokens, int hq, int group
              CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int G, bool kKeyMask>
+template <int G, bool kKeyMask, bool kDual>
 bool launch_gk(const Ctx& c, const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mo,
               const Params& prm, int sms) {
   const size_t smem = sizeof(Smem);
@@ -1198,13 +1318,13 @@ bool launch_gk(const Ctx& c, const CUtensorMap& mq, const CUtensorMap& mk, const
   int dev = 0;
   cudaGetDevice(&dev);
   if (dev < 0 || dev >= 64 || !attr_done[dev]) {
-    if (cudaFuncSetAttribute(prefill_sm100_kernel<G, kKeyMask>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
+    if (cudaFuncSetAttribute(prefill_sm100_kernel<G, kKeyMask, kDual>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) {
       note_error("prefill_sm100: cudaFuncSetAttribute(MaxDynamicSharedMemorySize) failed");
       return false;
     }
     if (dev >= 0 && dev < 64) attr_done[dev] = true;
   }
-  prefill_sm100_kernel<G, kKeyMask><<<sms, kThreads, smem, c.stream>>>(mq, mk, mv, mo, prm);
+  prefill_sm100_kernel<G, kKeyMask, kDual><<<sms, kThreads, smem, c.stream>>>(mq, mk, mv, mo, prm);
   note_launch();
   return true;
 }
@@ -1212,7 +1332,8 @@ bool launch_gk(const Ctx& c, const CUtensorMap& mq, const CUtensorMap& mk, const
 template <int G>
 bool launch_g(const Ctx& c, const CUtensorMap& mq, const CUtensorMap& mk, const CUtensorMap& mv, const CUtensorMap& mo,
               const Params& prm, int sms) {
-  return (c.flags & MINIPIC_KEY_MASK) ? launch_gk<G, true>(c, mq, mk, mv, mo, prm, sms) : launch_gk<G, false>(c, mq, mk, mv, mo, prm, sms);
+  if (c.flags & MINIPIC_KEY_MASK) return launch_gk<G, true, true>(c, mq, mk, mv, mo, prm, sms);
+  return prm.dual_ok ? launch_gk<G, false, true>(c, mq, mk, mv, mo, prm, sms) : launch_gk<G, false, false>(c, mq, mk, mv, mo, prm, sms);
 }
 
 }  // namespace
@@ -1269,15 +1390,21 @@ bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
   TileDesc* sorted = (TileDesc*)((char*)a.workspace + sizeof(PlanHeader));
   TileDesc* tmp = sorted + (a.num_q_tokens + 1);
   const int tok2 = 4 * BM / c.group;   // query tokens per work item: two 128-row tiles in each CTA of a pair
+  // dual items (short Q over a long KV range split between the two tile slots, struct Item) only pay on small grids, where
+  // a few long items set the time; on large ones they would just add code to the hot loops.  Decided from host scalars:
+  // fewer than ~32 full items per CTA pair, or the key-mask variant (a cold path anyway).
+  const long long items_upper = ((long long)a.num_q_tokens / tok2 + a.num_reqs) * c.hkv;
+  const int dual_ok = (c.flags & MINIPIC_KEY_MASK) || items_upper < 32LL * (current_sm_count() / 2) ? 1 : 0;
   if (cudaMemsetAsync(hdr, 0, sizeof(PlanHeader), c.stream) != cudaSuccess) return false;
   if (a.num_q_tokens > 0) {
-    plan_kernel<<<(a.num_q_tokens + kPlanThreads - 1) / kPlanThreads, kPlanThreads, 0, c.stream>>>(a, tok2, hdr, tmp, sorted);
+    plan_kernel<<<(a.num_q_tokens + kPlanThreads - 1) / kPlanThreads, kPlanThreads, 0, c.stream>>>(a, tok2, dual_ok, hdr, tmp, sorted);
     note_launch(1);
   }
   Params prm;
   prm.a = a; prm.hq = c.hq; prm.hkv = c.hkv; prm.scale_log2 = c.scale_log2; prm.flags = c.flags;
   prm.hdr = hdr; prm.tiles = sorted;
   prm.oob_grp = c.num_blocks * c.hkv * 2;
+  prm.dual_ok = dual_ok;
   for (int i = 0; i < 64; ++i) {
     prm.phase_inc[i] = c.rope.phase_inc[i];
     const double c1 = c.rope_step_cos[i], s1 = c.rope_step_sin[i];
