@@ -644,3 +644,20 @@ def test_pool_derived_tables_end_to_end():
         assert do.max() <= OUT_MAX and do.mean() <= OUT_MEAN and dl.mean() <= LSE_TOL, (kind, float(do.max()), float(dl.mean()))
     assert gk.cpu().numpy().view(np.uint16).tobytes() == kc.tobytes() and gv.cpu().numpy().view(np.uint16).tobytes() == vc.tobytes()
     assert hits_in_finals > 100
+
+
+@pytest.mark.parametrize("hq,suffix,spans", [(8, 37, [256, 144, 160]), (8, 20, [256, 144, 160]), (16, 27, [128, 400, 80, 16]),
+                                             (16, 9, [512, 96]), (8, 64, [1024, 512])])
+def test_dual_items_ragged(hq, suffix, spans):
+    """Short-Q items over a long KV range (suffix rows) run as DUAL items on small grids: both tile slots take the same rows
+    and split the KV tiles.  Odd and even tile counts, a ragged last block in slot B (V tail zeroing), a peer CTA without
+    rows, NaN bit patterns in every unwritten cache slot."""
+    w = W.single_request_prefill(name="dual", hq=hq, hkv=2, d=128, theta=5e5, dtype="bf16", sigma=1.0, span_lens=spans,
+                                 suffix_len=suffix, num_blocks=(sum(spans) + suffix) // 16 + 9, seed=hq + suffix)
+    dw = DeviceWorkload(w, cache_fill=0x7FC1)
+    dw.step(); torch.cuda.synchronize()
+    st = compare(dw, expect_variant="prefill_sm100_tcgen05")
+    assert st["entries"] == w.num_q_tokens * hq
+    out1 = dw.out.clone()
+    dw.attention(); torch.cuda.synchronize()
+    assert torch.equal(out1, dw.out)                      # run-to-run bitwise determinism (no float atomics in the merge)
