@@ -141,8 +141,12 @@ int minipic_block_rerotate(const minipic_config* cfg, void* k_cache, void* v_cac
  *   q' = R(pi_r(q_seq_idx[t])) q[t,h]      (skipped under MINIPIC_Q_PREROTATED)
  *   k_j = R(pi_r(j)) k~_j  gathered through block_tables[r]   (skipped under MINIPIC_K_PREROTATED)
  *   out[t,h] = softmax_j(q'.k_j * scale) V_j over q_vis_lo[t] <= j <= q_seq_idx[t];  lse[t,h].
- * Requires q_seq_idx[t] < kv_lens[r].  workspace: device scratch of at least
- * minipic_prefill_workspace_bytes(...) bytes, 256-byte aligned; contents are overwritten. */
+ * Requires q_seq_idx[t] < kv_lens[r].  workspace: device scratch, 256-byte aligned; contents are overwritten.
+ * minipic_prefill_workspace_bytes(...) bytes are always enough.  On small inputs (a few requests' questions over long
+ * cached contexts) that figure includes up to 64 MiB for the partial rows of KV-RANGE SPLITS: an item whose KV range is too
+ * long for a balanced grid is cut into chunks that run on different CTA pairs and are merged by a second kernel (same
+ * result up to fp32 rounding order).  A workspace sized for a LARGER call (more tokens) is accepted for a smaller one: the
+ * call then needs only the planning part and runs without splits.  Smaller than that: MINIPIC_ERR_WORKSPACE_TOO_SMALL. */
 size_t minipic_prefill_workspace_bytes(const minipic_config* cfg, int32_t num_reqs, int32_t num_q_tokens);
 int minipic_prefill_attention(const minipic_config* cfg,
                               const void* q,                    /* [Tq, Hq, D]                       */

@@ -207,10 +207,12 @@ int minipic_prefill_attention(const minipic_config* cfg, const void* q, const vo
     return MINIPIC_ERR_INVALID_ARG;
   if ((long long)max_blocks_per_req * kBlock < max_kv_len) return MINIPIC_ERR_INVALID_ARG;
   if (((uintptr_t)q | (uintptr_t)k_cache | (uintptr_t)v_cache | (uintptr_t)out) & 15) return MINIPIC_ERR_INVALID_ARG;
-  const size_t need = minipic_prefill_workspace_bytes(cfg, num_reqs, num_q_tokens);
-  if (workspace_bytes < need || (need && !workspace)) return MINIPIC_ERR_WORKSPACE_TOO_SMALL;
-  if ((uintptr_t)workspace & 255) return MINIPIC_ERR_INVALID_ARG;
   Ctx c; make_ctx(cfg, cuda_stream, &c);
+  // required: the planning part.  minipic_prefill_workspace_bytes() asks for more on small inputs (partial rows of KV-range
+  // splits); a caller that sized the workspace for a larger call simply runs those inputs unsplit.
+  const size_t need = 256 + (prefill_sm100_supported(c) ? prefill_sm100_workspace_min_bytes(c, num_reqs, num_q_tokens) : 0);
+  if (workspace_bytes < need || !workspace) return MINIPIC_ERR_WORKSPACE_TOO_SMALL;
+  if ((uintptr_t)workspace & 255) return MINIPIC_ERR_INVALID_ARG;
   PrefillArgs a{q, k_cache, v_cache, block_tables, max_blocks_per_req, cu_q_lens, kv_lens, cu_kv_lens, kv_positions,
                 q_seq_idx, q_vis_lo, num_reqs, num_q_tokens, max_kv_len, out, lse, workspace, workspace_bytes};
   if (!(c.flags & MINIPIC_FORCE_SIMT) && prefill_sm100_supported(c)) {

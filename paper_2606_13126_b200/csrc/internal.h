@@ -62,7 +62,8 @@ bool launch_decode_mma(const Ctx& c, const DecodeArgs& a, const SplitPlan& sp, f
 bool make_cache_tensor_map(CUtensorMap* m, const void* cache, int num_blocks, int hkv, int halves);
 // a2-a9 tcgen05 / TMEM / TMA prefill: bf16, D=128, G in {1,2,4,8}
 bool prefill_sm100_supported(const Ctx& c);
-size_t prefill_sm100_workspace_bytes(const Ctx& c, int num_reqs, int num_q_tokens);
+size_t prefill_sm100_workspace_bytes(const Ctx& c, int num_reqs, int num_q_tokens);       // with room for KV-range splits
+size_t prefill_sm100_workspace_min_bytes(const Ctx& c, int num_reqs, int num_q_tokens);   // what a call needs at least
 bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a);
 int prefill_sm100_error_word(const void* workspace, cudaStream_t s, int* word);   // cudaError as int; *word = 0 if healthy
 

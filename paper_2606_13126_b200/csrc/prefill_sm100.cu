@@ -22,6 +22,7 @@
 //
 // All hand-offs are mbarriers; generic-proxy smem writes are fenced with fence.proxy.async before the MMA reads.
 #include <cuda.h>
+#include <algorithm>
 #include <cstddef>
 
 #include "internal.h"
@@ -93,12 +94,19 @@ constexpr int kMaxBins = 4096;
 constexpr int kDualMinTiles = 4;   // a "dual" item (see struct Item) needs at least this many KV tiles
 constexpr unsigned kWaitMaxSpins = 1u << 26;   // x (>= 30 cycles per failed try_wait) = seconds
 
-struct TileDesc { int t0, ntok, r, idx0, lo, n_kv, kv_hi, kv_len, kv_off, pad; };   // kv_off = cu_kv_lens[r]
+struct TileDesc { int t0, ntok, r, idx0, lo, n_kv, kv_hi, kv_len, kv_off, pad, part, rsv; };   // kv_off = cu_kv_lens[r]; pad: dual item; part: see SplitGroup
+// KV-RANGE SPLITS (small grids only): an item whose tile steps exceed what one CTA pair should get is cut into chunks over
+// consecutive KV tiles; every chunk is an item of its own that writes (O normalised over the chunk, lse of the chunk) as fp32
+// into partial token slots of the workspace - chunk s of a group owns slots [base + s ntok, base + (s + 1) ntok), part = 1 +
+// its first slot - and split_merge_kernel combines them: the 64-token question of ONE request over a long cached context then
+// runs on many CTA pairs instead of on hkv of them.
+struct SplitGroup { int t0, ntok, nsplit, base; };
 // magic tags a header written by THIS kernel family, so minipic_prefill_status() can tell it from a workspace that a call
 // dispatched to another kernel never touched (err and magic are adjacent: one 8-byte read)
 constexpr int kPlanMagic = 0x4d504943;   // "MPIC"
-struct PlanHeader { int n_tiles; int next_item; int err; int magic; int err_info[4]; int pad[56]; int hist[kMaxBins]; };
-struct ItemInfo { int t0, ntok, r, idx0, lo, kvh, n_kv, kv_hi, kv_len, kv_off, pad[2]; };   // 48 B ring entry; t0 < 0 = stop
+struct PlanHeader { int n_tiles; int next_item; int err; int magic; int err_info[4]; int ticket; int n_raw; int n_groups; int part_used; int pad[52]; };
+static_assert(sizeof(PlanHeader) == 256, "header size");
+struct ItemInfo { int t0, ntok, r, idx0, lo, kvh, n_kv, kv_hi, kv_len, kv_off, pad[2]; };   // 48 B ring entry; t0 < 0 = stop; pad = {dual, part}
 
 // ------------------------------------------------------------------------------------------------ PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -325,18 +333,53 @@ __device__ __forceinline__ bool tile_starts(const PrefillArgs& a, int t, int r, 
 
 // ONE launch (a2).  Every block marks its 256 query tokens: the start flags of those tokens and of the next `tok` ones go
 // into a shared bitmask, so a starting token finds the length of its item with a find-first-set instead of a sequential
-// scan (which alone took 22 us on config 2); descriptors and the cost histogram are appended with atomics.  The LAST block
-// to finish (ticket) turns the histogram into offsets in DESCENDING cost order and scatters the descriptors: a counting
-// sort, longest item first, that the persistent kernel's atomic work counter then walks.
+// scan (which alone took 22 us on config 2), and appends its descriptor with an atomic.  The LAST block to finish (ticket)
+// then sees every item: it adds up the tile steps, cuts items that are too long for a balanced grid into KV-range chunks
+// (SplitGroup; only when the host allows it), and sorts all descriptors by DESCENDING cost - a counting sort in shared
+// memory, longest item first - for the persistent kernel's atomic work counter to walk.
 constexpr int kPlanThreads = 256, kPlanMaxTok = 512;   // tok = 4 * 128 / G <= 512
+constexpr int kPlanCache = 2560;                         // descriptors the last block keeps in shared memory when it may split
+constexpr int kSplitMinSteps = 4, kSplitMax = 16;      // a chunk runs at least 4 tile steps; at most 16 chunks per item
 __device__ __forceinline__ int tile_cost(const TileDesc& td) { return td.pad ? (td.n_kv + 1) >> 1 : td.n_kv; }   // tile steps
-__global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, int tok, int dual_ok, PlanHeader* hdr, TileDesc* tmp, TileDesc* sorted) {
+__device__ __forceinline__ int dual_flag(int dual_ok, int ntok, int tok, int n_kv) {   // dual item: at most 2 TOK tokens over a long KV range
+  return (dual_ok && 2 * ntok <= tok && n_kv >= kDualMinTiles) ? 1 : 0;
+}
+// chunks an item of `cost` steps is cut into when a pair should not run more than `tsplit` steps of it (1 = not cut)
+__device__ __forceinline__ int split_count(int cost, int n_kv, int tsplit, int* tiles_per_chunk) {
+  *tiles_per_chunk = n_kv;
+  if (2 * cost <= 3 * tsplit) return 1;   // not worth a second item (per-item overhead ~ one tile step, plus the merge)
+  const int ns = min(kSplitMax, (cost + tsplit - 1) / tsplit);
+  const int ct = (n_kv + ns - 1) / ns;
+  *tiles_per_chunk = ct;
+  return (n_kv + ct - 1) / ct;
+}
+struct PlanArgs {
+  int tok, dual_ok;
+  int split_pairs;    // 0: no KV-range splits; else the number of CTA pairs to balance for
+  int hkv, part_cap;  // partial token slots the workspace has room for
+  int sorted_cap;     // descriptors `sorted` has room for
+  PlanHeader* hdr; TileDesc* tmp; TileDesc* sorted; SplitGroup* groups;
+};
+__device__ __forceinline__ TileDesc load_desc(const TileDesc* p) {   // written by other blocks of this launch: read through L2
+  TileDesc td;
+  const int* src = reinterpret_cast<const int*>(p);
+  int* dst = reinterpret_cast<int*>(&td);
+#pragma unroll
+  for (int e = 0; e < (int)(sizeof(TileDesc) / sizeof(int)); ++e) dst[e] = __ldcg(src + e);
+  return td;
+}
+__global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanArgs pa) {
   constexpr int kWords = (kPlanThreads + kPlanMaxTok) / 32;
   __shared__ unsigned sflag[kWords];
-  __shared__ int s_last;
+  __shared__ int s_last, s_groups, s_slots;
   __shared__ int wsum[kPlanThreads / 32];
+  __shared__ int red[3], cand_items[8], cand_max[8], s_nlong, long_idx[kPlanThreads];
+  __shared__ unsigned short s_cost[kPlanCache], s_nkv[kPlanCache], s_ntk[kPlanCache];
+  __shared__ int shist[kMaxBins];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
   const int b0 = blockIdx.x * kPlanThreads;
+  const int tok = pa.tok;
+  PlanHeader* hdr = pa.hdr;
   if (blockIdx.x == 0 && tid == 0) hdr->magic = kPlanMagic;
   auto request_of = [&](int t) {
     int lo_r = 0, hi_r = a.num_reqs;
@@ -376,22 +419,112 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, int t
     const int kv_lo = td.lo & ~(kBlock - 1);
     td.kv_hi = min(td.idx0 + n, td.kv_len);
     td.n_kv = td.kv_hi > kv_lo ? (td.kv_hi - kv_lo + BN - 1) / BN : 0;
-    td.pad = (dual_ok && 2 * n <= tok && td.n_kv >= kDualMinTiles) ? 1 : 0;   // dual item: at most 2 TOK tokens over a long KV range
-    tmp[atomicAdd(&hdr->n_tiles, 1)] = td;
-    atomicAdd(&hdr->hist[min(tile_cost(td), kMaxBins - 1)], 1);
+    td.pad = dual_flag(pa.dual_ok, n, tok, td.n_kv);
+    td.part = 0; td.rsv = 0;
+    pa.tmp[atomicAdd(&hdr->n_raw, 1)] = td;
   }
-  // ---- last block: counting sort of all descriptors, longest first
+  // ---- last block: balance (KV-range splits) and counting sort of all descriptors, longest first
   __threadfence();
   __syncthreads();
-  if (tid == 0) s_last = atomicAdd(&hdr->pad[0], 1) == (int)gridDim.x - 1;
+  if (tid == 0) s_last = atomicAdd(&hdr->ticket, 1) == (int)gridDim.x - 1;
   __syncthreads();
   if (!s_last) return;
   __threadfence();
-  constexpr int PER = kMaxBins / kPlanThreads;   // 16 ranks per thread; rank = kMaxBins - 1 - bin (descending cost)
-  volatile int* hist = hdr->hist;
+  const int n_raw = *(volatile int*)&hdr->n_raw;
+  auto block_reduce = [&](int v0, int v1, int vmax) {   // red[0], red[1] = block-wide sums, red[2] = block-wide max (>= 0)
+    __syncthreads();
+    if (tid < 3) red[tid] = 0;
+    __syncthreads();
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      v0 += __shfl_xor_sync(0xffffffffu, v0, o); v1 += __shfl_xor_sync(0xffffffffu, v1, o);
+      vmax = max(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
+    }
+    if (lane == 0) { atomicAdd(&red[0], v0); atomicAdd(&red[1], v1); atomicMax(&red[2], vmax); }
+    __syncthreads();
+  };
+  int tsplit = 0x3fffffff;
+  constexpr int kCand = 8;   // candidate chunk lengths
+  if (pa.split_pairs > 0 && n_raw <= kPlanCache) {   // kPlanCache descriptors: more than any small grid has
+    int steps = 0, cmax_all = 0;
+    for (int i = tid; i < n_raw; i += kPlanThreads) {
+      const TileDesc td = load_desc(pa.tmp + i);
+      const int c = tile_cost(td);
+      s_cost[i] = (unsigned short)min(c, 65535); s_nkv[i] = (unsigned short)min(td.n_kv, 65535); s_ntk[i] = (unsigned short)td.ntok;
+      steps += c; cmax_all = max(cmax_all, c);
+    }
+    block_reduce(steps, 0, cmax_all);
+    const long long all_steps = (long long)red[0] * pa.hkv;
+    const int per_pair = max(kSplitMinSteps, (int)((all_steps + pa.split_pairs - 1) / pa.split_pairs));
+    const int cstep = max(1, per_pair / 8);
+    if (2 * red[2] > 3 * per_pair && red[2] < 65535) {   // at least one item is long enough to be cut
+      __syncthreads();
+      if (tid < kCand) { cand_items[tid] = n_raw; cand_max[tid] = 0; }
+      if (tid == 0) { s_nlong = 0; s_groups = 0; s_slots = 0; }
+      __syncthreads();
+      int short_max = 0;
+      for (int i = tid; i < n_raw; i += kPlanThreads) {
+        const int c = s_cost[i];
+        if (2 * c > 3 * per_pair) { const int j = atomicAdd(&s_nlong, 1); if (j < kPlanThreads) long_idx[j] = i; }
+        else short_max = max(short_max, c);
+      }
+      block_reduce(0, 0, short_max);
+      short_max = red[2];
+      const int n_long = s_nlong;
+      if (n_long <= kPlanThreads) {
+        // a few candidate chunk lengths: keep the one with the shortest estimated makespan - rounds of items x mean item cost,
+        // but at least the longest item - so that e.g. 8 long items become 72 chunks on 74 pairs rather than 80.  One task per
+        // (long item, candidate); the short items count 1 each whatever the candidate.
+        for (int task = tid; task < n_long * kCand; task += kPlanThreads) {
+          const int k = task % kCand, i = long_idx[task / kCand];
+          int ct;
+          const int ns = split_count(s_cost[i], s_nkv[i], per_pair + k * cstep, &ct);
+          atomicAdd(&cand_items[k], ns - 1);
+          atomicMax(&cand_max[k], dual_flag(pa.dual_ok, s_ntk[i], tok, ct) ? (ct + 1) >> 1 : ct);
+        }
+        __syncthreads();
+        long long best = 0x7fffffffffffffffLL;
+        for (int k = 0; k < kCand; ++k) {
+          const long long n_it = (long long)cand_items[k] * pa.hkv, rounds = (n_it + pa.split_pairs - 1) / pa.split_pairs;
+          // + 1024: the fixed cost of an item (Q load + rotation, pipeline fill, epilogue) is about one tile step
+          const long long est = max((long long)max(cand_max[k], short_max) * 1024, rounds * (all_steps * 1024 / n_it)) + rounds * 1024;
+          if (est < best) { best = est; tsplit = per_pair + k * cstep; }
+        }
+        int slots = 0, extra = 0;
+        if (tid < n_long) {
+          const int i = long_idx[tid];
+          int ct;
+          const int ns = split_count(s_cost[i], s_nkv[i], tsplit, &ct);
+          if (ns > 1) { slots = ns * s_ntk[i]; extra = ns - 1; }
+        }
+        block_reduce(slots, extra, 0);
+        if (red[0] > pa.part_cap || n_raw + red[1] > pa.sorted_cap) tsplit = 0x3fffffff;   // no room: run unsplit
+      }
+    }
+    __syncthreads();
+  }
+  for (int i = tid; i < kMaxBins; i += kPlanThreads) shist[i] = 0;
+  if (tid == 0) { s_groups = 0; s_slots = 0; }
+  __syncthreads();
+  // pass 1: histogram of the (chunk) costs
+  for (int i = tid; i < n_raw; i += kPlanThreads) {
+    const TileDesc td = load_desc(pa.tmp + i);
+    int ct;
+    const int ns = split_count(tile_cost(td), td.n_kv, tsplit, &ct);
+    if (ns == 1) { atomicAdd(&shist[min(tile_cost(td), kMaxBins - 1)], 1); continue; }
+    for (int sidx = 0; sidx < ns; ++sidx) {
+      TileDesc ch = td;
+      ch.n_kv = min(ct, td.n_kv - sidx * ct);
+      ch.pad = dual_flag(pa.dual_ok, td.ntok, tok, ch.n_kv);
+      atomicAdd(&shist[min(tile_cost(ch), kMaxBins - 1)], 1);
+    }
+  }
+  __syncthreads();
+  // exclusive prefix over the bins in DESCENDING cost order: rank = kMaxBins - 1 - bin
+  constexpr int PER = kMaxBins / kPlanThreads;   // 16 ranks per thread
   int v[PER], tot = 0;
 #pragma unroll
-  for (int e = 0; e < PER; ++e) { v[e] = hist[kMaxBins - 1 - (PER * tid + e)]; tot += v[e]; }
+  for (int e = 0; e < PER; ++e) { v[e] = shist[kMaxBins - 1 - (PER * tid + e)]; tot += v[e]; }
   int incl = tot;
 #pragma unroll
   for (int o = 1; o < 32; o <<= 1) {
@@ -403,18 +536,63 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, int t
   int base = incl - tot;
   for (int w2 = 0; w2 < wid; ++w2) base += wsum[w2];
 #pragma unroll
-  for (int e = 0; e < PER; ++e) { hist[kMaxBins - 1 - (PER * tid + e)] = base; base += v[e]; }
+  for (int e = 0; e < PER; ++e) { shist[kMaxBins - 1 - (PER * tid + e)] = base; base += v[e]; }
+  if (tid == kPlanThreads - 1) hdr->n_tiles = base;   // total number of descriptors after the splits
   __syncthreads();
-  const int n_tiles = *(volatile int*)&hdr->n_tiles;
-  for (int i = tid; i < n_tiles; i += kPlanThreads) {
-    TileDesc td;   // written by other blocks of this launch: read through L2
-    {
-      const int* src = reinterpret_cast<const int*>(tmp + i);
-      int* dst = reinterpret_cast<int*>(&td);
-#pragma unroll
-      for (int e = 0; e < (int)(sizeof(TileDesc) / sizeof(int)); ++e) dst[e] = __ldcg(src + e);
+  // pass 2: scatter
+  for (int i = tid; i < n_raw; i += kPlanThreads) {
+    const TileDesc td = load_desc(pa.tmp + i);
+    int ct;
+    const int ns = split_count(tile_cost(td), td.n_kv, tsplit, &ct);
+    if (ns == 1) { pa.sorted[atomicAdd(&shist[min(tile_cost(td), kMaxBins - 1)], 1)] = td; continue; }
+    const int g = atomicAdd(&s_groups, 1), slot0 = atomicAdd(&s_slots, ns * td.ntok);
+    pa.groups[g] = SplitGroup{td.t0, td.ntok, ns, slot0};
+    const int kv_lo = td.lo & ~(kBlock - 1);
+    for (int sidx = 0; sidx < ns; ++sidx) {
+      TileDesc ch = td;
+      ch.n_kv = min(ct, td.n_kv - sidx * ct);
+      if (sidx > 0) ch.lo = kv_lo + sidx * ct * BN;                    // a multiple of 128: no vis_lo mask inside the chunk
+      if (sidx < ns - 1) ch.kv_hi = kv_lo + (sidx + 1) * ct * BN;       // < kv_hi: whole tiles, no partial last block
+      ch.pad = dual_flag(pa.dual_ok, td.ntok, tok, ch.n_kv);
+      ch.part = 1 + slot0 + sidx * td.ntok;
+      pa.sorted[atomicAdd(&shist[min(tile_cost(ch), kMaxBins - 1)], 1)] = ch;
     }
-    sorted[atomicAdd(&hdr->hist[min(tile_cost(td), kMaxBins - 1)], 1)] = td;
+  }
+  __syncthreads();
+  if (tid == 0) { hdr->n_groups = s_groups; hdr->part_used = s_slots; }
+}
+
+// a9 for split items: out[t, h] = sum_s w_s O_s / sum_s w_s with w_s = e^{lse_s - max}, lse = max + ln sum_s w_s.  One warp
+// per (token, head) row, a lane owns 4 of the 128 columns.  Launched after the attention kernel whenever splits were
+// allowed; with no group in the header it returns at once.
+__global__ void __launch_bounds__(256) split_merge_kernel(const PlanHeader* hdr, const SplitGroup* groups, const float* part_o,
+                                                          const float* part_lse, int hq, __nv_bfloat16* out, float* lse) {
+  const int n_groups = hdr->n_groups;
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  for (int g = 0; g < n_groups; ++g) {   // every block takes a slice of every group's rows (there are few groups)
+    const SplitGroup sg = groups[g];
+    for (int rowi = blockIdx.x * 8 + wib; rowi < sg.ntok * hq; rowi += gridDim.x * 8) {
+      const int j = rowi / hq, h = rowi % hq;
+      float mx = -INFINITY;
+      for (int sidx = 0; sidx < sg.nsplit; ++sidx) mx = fmaxf(mx, part_lse[(size_t)(sg.base + sidx * sg.ntok + j) * hq + h]);
+      float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+      float wsum_ = 0.f;
+      if (mx > -INFINITY) {
+        for (int sidx = 0; sidx < sg.nsplit; ++sidx) {
+          const size_t prow = (size_t)(sg.base + sidx * sg.ntok + j) * hq + h;
+          const float wgt = __expf(part_lse[prow] - mx);   // e^{-inf} = 0: a chunk with no visible key for this row
+          const float4 o = *reinterpret_cast<const float4*>(part_o + prow * D + 4 * lane);
+          acc.x += wgt * o.x; acc.y += wgt * o.y; acc.z += wgt * o.z; acc.w += wgt * o.w;
+          wsum_ += wgt;
+        }
+      }
+      const float inv = wsum_ > 0.f ? 1.f / wsum_ : 0.f;
+      const size_t orow = (size_t)(sg.t0 + j) * hq + h;
+      uint2 pk;
+      pk.x = pack_bf16(acc.x * inv, acc.y * inv); pk.y = pack_bf16(acc.z * inv, acc.w * inv);
+      *reinterpret_cast<uint2*>(out + orow * D + 4 * lane) = pk;
+      if (lane == 0) lse[orow] = wsum_ > 0.f ? mx + logf(wsum_) : -INFINITY;
+    }
   }
 }
 
@@ -469,6 +647,8 @@ struct Params {
   const TileDesc* tiles;
   int oob_grp;                       // first row-group coordinate beyond the cache tensor map: TMA zero-fills
   int dual_ok;                       // the plan may make dual items (host decision from scalars: small grids only)
+  float* part_o;                     // KV-range splits: partial O [token slot][hq][128] fp32 and the chunk's lse [token slot][hq]
+  float* part_lse;
   unsigned long long phase_inc[64];  // F_i (common.cuh)
   float2 step1[64];                  // (cos f_i, sin f_i)
   float2 step4[64];                  // (cos 4 f_i, sin 4 f_i): the four-position RoPE step of the rotation lanes
@@ -485,6 +665,7 @@ struct Params {
 struct Item {
   int t0, ntok, r, idx0, lo, kvh, n_kv, kv_hi, kv_len, kv_off;
   int kv_lo, tb, ntok_a, ntok_b, n_a, n_b;
+  int part;   // > 0: a KV-range chunk; its rows go to partial token slots part - 1 + (token within the item)
   bool dual;
   __device__ __forceinline__ int ntok_x(int x) const { return x ? ntok_b : ntok_a; }
   __device__ __forceinline__ int n_x(int x) const { return x ? n_b : n_a; }   // KV tiles slot x runs (0: the pair skips the slot)
@@ -499,6 +680,7 @@ __device__ __forceinline__ Item load_item(const ItemInfo& ii, int rank) {
   it.kv_hi = ii.kv_hi; it.kv_len = ii.kv_len; it.kv_off = ii.kv_off;
   it.kv_lo = it.lo & ~(kBlock - 1);
   it.dual = kDual && ii.pad[0] != 0;   // kDual = false: a compile-time constant, every dual branch folds away
+  it.part = kDual ? ii.pad[1] : 0;     // splits are only made where dual items are
   if (it.dual) {
     it.tb = rank * TOK;
     it.ntok_a = it.ntok_b = min(max(it.ntok - it.tb, 0), TOK);
@@ -628,12 +810,12 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
             ii.kv_hi = td.kv_hi; ii.kv_len = td.kv_len; ii.kv_off = td.kv_off;
           }
           ii.pad[0] = ii.pad[1] = 0;
-          if (item < n_items) ii.pad[0] = prm.tiles[item / prm.hkv].pad;
+          if (item < n_items) { ii.pad[0] = prm.tiles[item / prm.hkv].pad; ii.pad[1] = prm.tiles[item / prm.hkv].part; }
           sm.ring[slot] = ii;
           const uint32_t dst = ring_p + (uint32_t)slot * (uint32_t)sizeof(ItemInfo);
           st_cluster_v4(dst, ii.t0, ii.ntok, ii.r, ii.idx0);
           st_cluster_v4(dst + 16, ii.lo, ii.kvh, ii.n_kv, ii.kv_hi);
-          st_cluster_v4(dst + 32, ii.kv_len, ii.kv_off, ii.pad[0], 0);
+          st_cluster_v4(dst + 32, ii.kv_len, ii.kv_off, ii.pad[0], ii.pad[1]);
           mbar_arrive_cl_release(lbar(SCHED_FULL + slot));
           mbar_arrive_cl_release(full_p + 8u * (uint32_t)slot);
           TRACE(0, 1);
@@ -974,7 +1156,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
     const uint32_t t_s = t_lane + x * BN, t_o = t_lane + (2 + x) * BN;
     const int tok_in = row / G, hg = row % G;
     uint32_t sc = 0, oc = 0, qc = 0, xc = 0;
-    struct { bool valid, dual; int t0, kvh, ntok_x, n; float l, m; } pe;
+    struct { bool valid, dual; int t0, kvh, ntok_x, n, pslot; float l, m; } pe;   // pslot >= 0: partial token slot of the tile's first token
     pe.valid = false;
     auto epilogue = [&]() {
       // ---- epilogue (a9): O / l -> out, LSE = ln sum exp of the scaled scores.  A thread owns a row in TMEM, but a row
@@ -1028,6 +1210,14 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
               o[4 * c + 2] = o[4 * c + 2] * wa + __uint_as_float(u.z) * wb; o[4 * c + 3] = o[4 * c + 3] * wa + __uint_as_float(u.w) * wb;
             }
           }
+          if (kDual && pe.pslot >= 0) {   // KV-range chunk: the row, normalised over the chunk, goes to its partial slot as fp32
+            if (tok_in < pe.ntok_x) {
+              float4* po = reinterpret_cast<float4*>(prm.part_o + ((size_t)(pe.pslot + tok_in) * prm.hq + pe.kvh * G + hg) * D + pass * 64);
+#pragma unroll
+              for (int c = 0; c < 16; ++c) po[c] = make_float4(o[4 * c] * inv, o[4 * c + 1] * inv, o[4 * c + 2] * inv, o[4 * c + 3] * inv);
+            }
+            continue;
+          }
           if (lane == 0) tma_store_wait_read();   // the previous store out of this staging buffer has been read
           __syncwarp();
 #pragma unroll
@@ -1058,9 +1248,11 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         }
       }
       if ((warp & 3) == 0) TRACE_L0(3 + x, 43);
-      if ((tok_in < pe.ntok_x))
-        a.lse[(size_t)(pe.t0 + tok_in) * prm.hq + pe.kvh * G + hg] =
-            pe.l > 0.f ? (pe.m + log2f(pe.l)) * 0.6931471805599453f : -INFINITY;
+      if ((tok_in < pe.ntok_x)) {
+        const float lse_row = pe.l > 0.f ? (pe.m + log2f(pe.l)) * 0.6931471805599453f : -INFINITY;
+        if (kDual && pe.pslot >= 0) prm.part_lse[(size_t)(pe.pslot + tok_in) * prm.hq + pe.kvh * G + hg] = lse_row;
+        else a.lse[(size_t)(pe.t0 + tok_in) * prm.hq + pe.kvh * G + hg] = lse_row;
+      }
         };
     // Q rotation (a3) state of this lane: same row / chunk mapping as the K rotation lanes
     const int rw = warp & 3, rsub = lane >> 3, ch = lane & 7;
@@ -1234,7 +1426,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       // next item starts ~3 K cycles earlier; pe = what it needs.  A tile slot that ran KV tiles for the peer's rows only
       // (ntok_x = 0, n > 0) still has to consume O_FULL and release O.
       pe.valid = it.ntok_x(x) > 0 || n > 0; pe.t0 = it.t0 + tile_t; pe.kvh = it.kvh; pe.ntok_x = it.ntok_x(x); pe.n = n;
-      pe.l = l_run; pe.m = m_used; pe.dual = it.dual;
+      pe.l = l_run; pe.m = m_used; pe.dual = it.dual; pe.pslot = it.part > 0 ? it.part - 1 + tile_t : -1;
       if (it.dual && x == 1) {
         // ---- dual item, slot B: hand (O_B, m_B, l_B) to the tile-A warps of this CTA right away (not deferred)
         w.wait(bar(O_FULL + 1), oc & 1); ++oc;
@@ -1375,8 +1567,40 @@ bool prefill_sm100_supported(const Ctx& c) {
   return c.dtype == MINIPIC_BF16 && c.d == 128 && (c.group == 1 || c.group == 2 || c.group == 4 || c.group == 8);
 }
 
-size_t prefill_sm100_workspace_bytes(const Ctx&, int, int num_q_tokens) {
-  return sizeof(PlanHeader) + 2 * (size_t)(num_q_tokens + 1) * sizeof(TileDesc) + 512;
+// Workspace: [PlanHeader][sorted descriptors][unsorted descriptors][split groups][partial lse][partial O].  The part up to the
+// split groups is REQUIRED; the partial slots are optional: KV-range splits are made only if they fit in what the caller gave.
+struct WsLayout { size_t sorted, tmp, groups, part, min_bytes; int sorted_cap; };
+static size_t up256(size_t x) { return (x + 255) & ~(size_t)255; }
+static WsLayout ws_layout(int num_q_tokens) {
+  WsLayout l;
+  l.sorted_cap = 2 * (num_q_tokens + 1);   // room for the chunks of split items
+  l.sorted = sizeof(PlanHeader);
+  l.tmp = up256(l.sorted + (size_t)l.sorted_cap * sizeof(TileDesc));
+  l.groups = up256(l.tmp + (size_t)(num_q_tokens + 1) * sizeof(TileDesc));
+  l.part = up256(l.groups + (size_t)(num_q_tokens + 1) * sizeof(SplitGroup));
+  l.min_bytes = l.part;
+  return l;
+}
+static size_t slot_bytes(const Ctx& c) { return (size_t)c.hq * (D + 1) * sizeof(float); }   // one partial token slot: O row + lse per head
+// small grids only (fewer than ~32 full items per CTA pair): there a few long items set the time, and dual items / KV-range
+// splits pay; on large grids they would only add code to the hot loops.  Decided from host scalars.
+static bool small_grid(const Ctx& c, int num_q_tokens, int num_reqs) {
+  const int tok2 = 4 * BM / c.group;   // query tokens per work item: two 128-row tiles in each CTA of a pair
+  const long long items_upper = ((long long)num_q_tokens / tok2 + num_reqs) * c.hkv;
+  return items_upper < 32LL * (current_sm_count() / 2);
+}
+constexpr int kPartSlotsMax = 4096;                 // partial token slots asked for ...
+constexpr size_t kPartBytesMax = (size_t)64 << 20;   // ... within this many bytes
+
+size_t prefill_sm100_workspace_min_bytes(const Ctx&, int, int num_q_tokens) { return ws_layout(num_q_tokens).min_bytes + 512; }
+
+size_t prefill_sm100_workspace_bytes(const Ctx& c, int, int num_q_tokens) {
+  size_t b = ws_layout(num_q_tokens).min_bytes + 512;
+  if (small_grid(c, num_q_tokens, 0)) {   // a superset of the launches that may split (num_reqs only makes the grid larger)
+    const size_t slots = std::min<size_t>(kPartSlotsMax, kPartBytesMax / slot_bytes(c));
+    b += slots * slot_bytes(c) + 256;
+  }
+  return b;
 }
 
 bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
@@ -1386,18 +1610,28 @@ bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
     note_error("prefill_sm100: cuTensorMapEncodeTiled failed (driver entry point missing or bad tensor geometry)");
     return false;
   }
-  PlanHeader* hdr = (PlanHeader*)a.workspace;
-  TileDesc* sorted = (TileDesc*)((char*)a.workspace + sizeof(PlanHeader));
-  TileDesc* tmp = sorted + (a.num_q_tokens + 1);
-  const int tok2 = 4 * BM / c.group;   // query tokens per work item: two 128-row tiles in each CTA of a pair
-  // dual items (short Q over a long KV range split between the two tile slots, struct Item) only pay on small grids, where
-  // a few long items set the time; on large ones they would just add code to the hot loops.  Decided from host scalars:
-  // fewer than ~32 full items per CTA pair, or the key-mask variant (a cold path anyway).
-  const long long items_upper = ((long long)a.num_q_tokens / tok2 + a.num_reqs) * c.hkv;
-  const int dual_ok = (c.flags & MINIPIC_KEY_MASK) || items_upper < 32LL * (current_sm_count() / 2) ? 1 : 0;
+  const WsLayout wl = ws_layout(a.num_q_tokens);
+  char* ws = (char*)a.workspace;
+  PlanHeader* hdr = (PlanHeader*)ws;
+  TileDesc* sorted = (TileDesc*)(ws + wl.sorted);
+  TileDesc* tmp = (TileDesc*)(ws + wl.tmp);
+  SplitGroup* groups = (SplitGroup*)(ws + wl.groups);
+  const int tok2 = 4 * BM / c.group;
+  // dual items (short Q over a long KV range split between the two tile slots, struct Item) and KV-range splits (SplitGroup):
+  // small grids, or the key-mask variant (a cold path anyway)
+  const int dual_ok = (c.flags & MINIPIC_KEY_MASK) || small_grid(c, a.num_q_tokens, a.num_reqs) ? 1 : 0;
+  const int pairs = current_sm_count() / 2;
+  int part_cap = 0;
+  if (dual_ok && a.workspace_bytes > wl.part + 256)
+    part_cap = (int)std::min<size_t>(kPartSlotsMax, (a.workspace_bytes - wl.part - 256) / slot_bytes(c));
+  float* part_lse = (float*)(ws + wl.part);
+  float* part_o = (float*)(ws + up256(wl.part + (size_t)part_cap * c.hq * sizeof(float)));
   if (cudaMemsetAsync(hdr, 0, sizeof(PlanHeader), c.stream) != cudaSuccess) return false;
   if (a.num_q_tokens > 0) {
-    plan_kernel<<<(a.num_q_tokens + kPlanThreads - 1) / kPlanThreads, kPlanThreads, 0, c.stream>>>(a, tok2, dual_ok, hdr, tmp, sorted);
+    PlanArgs pa;
+    pa.tok = tok2; pa.dual_ok = dual_ok; pa.split_pairs = part_cap > 0 ? pairs : 0; pa.hkv = c.hkv; pa.part_cap = part_cap;
+    pa.sorted_cap = wl.sorted_cap; pa.hdr = hdr; pa.tmp = tmp; pa.sorted = sorted; pa.groups = groups;
+    plan_kernel<<<(a.num_q_tokens + kPlanThreads - 1) / kPlanThreads, kPlanThreads, 0, c.stream>>>(a, pa);
     note_launch(1);
   }
   Params prm;
@@ -1405,6 +1639,7 @@ bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
   prm.hdr = hdr; prm.tiles = sorted;
   prm.oob_grp = c.num_blocks * c.hkv * 2;
   prm.dual_ok = dual_ok;
+  prm.part_o = part_o; prm.part_lse = part_lse;
   for (int i = 0; i < 64; ++i) {
     prm.phase_inc[i] = c.rope.phase_inc[i];
     const double c1 = c.rope_step_cos[i], s1 = c.rope_step_sin[i];
@@ -1413,13 +1648,18 @@ bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
     prm.step4[i] = make_float2((float)(c2 * c2 - s2 * s2), (float)(2.0 * s2 * c2));
   }
   const int sms = current_sm_count() & ~1;   // CTA pairs (clusters of 2)
+  bool ok = false;
   switch (c.group) {
-    case 1: return launch_g<1>(c, mq, mk, mv, mo, prm, sms);
-    case 2: return launch_g<2>(c, mq, mk, mv, mo, prm, sms);
-    case 4: return launch_g<4>(c, mq, mk, mv, mo, prm, sms);
-    case 8: return launch_g<8>(c, mq, mk, mv, mo, prm, sms);
+    case 1: ok = launch_g<1>(c, mq, mk, mv, mo, prm, sms); break;
+    case 2: ok = launch_g<2>(c, mq, mk, mv, mo, prm, sms); break;
+    case 4: ok = launch_g<4>(c, mq, mk, mv, mo, prm, sms); break;
+    case 8: ok = launch_g<8>(c, mq, mk, mv, mo, prm, sms); break;
   }
-  return false;
+  if (ok && part_cap > 0) {   // the plan may have split items: combine their partial rows (no group: the kernel returns at once)
+    split_merge_kernel<<<sms, 256, 0, c.stream>>>(hdr, groups, part_o, part_lse, c.hq, (__nv_bfloat16*)a.out, a.lse);
+    note_launch(1);
+  }
+  return ok;
 }
 
 }  // namespace minipic

@@ -661,3 +661,65 @@ def test_dual_items_ragged(hq, suffix, spans):
     out1 = dw.out.clone()
     dw.attention(); torch.cuda.synchronize()
     assert torch.equal(out1, dw.out)                      # run-to-run bitwise determinism (no float atomics in the merge)
+
+
+def _split_groups(dw):
+    """White-box: number of KV-range split groups the last plan made (int 10 of the workspace header)."""
+    return int(dw.workspace[:48].cpu().numpy().view(np.int32)[10])
+
+
+@pytest.mark.parametrize("hq,hkv,suffix,ctx_spans,uncached", [(32, 8, 64, 12, 0), (8, 2, 37, 10, 1), (8, 8, 20, 9, 0),
+                                                              (16, 2, 64, 7, 1), (8, 1, 5, 14, 0)])
+def test_kv_range_splits_question_over_long_context(hq, hkv, suffix, ctx_spans, uncached):
+    """ONE request's question over a long cached context (the paper's partial prefill): the few long items are cut into
+    KV-range chunks that run on different CTA pairs and are merged by a second kernel.  Ragged span lengths (chunk borders
+    fall anywhere), an uncached span (span-local rows: some chunks hold no visible key for them), GQA groups 1, 4 and 8, NaN
+    bit patterns in unwritten cache slots; the result is bitwise reproducible and equal to the unsplit run within rounding."""
+    w = W.rag_partial_prefill(name="split", seed=hq + suffix, hq=hq, hkv=hkv, num_reqs=1, pool_spans=ctx_spans + 3,
+                              spans_per_req=ctx_spans, span_min=300, span_max=700, uncached_per_req=uncached, suffix_len=suffix)
+    dw = DeviceWorkload(w, cache_fill=0x7FC1)
+    dw.step(); torch.cuda.synchronize()
+    assert _split_groups(dw) > 0, "this shape is meant to exercise the split path"
+    st = compare(dw, expect_variant="prefill_sm100_tcgen05")
+    assert st["entries"] == w.num_q_tokens * hq
+    out1, lse1 = dw.out.clone(), dw.lse.clone()
+    dw.attention(); torch.cuda.synchronize()
+    assert torch.equal(out1, dw.out) and torch.equal(lse1, dw.lse)      # run-to-run bitwise determinism
+    # the same call with only the REQUIRED part of the workspace runs unsplit and agrees within the rounding of the merge
+    need_all = dw.ws_bytes
+    lo = 256 + 2 * (w.num_q_tokens + 1) * 48 + (w.num_q_tokens + 1) * (48 + 16) + 4096      # planning part, generous
+    assert lo < need_all
+    dw.ws_bytes = lo
+    dw.attention(); torch.cuda.synchronize(); dw.check_health()
+    assert _split_groups(dw) == 0
+    d = (dw.out.view(torch.bfloat16).double() - out1.view(torch.bfloat16).double()).abs()
+    assert float(d.max()) <= OUT_MAX and float((dw.lse - lse1).abs().max()) <= 1e-4
+    dw.ws_bytes = need_all
+
+
+def test_kv_range_splits_with_key_mask_and_batch():
+    """Four requests' questions over long contexts, 6 % of the cached keys masked (MINIPIC_KEY_MASK): split chunks that
+    consist of masked keys only for some rows, merged with the rest."""
+    w = W.rag_partial_prefill(name="splitmask", seed=77, hq=16, hkv=4, num_reqs=4, pool_spans=30, spans_per_req=11, span_min=256,
+                              span_max=640, uncached_per_req=0, suffix_len=48)
+    w = W.with_masked_keys(w, seed=5, frac=0.06)
+    dw = DeviceWorkload(w, cache_fill=0x7FC1, flags=mp.MINIPIC_KEY_MASK)
+    dw.step(); torch.cuda.synchronize()
+    assert _split_groups(dw) > 0
+    compare(dw, expect_variant="prefill_sm100_tcgen05", key_mask=True)
+
+
+def test_prefill_workspace_sized_for_a_larger_call_is_accepted():
+    """A workspace sized for many tokens (no room for partial rows asked) must serve a small call: planning part only."""
+    w = W.single_request_prefill(name="wsmono", hq=32, hkv=8, d=128, theta=5e5, dtype="bf16", sigma=1.0, span_lens=[256, 144],
+                                 suffix_len=33, num_blocks=40, seed=3)
+    dw = DeviceWorkload(w)
+    big = mp.minipic_prefill_workspace_bytes(dw.cfg, 64, 60000)
+    small = mp.minipic_prefill_workspace_bytes(dw.cfg, w.num_reqs, w.num_q_tokens)
+    assert big < small, "the small call asks for partial rows, the large one does not"
+    dw.workspace = torch.empty(big, dtype=torch.uint8, device="cuda:0"); dw.ws_bytes = big
+    dw.step(); torch.cuda.synchronize()
+    compare(dw, expect_variant="prefill_sm100_tcgen05")
+    dw.ws_bytes = 1024
+    with pytest.raises(Exception):
+        dw.attention()
