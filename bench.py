@@ -431,6 +431,20 @@ def run_ours(args):
                                 "tokens_per_s_warm": w.num_q_tokens / (warm[0] * 1e-3),
                                 "tflops_warm": fl / (warm[0] * 1e-3) / 1e12, "variant": mp.minipic_last_variant()}
                 del dw
+            # one request's 64-token question over 32 K cached tokens: KV-range splits vs the same call given only the planning
+            # part of the workspace (which runs unsplit: 8 work items on 74 CTA pairs)
+            wq = W.question_over_context()
+            dq = DeviceWorkload(wq, device=dev)
+            dq.step(); torch.cuda.synchronize()
+            tq = time_calls(dq.attention, 50, 5, torch)
+            full_ws = dq.ws_bytes
+            dq.ws_bytes = 256 + (wq.num_q_tokens + 1) * 400 + 4096
+            tq0 = time_calls(dq.attention, 50, 5, torch)
+            dq.ws_bytes = full_ws
+            extras["question64_ctx32k"] = {"ms": tq[0], "ms_best": tq[1], "ms_without_kv_range_splits": tq0[0],
+                                           "tflops": wq.attention_flops() / (tq[0] * 1e-3) / 1e12, "kv_len": int(wq.max_kv_len),
+                                           "query_tokens": int(wq.num_q_tokens)}
+            del dq
             wp = W.config4(private_pool=True)
             dp = DeviceWorkload(wp, device=dev)
             dp.step(); torch.cuda.synchronize()

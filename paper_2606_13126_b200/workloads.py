@@ -287,6 +287,15 @@ def config3(seed: int = 2) -> Workload:
     return rag_partial_prefill(seed=seed)
 
 
+def question_over_context(ctx_spans: int = 64, span_len: int = 512, question: int = 64, seed: int = 8, **kw) -> Workload:
+    """ONE request whose whole context (``ctx_spans`` spans of ``span_len`` tokens + the system prefix) is already cached:
+    only the question's ``question`` tokens are computed (the partial prefill that sets TTFT once every chunk
+    hits).  Few, long work items: the shape KV-range splits are for."""
+    return rag_partial_prefill(name=f"question{question}_ctx{ctx_spans * span_len // 1024}k", seed=seed, num_reqs=1,
+                               pool_spans=ctx_spans + 4, spans_per_req=ctx_spans, span_min=span_len, span_max=span_len,
+                               uncached_per_req=0, suffix_len=question, **kw)
+
+
 def epic_linked_prefill(*, name: str = "epic_linked_prefill", seed: int = 6, hq: int = 32, hkv: int = 8, d: int = 128,
                         theta: float = 5e5, dtype: str = "bf16", sigma: float = 1.0, pool_spans: int = 200,
                         span_min: int = 128, span_max: int = 512, num_reqs: int = 32, spans_per_req: int = 10,
