@@ -457,7 +457,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanA
     const long long all_steps = (long long)red[0] * pa.hkv;
     const int per_pair = max(kSplitMinSteps, (int)((all_steps + pa.split_pairs - 1) / pa.split_pairs));
     const int cstep = max(1, per_pair / 8);
-    if (2 * red[2] > 3 * per_pair && red[2] < 65535) {   // at least one item is long enough to be cut
+    if (2 * red[2] > 3 * per_pair && red[2] < 32767) {   // at least one item is long enough to be cut (and n_kv <= 2 cost fits 16 bits)
       __syncthreads();
       if (tid < kCand) { cand_items[tid] = n_raw; cand_max[tid] = 0; }
       if (tid == 0) { s_nlong = 0; s_groups = 0; s_slots = 0; }
