@@ -181,9 +181,14 @@ int minipic_decode_attention(const minipic_config* cfg,
  * (new K/V rows, slot mapping, Q, index tables) is read from HOST memory and the result (out, lse)
  * is written to HOST memory; the resident KV cache stays on the device.  `arena` is caller-owned
  * DEVICE scratch of at least minipic_*_host_arena_bytes(...) bytes (256-byte aligned) that receives
- * the staged inputs, the workspace and the device-side result.  All copies and kernels are enqueued
- * on `cuda_stream` (cudaMemcpyAsync: pin the host buffers for true asynchrony); the call does not
- * synchronise - outputs are valid once the stream has drained.  num_new_tokens may be 0. */
+ * the staged inputs, the workspace and the device-side result.  Copies and kernels are ordered by
+ * `cuda_stream` (cudaMemcpyAsync: pin the host buffers for true asynchrony); the call does not
+ * synchronise - outputs are valid once the stream has drained.  num_new_tokens may be 0.
+ * The prefill step with more than 8192 query tokens runs as up to 16 token-range CHUNKS: Q goes up and
+ * out / lse come down on two copy streams the library creates once per device (forked from and joined
+ * back into `cuda_stream`), one attention call per chunk in between, so that the upload of chunk i + 1,
+ * the attention of chunk i and the download of chunk i - 1 overlap (the step is PCIe bound and the link
+ * is full duplex).  Rows are independent, so the cuts are invisible in the result up to rounding order. */
 size_t minipic_prefill_host_arena_bytes(const minipic_config* cfg, int32_t num_reqs, int32_t num_q_tokens,
                                         int32_t num_new_tokens, int32_t max_blocks_per_req, int32_t total_kv_len);
 int minipic_prefill_step_host(const minipic_config* cfg,

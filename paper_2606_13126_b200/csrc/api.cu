@@ -1,9 +1,12 @@
 // extern "C" boundary of libminipic.so: argument validation, dispatch, host-buffer entry points.
 // See include/minipic.h for the contract of every call.
+#include <algorithm>
 #include <atomic>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
+#include <vector>
 
 #include "internal.h"
 
@@ -292,6 +295,37 @@ void* up(A& ar, const void* host, size_t bytes, cudaStream_t s, bool* ok) {
   if (cudaMemcpyAsync(d, host, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) *ok = false;
   return d;
 }
+// ---- chunked overlap of the prefill host step: Q goes up and out / lse come down in token-range chunks on two auxiliary
+//      streams (forked from and joined back into the caller's stream), so that H2D of chunk i + 1, attention of chunk i and D2H
+//      of chunk i - 1 run at the same time: the step is PCIe bound and the link is full duplex.
+constexpr int kHostChunkMin = 8192, kHostChunksMax = 16;
+int host_chunk_tokens(int num_q_tokens) {
+  const int per = (num_q_tokens + kHostChunksMax - 1) / kHostChunksMax;
+  return per > kHostChunkMin ? per : kHostChunkMin;
+}
+struct AuxStreams { cudaStream_t h2d = nullptr, d2h = nullptr; };
+bool aux_streams(AuxStreams* out) {   // per device, created once
+  static std::mutex mu;
+  static AuxStreams per_dev[64];
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return false;
+  std::lock_guard<std::mutex> lk(mu);
+  AuxStreams& a = per_dev[dev];
+  if (!a.h2d) {
+    if (cudaStreamCreateWithFlags(&a.h2d, cudaStreamNonBlocking) != cudaSuccess) { a.h2d = nullptr; return false; }
+    if (cudaStreamCreateWithFlags(&a.d2h, cudaStreamNonBlocking) != cudaSuccess) { cudaStreamDestroy(a.h2d); a.h2d = a.d2h = nullptr; return false; }
+  }
+  *out = a;
+  return true;
+}
+// `to` waits for everything enqueued on `from` so far
+bool stream_after(cudaStream_t to, cudaStream_t from) {
+  cudaEvent_t e;
+  if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) return false;
+  const bool ok = cudaEventRecord(e, from) == cudaSuccess && cudaStreamWaitEvent(to, e, 0) == cudaSuccess;
+  cudaEventDestroy(e);   // released once the enqueued record / wait have completed
+  return ok;
+}
 }  // namespace
 
 extern "C" {
@@ -308,7 +342,9 @@ size_t minipic_prefill_host_arena_bytes(const minipic_config* cfg, int32_t num_r
   a.take((size_t)(num_reqs + 1) * 4); a.take((size_t)num_reqs * 4); a.take((size_t)(num_reqs + 1) * 4);
   a.take((size_t)total_kv_len * 4); a.take((size_t)num_q_tokens * 4); a.take((size_t)num_q_tokens * 4);
   a.take((size_t)num_q_tokens * cfg->num_q_heads * d * is); a.take((size_t)num_q_tokens * cfg->num_q_heads * 4);
-  a.take(minipic_prefill_workspace_bytes(cfg, num_reqs, num_q_tokens));
+  const int chunk = host_chunk_tokens(num_q_tokens), n_chunks = num_q_tokens > 0 ? (num_q_tokens + chunk - 1) / chunk : 1;
+  a.take(minipic_prefill_workspace_bytes(cfg, num_reqs, num_q_tokens < chunk ? num_q_tokens : chunk));
+  a.take((size_t)n_chunks * (num_reqs + 1) * 4);   // cu_q_lens of every chunk, rebased to its first token
   return align_up(a.off) + 256;
 }
 
@@ -333,7 +369,8 @@ int minipic_prefill_step_host(const minipic_config* cfg, const void* k_new_host,
   void* dv = up(ar, v_new_host, kvb, s, &ok);
   void* dslots = up(ar, slot_mapping_host, (size_t)num_new_tokens * 8, s, &ok);
   const size_t qb = (size_t)num_q_tokens * cfg->num_q_heads * d * is;
-  void* dq = up(ar, q_host, qb, s, &ok);
+  const size_t row_b = (size_t)cfg->num_q_heads * d * is;          // one query / output token
+  char* dq = (char*)ar.take(qb);                                     // filled chunk by chunk below
   void* dbt = up(ar, block_tables_host, (size_t)num_reqs * max_blocks_per_req * 4, s, &ok);
   void* dcuq = up(ar, cu_q_lens_host, (size_t)(num_reqs + 1) * 4, s, &ok);
   void* dkvl = up(ar, kv_lens_host, (size_t)num_reqs * 4, s, &ok);
@@ -341,25 +378,76 @@ int minipic_prefill_step_host(const minipic_config* cfg, const void* k_new_host,
   void* dpos = up(ar, kv_positions_host, (size_t)total_kv * 4, s, &ok);
   void* didx = up(ar, q_seq_idx_host, (size_t)num_q_tokens * 4, s, &ok);
   void* dlo = up(ar, q_vis_lo_host, (size_t)num_q_tokens * 4, s, &ok);
-  void* dout = ar.take(qb);
+  char* dout = (char*)ar.take(qb);
   float* dlse = (float*)ar.take((size_t)num_q_tokens * cfg->num_q_heads * 4);
-  const size_t wsb = minipic_prefill_workspace_bytes(cfg, num_reqs, num_q_tokens);
+  const int chunk = host_chunk_tokens(num_q_tokens), n_chunks = (num_q_tokens + chunk - 1) / chunk;
+  const size_t wsb = minipic_prefill_workspace_bytes(cfg, num_reqs, num_q_tokens < chunk ? num_q_tokens : chunk);
   void* ws = ar.take(wsb);
-  if (!ar.ok || !dout || !dlse || !ws) return MINIPIC_ERR_WORKSPACE_TOO_SMALL;
+  int* dcu_chunks = (int*)ar.take((size_t)n_chunks * (num_reqs + 1) * 4);
+  if (!ar.ok || !dq || !dout || !dlse || !ws || !dcu_chunks) return MINIPIC_ERR_WORKSPACE_TOO_SMALL;
+  (void)dcuq;
+  // ---- token-range chunks: chunk i = query tokens [t0, t1) and the requests r0 .. r1 - 1 they belong to; its cu_q_lens are
+  //      the global ones clipped to the range and rebased to t0.  Rows are independent, so any cut is legal.
+  struct Chunk { int t0, t1, r0, nr; };
+  std::vector<Chunk> chunks;
+  std::vector<int> cu_host;
+  {
+    int r = 0;
+    for (int i = 0; i < n_chunks; ++i) {
+      Chunk c{i * chunk, std::min(num_q_tokens, (i + 1) * chunk), 0, 0};
+      while (r + 1 < num_reqs && cu_q_lens_host[r + 1] <= c.t0) ++r;
+      c.r0 = r;
+      int r1 = r;
+      while (r1 < num_reqs && cu_q_lens_host[r1] < c.t1) ++r1;
+      c.nr = r1 - c.r0;
+      for (int k = 0; k <= c.nr; ++k) cu_host.push_back(std::min(std::max(cu_q_lens_host[c.r0 + k] - c.t0, 0), c.t1 - c.t0));
+      cu_host.resize((size_t)(i + 1) * (num_reqs + 1), c.t1 - c.t0);
+      chunks.push_back(c);
+    }
+  }
+  // pageable source: the driver stages it before the call returns, the vector may go
+  if (cudaMemcpyAsync(dcu_chunks, cu_host.data(), cu_host.size() * 4, cudaMemcpyHostToDevice, s) != cudaSuccess) ok = false;
   if (!ok) { check_launch("h2d"); return MINIPIC_ERR_CUDA; }
   if (num_new_tokens) {
     st = minipic_cache_write(cfg, dk, dv, (const int64_t*)dslots, num_new_tokens, k_cache, v_cache, cuda_stream);
     if (st != MINIPIC_OK) return st;
   }
-  st = minipic_prefill_attention(cfg, dq, k_cache, v_cache, (const int*)dbt, max_blocks_per_req, (const int*)dcuq,
-                                 (const int*)dkvl, (const int*)dcukv, (const int*)dpos, (const int*)didx, (const int*)dlo,
-                                 num_reqs, num_q_tokens, max_kv_len, dout, dlse, ws, wsb, cuda_stream);
-  if (st != MINIPIC_OK) return st;
-  if (cudaMemcpyAsync(out_host, dout, qb, cudaMemcpyDeviceToHost, s) != cudaSuccess ||
-      cudaMemcpyAsync(lse_host, dlse, (size_t)num_q_tokens * cfg->num_q_heads * 4, cudaMemcpyDeviceToHost, s) != cudaSuccess) {
-    check_launch("d2h");
-    return MINIPIC_ERR_CUDA;
+  AuxStreams aux;
+  const bool overlap = n_chunks > 1 && aux_streams(&aux);
+  cudaStream_t s_in = overlap ? aux.h2d : s, s_out = overlap ? aux.d2h : s;
+  if (overlap && !stream_after(s_in, s)) return MINIPIC_ERR_CUDA;   // the arena may still be in use by earlier work on s
+  if (overlap && !stream_after(s_out, s)) return MINIPIC_ERR_CUDA;
+  std::vector<cudaEvent_t> landed(n_chunks, nullptr);
+  bool cuda_ok = true;
+  for (int i = 0; i < n_chunks && cuda_ok; ++i) {   // all uploads are enqueued first: the copy engine never waits for compute
+    const Chunk& c = chunks[i];
+    cuda_ok = cudaMemcpyAsync(dq + (size_t)c.t0 * row_b, (const char*)q_host + (size_t)c.t0 * row_b, (size_t)(c.t1 - c.t0) * row_b,
+                              cudaMemcpyHostToDevice, s_in) == cudaSuccess;
+    if (overlap && cuda_ok)
+      cuda_ok = cudaEventCreateWithFlags(&landed[i], cudaEventDisableTiming) == cudaSuccess && cudaEventRecord(landed[i], s_in) == cudaSuccess;
   }
+  for (int i = 0; i < n_chunks && cuda_ok && st == MINIPIC_OK; ++i) {
+    const Chunk& c = chunks[i];
+    const int nt = c.t1 - c.t0;
+    if (overlap) cuda_ok = cudaStreamWaitEvent(s, landed[i], 0) == cudaSuccess;
+    if (!cuda_ok) break;
+    st = minipic_prefill_attention(cfg, dq + (size_t)c.t0 * row_b, k_cache, v_cache, (const int*)dbt + (size_t)c.r0 * max_blocks_per_req,
+                                   max_blocks_per_req, dcu_chunks + (size_t)i * (num_reqs + 1), (const int*)dkvl + c.r0,
+                                   (const int*)dcukv + c.r0, (const int*)dpos, (const int*)didx + c.t0, (const int*)dlo + c.t0, c.nr, nt,
+                                   max_kv_len, dout + (size_t)c.t0 * row_b, dlse + (size_t)c.t0 * cfg->num_q_heads, ws, wsb, cuda_stream);
+    if (st != MINIPIC_OK) break;
+    if (overlap) cuda_ok = stream_after(s_out, s);
+    cuda_ok = cuda_ok &&
+              cudaMemcpyAsync((char*)out_host + (size_t)c.t0 * row_b, dout + (size_t)c.t0 * row_b, (size_t)nt * row_b, cudaMemcpyDeviceToHost, s_out) == cudaSuccess &&
+              cudaMemcpyAsync(lse_host + (size_t)c.t0 * cfg->num_q_heads, dlse + (size_t)c.t0 * cfg->num_q_heads,
+                              (size_t)nt * cfg->num_q_heads * 4, cudaMemcpyDeviceToHost, s_out) == cudaSuccess;
+  }
+  for (cudaEvent_t e : landed) if (e) cudaEventDestroy(e);
+  if (overlap) {   // join: the caller's stream has drained only when every copy has
+    if (!stream_after(s, s_in) || !stream_after(s, s_out)) cuda_ok = false;
+  }
+  if (st != MINIPIC_OK) return st;
+  if (!cuda_ok) { check_launch("host step copies"); return MINIPIC_ERR_CUDA; }
   return MINIPIC_OK;
 }
 

@@ -384,6 +384,30 @@ def test_host_step_entry_points_match_device_path():
         assert hs.h2d_bytes > 0 and hs.d2h_bytes > 0
 
 
+def test_host_step_chunked_overlap_matches_device_path():
+    """More than 8192 query tokens: minipic_prefill_step_host uploads Q and downloads out / lse in token-range chunks on its
+    own copy streams while the attention of the chunk in between runs (one attention call per chunk: the cuts fall inside
+    requests and inside spans).  Same rows as the one-call device path, up to the rounding order of the online softmax;
+    repeated calls on the same arena (the next upload may not overtake the previous download) stay identical."""
+    w = W.long_context_prefill(name="hostchunks", seed=12, hq=8, hkv=2, num_reqs=3, slots_per_req=24, span_len=512, suffix_len=77)
+    assert w.num_q_tokens > 2 * 8192 and w.num_q_tokens % 8192 != 0
+    dw = DeviceWorkload(w)
+    hs = HostStep(dw)
+    hs.run(); torch.cuda.synchronize()
+    o1, l1 = hs.out_f64().copy(), hs.lse_f64().copy()
+    dw2 = DeviceWorkload(w); dw2.step(); torch.cuda.synchronize(); dw2.check_health()
+    do = np.abs(o1 - dw2.out_f64())
+    assert do.max() <= 2.0 ** -6 and do.mean() <= 1e-4, (float(do.max()), float(do.mean()))
+    assert np.abs(l1 - dw2.lse_f64()).max() <= LSE_TOL      # other item cuts: dual halves and KV-range chunks merge in another order
+    for _ in range(3):
+        hs.out.zero_(); hs.lse.zero_()
+        hs.run()
+    torch.cuda.synchronize()
+    assert np.array_equal(hs.out_f64(), o1) and np.array_equal(hs.lse_f64(), l1)
+    st = compare(dw2, rows=np.arange(0, w.num_q_tokens, 97), expect_variant="prefill_sm100_tcgen05")
+    assert st["entries"] > 0
+
+
 # --------------------------------------------------------------------------- BASELINE configs at full size
 def _sampled(w, n_rows, n_heads, seed=0):
     rng = np.random.default_rng(seed)
