@@ -94,7 +94,8 @@ constexpr int kMaxBins = 4096;
 constexpr int kDualMinTiles = 4;   // a "dual" item (see struct Item) needs at least this many KV tiles
 constexpr unsigned kWaitMaxSpins = 1u << 26;   // x (>= 30 cycles per failed try_wait) = seconds
 
-struct TileDesc { int t0, ntok, r, idx0, lo, n_kv, kv_hi, kv_len, kv_off, pad, part, rsv; };   // kv_off = cu_kv_lens[r]; pad: dual item; part: see SplitGroup
+// kv_off = cu_kv_lens[r]; pad: dual item; part: see SplitGroup.  plan_kernel pass 1 reads ints 1, 5, 9 (ntok, n_kv, pad) by index
+struct TileDesc { int t0, ntok, r, idx0, lo, n_kv, kv_hi, kv_len, kv_off, pad, part, rsv; };
 // KV-RANGE SPLITS (small grids only): an item whose tile steps exceed what one CTA pair should get is cut into chunks over
 // consecutive KV tiles; every chunk is an item of its own that writes (O normalised over the chunk, lse of the chunk) as fp32
 // into partial token slots of the workspace - chunk s of a group owns slots [base + s ntok, base + (s + 1) ntok), part = 1 +
@@ -380,6 +381,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanA
   const int b0 = blockIdx.x * kPlanThreads;
   const int tok = pa.tok;
   PlanHeader* hdr = pa.hdr;
+  asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the attention grid may start its prologue (see its scheduler)
   if (blockIdx.x == 0 && tid == 0) hdr->magic = kPlanMagic;
   auto request_of = [&](int t) {
     int lo_r = 0, hi_r = a.num_reqs;
@@ -506,17 +508,18 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanA
   for (int i = tid; i < kMaxBins; i += kPlanThreads) shist[i] = 0;
   if (tid == 0) { s_groups = 0; s_slots = 0; }
   __syncthreads();
-  // pass 1: histogram of the (chunk) costs
+  // pass 1: histogram of the (chunk) costs - from the shared-memory copy when pass 0 made one
+  const bool cached = pa.split_pairs > 0 && n_raw <= kPlanCache;
   for (int i = tid; i < n_raw; i += kPlanThreads) {
-    const TileDesc td = load_desc(pa.tmp + i);
+    int cost, n_kv, ntok;
+    if (cached) { cost = s_cost[i]; n_kv = s_nkv[i]; ntok = s_ntk[i]; }
+    else { const int* src = reinterpret_cast<const int*>(pa.tmp + i); ntok = __ldcg(src + 1); n_kv = __ldcg(src + 5); cost = __ldcg(src + 9) ? (n_kv + 1) >> 1 : n_kv; }
     int ct;
-    const int ns = split_count(tile_cost(td), td.n_kv, tsplit, &ct);
-    if (ns == 1) { atomicAdd(&shist[min(tile_cost(td), kMaxBins - 1)], 1); continue; }
+    const int ns = split_count(cost, n_kv, tsplit, &ct);
+    if (ns == 1) { atomicAdd(&shist[min(cost, kMaxBins - 1)], 1); continue; }
     for (int sidx = 0; sidx < ns; ++sidx) {
-      TileDesc ch = td;
-      ch.n_kv = min(ct, td.n_kv - sidx * ct);
-      ch.pad = dual_flag(pa.dual_ok, td.ntok, tok, ch.n_kv);
-      atomicAdd(&shist[min(tile_cost(ch), kMaxBins - 1)], 1);
+      const int nk = min(ct, n_kv - sidx * ct);
+      atomicAdd(&shist[min(dual_flag(pa.dual_ok, ntok, tok, nk) ? (nk + 1) >> 1 : nk, kMaxBins - 1)], 1);
     }
   }
   __syncthreads();
@@ -567,23 +570,35 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanA
 // allowed; with no group in the header it returns at once.
 __global__ void __launch_bounds__(256) split_merge_kernel(const PlanHeader* hdr, const SplitGroup* groups, const float* part_o,
                                                           const float* part_lse, int hq, __nv_bfloat16* out, float* lse) {
-  const int n_groups = hdr->n_groups;
+  asm volatile("griddepcontrol.wait;" ::: "memory");   // launched as a programmatic dependent of the attention grid
+  const int n_groups = *(volatile const int*)&hdr->n_groups;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   for (int g = 0; g < n_groups; ++g) {   // every block takes a slice of every group's rows (there are few groups)
     const SplitGroup sg = groups[g];
     for (int rowi = blockIdx.x * 8 + wib; rowi < sg.ntok * hq; rowi += gridDim.x * 8) {
       const int j = rowi / hq, h = rowi % hq;
+      // all loads first (nsplit <= kSplitMax, fixed trip count): two memory round trips per row instead of one per chunk
+      float ls[kSplitMax];
+      float4 os[kSplitMax];
+#pragma unroll
+      for (int sidx = 0; sidx < kSplitMax; ++sidx) {
+        const size_t prow = (size_t)(sg.base + min(sidx, sg.nsplit - 1) * sg.ntok + j) * hq + h;
+        ls[sidx] = sidx < sg.nsplit ? __ldcg(part_lse + prow) : -INFINITY;
+        os[sidx] = __ldcg(reinterpret_cast<const float4*>(part_o + prow * D + 4 * lane));
+      }
       float mx = -INFINITY;
-      for (int sidx = 0; sidx < sg.nsplit; ++sidx) mx = fmaxf(mx, part_lse[(size_t)(sg.base + sidx * sg.ntok + j) * hq + h]);
+#pragma unroll
+      for (int sidx = 0; sidx < kSplitMax; ++sidx) mx = fmaxf(mx, ls[sidx]);
       float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
       float wsum_ = 0.f;
       if (mx > -INFINITY) {
-        for (int sidx = 0; sidx < sg.nsplit; ++sidx) {
-          const size_t prow = (size_t)(sg.base + sidx * sg.ntok + j) * hq + h;
-          const float wgt = __expf(part_lse[prow] - mx);   // e^{-inf} = 0: a chunk with no visible key for this row
-          const float4 o = *reinterpret_cast<const float4*>(part_o + prow * D + 4 * lane);
-          acc.x += wgt * o.x; acc.y += wgt * o.y; acc.z += wgt * o.z; acc.w += wgt * o.w;
-          wsum_ += wgt;
+#pragma unroll
+        for (int sidx = 0; sidx < kSplitMax; ++sidx) {   // fixed order: bit reproducible
+          const float wgt = __expf(ls[sidx] - mx);       // e^{-inf} = 0: no such chunk, or a chunk with no visible key for this row
+          if (sidx < sg.nsplit && wgt > 0.f) {            // (the guard keeps 0 x NaN of a never-written slot out)
+            acc.x += wgt * os[sidx].x; acc.y += wgt * os[sidx].y; acc.z += wgt * os[sidx].z; acc.w += wgt * os[sidx].w;
+            wsum_ += wgt;
+          }
         }
       }
       const float inv = wsum_ > 0.f ? 1.f / wsum_ : 0.f;
@@ -789,7 +804,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
   cluster_sync_all();   // barriers of BOTH CTAs are initialised before anyone arrives remotely
   tc_fence_after();
   const uint32_t tmem = sm.tmem_base;
-  const int n_items = prm.hdr->n_tiles * prm.hkv;
+  if (kDual) asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // split_merge_kernel (small grids) may queue up behind the tail
 
   if (warp >= 12) {
     reg_dec<kRegsCtl>();
@@ -797,6 +812,11 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       // ============================================================ scheduler (leader only): item ring of both CTAs
       const uint32_t ring_l = smem_u32(sm.ring), ring_p = mapa(ring_l, 1), full_p = mapa(bar(SCHED_FULL), 1);
       if (lane == 0) {
+        // PROGRAMMATIC DEPENDENT LAUNCH: this grid may start while plan_kernel is still sorting (its blocks signal
+        // launch_dependents at once), so the launch latency and the prologue above overlap the plan.  Only this thread reads
+        // what the plan writes (item count, sorted descriptors): it waits here for the plan grid to complete and flush.
+        asm volatile("griddepcontrol.wait;" ::: "memory");
+        const int n_items = *(volatile const int*)&prm.hdr->n_tiles * prm.hkv;
         for (uint32_t it_n = 0;; ++it_n) {
           const int slot = it_n & (kRing - 1);
           w.wait(bar(SCHED_EMPTY + slot), ((it_n / kRing) & 1) ^ 1);
@@ -1516,7 +1536,16 @@ bool launch_gk(const Ctx& c, const CUtensorMap& mq, const CUtensorMap& mk, const
     }
     if (dev >= 0 && dev < 64) attr_done[dev] = true;
   }
-  prefill_sm100_kernel<G, kKeyMask, kDual><<<sms, kThreads, smem, c.stream>>>(mq, mk, mv, mo, prm);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(sms); cfg.blockDim = dim3(kThreads); cfg.dynamicSmemBytes = smem; cfg.stream = c.stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // overlap with the tail of plan_kernel (griddepcontrol)
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr; cfg.numAttrs = 1;
+  if (cudaLaunchKernelEx(&cfg, prefill_sm100_kernel<G, kKeyMask, kDual>, mq, mk, mv, mo, prm) != cudaSuccess) {
+    note_error("prefill_sm100: cudaLaunchKernelEx failed");
+    return false;
+  }
   note_launch();
   return true;
 }
@@ -1656,7 +1685,17 @@ bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
     case 8: ok = launch_g<8>(c, mq, mk, mv, mo, prm, sms); break;
   }
   if (ok && part_cap > 0) {   // the plan may have split items: combine their partial rows (no group: the kernel returns at once)
-    split_merge_kernel<<<sms, 256, 0, c.stream>>>(hdr, groups, part_o, part_lse, c.hq, (__nv_bfloat16*)a.out, a.lse);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(sms); cfg.blockDim = dim3(256); cfg.stream = c.stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;   // its blocks take the SMs the attention grid's tail frees
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    if (cudaLaunchKernelEx(&cfg, split_merge_kernel, (const PlanHeader*)hdr, (const SplitGroup*)groups, (const float*)part_o,
+                           (const float*)part_lse, c.hq, (__nv_bfloat16*)a.out, a.lse) != cudaSuccess) {
+      note_error("prefill_sm100: cudaLaunchKernelEx(split_merge) failed");
+      return false;
+    }
     note_launch(1);
   }
   return ok;
