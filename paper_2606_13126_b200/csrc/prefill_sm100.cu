@@ -95,7 +95,8 @@ constexpr int kDualMinTiles = 4;   // a "dual" item (see struct Item) needs at l
 constexpr unsigned kWaitMaxSpins = 1u << 26;   // x (>= 30 cycles per failed try_wait) = seconds
 
 // kv_off = cu_kv_lens[r]; pad: dual item; part: see SplitGroup.  plan_kernel pass 1 reads ints 1, 5, 9 (ntok, n_kv, pad) by index
-struct TileDesc { int t0, ntok, r, idx0, lo, n_kv, kv_hi, kv_len, kv_off, pad, part, rsv; };
+struct alignas(16) TileDesc { int t0, ntok, r, idx0, lo, n_kv, kv_hi, kv_len, kv_off, pad, part, rsv; };
+static_assert(sizeof(TileDesc) == 48, "three 16-byte words");
 // KV-RANGE SPLITS (small grids only): an item whose tile steps exceed what one CTA pair should get is cut into chunks over
 // consecutive KV tiles; every chunk is an item of its own that writes (O normalised over the chunk, lse of the chunk) as fp32
 // into partial token slots of the workspace - chunk s of a group owns slots [base + s ntok, base + (s + 1) ntok), part = 1 +
@@ -508,18 +509,31 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanA
   for (int i = tid; i < kMaxBins; i += kPlanThreads) shist[i] = 0;
   if (tid == 0) { s_groups = 0; s_slots = 0; }
   __syncthreads();
-  // pass 1: histogram of the (chunk) costs - from the shared-memory copy when pass 0 made one
+  // pass 1: histogram of the (chunk) costs - from the shared-memory copy when pass 0 made one (only then can items be cut)
   const bool cached = pa.split_pairs > 0 && n_raw <= kPlanCache;
-  for (int i = tid; i < n_raw; i += kPlanThreads) {
-    int cost, n_kv, ntok;
-    if (cached) { cost = s_cost[i]; n_kv = s_nkv[i]; ntok = s_ntk[i]; }
-    else { const int* src = reinterpret_cast<const int*>(pa.tmp + i); ntok = __ldcg(src + 1); n_kv = __ldcg(src + 5); cost = __ldcg(src + 9) ? (n_kv + 1) >> 1 : n_kv; }
-    int ct;
-    const int ns = split_count(cost, n_kv, tsplit, &ct);
-    if (ns == 1) { atomicAdd(&shist[min(cost, kMaxBins - 1)], 1); continue; }
-    for (int sidx = 0; sidx < ns; ++sidx) {
-      const int nk = min(ct, n_kv - sidx * ct);
-      atomicAdd(&shist[min(dual_flag(pa.dual_ok, ntok, tok, nk) ? (nk + 1) >> 1 : nk, kMaxBins - 1)], 1);
+  if (cached) {
+    for (int i = tid; i < n_raw; i += kPlanThreads) {
+      const int cost = s_cost[i], n_kv = s_nkv[i], ntok = s_ntk[i];
+      int ct;
+      const int ns = split_count(cost, n_kv, tsplit, &ct);
+      if (ns == 1) { atomicAdd(&shist[min(cost, kMaxBins - 1)], 1); continue; }
+      for (int sidx = 0; sidx < ns; ++sidx) {
+        const int nk = min(ct, n_kv - sidx * ct);
+        atomicAdd(&shist[min(dual_flag(pa.dual_ok, ntok, tok, nk) ? (nk + 1) >> 1 : nk, kMaxBins - 1)], 1);
+      }
+    }
+  } else {   // large grids (thousands of items, nothing is cut): four descriptors in flight per thread, two words of each
+    for (int i0 = tid; i0 < n_raw; i0 += 4 * kPlanThreads) {
+      int nk[4], pd[4];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const int i = min(i0 + u * kPlanThreads, n_raw - 1);
+        const int* src = reinterpret_cast<const int*>(pa.tmp + i);
+        nk[u] = __ldcg(src + 5); pd[u] = __ldcg(src + 9);
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u)
+        if (i0 + u * kPlanThreads < n_raw) atomicAdd(&shist[min(pd[u] ? (nk[u] + 1) >> 1 : nk[u], kMaxBins - 1)], 1);
     }
   }
   __syncthreads();
@@ -543,6 +557,24 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanA
   if (tid == kPlanThreads - 1) hdr->n_tiles = base;   // total number of descriptors after the splits
   __syncthreads();
   // pass 2: scatter
+  if (!cached) {   // plain scatter, four 48-byte descriptors in flight per thread
+    for (int i0 = tid; i0 < n_raw; i0 += 4 * kPlanThreads) {
+      uint4 v[4][3];
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const uint4* src = reinterpret_cast<const uint4*>(pa.tmp + min(i0 + u * kPlanThreads, n_raw - 1));
+        v[u][0] = __ldcg(src); v[u][1] = __ldcg(src + 1); v[u][2] = __ldcg(src + 2);
+      }
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        if (i0 + u * kPlanThreads >= n_raw) continue;
+        const int n_kv = (int)v[u][1].y, cost = v[u][2].y ? (n_kv + 1) >> 1 : n_kv;   // ints 5 (n_kv) and 9 (pad)
+        uint4* dst = reinterpret_cast<uint4*>(pa.sorted + atomicAdd(&shist[min(cost, kMaxBins - 1)], 1));
+        dst[0] = v[u][0]; dst[1] = v[u][1]; dst[2] = v[u][2];
+      }
+    }
+    return;   // no groups: the header's counters stay 0
+  }
   for (int i = tid; i < n_raw; i += kPlanThreads) {
     const TileDesc td = load_desc(pa.tmp + i);
     int ct;
