@@ -90,6 +90,10 @@ constexpr int kStageBytes = 4096;            // epilogue staging per softmax war
 constexpr int kThreads = 512;
 constexpr int kRegsSoftmax = 184, kRegsRot = 96, kRegsCtl = 48;
 static_assert(256 * kRegsSoftmax + 128 * kRegsRot + 128 * kRegsCtl <= 65536, "setmaxnreg split exceeds the CTA register pool");
+#ifndef MINIPIC_PEARLY
+#define MINIPIC_PEARLY 1
+#endif
+constexpr int kPEarly = MINIPIC_PEARLY;   // 32-key chunks of P published early (P_HALF): PV of those keys starts under the remaining exps
 constexpr int kMaxBins = 4096;
 constexpr int kDualMinTiles = 4;   // a "dual" item (see struct Item) needs at least this many KV tiles
 constexpr unsigned kWaitMaxSpins = 1u << 26;   // x (>= 30 cycles per failed try_wait) = seconds
@@ -678,7 +682,8 @@ enum Bar {
   P_FULL = S_FULL + 2,                  // [2] leader, 4 softmax warps per CTA
   O_FULL = P_FULL + 2,                  // [2] multicast
   O_FREE = O_FULL + 2,                  // [2] leader, 4 softmax warps per CTA
-  XCHG = O_FREE + 2,                    // local, 128 tile-B softmax threads: (O_B, m_B, l_B) of a dual item are in shared memory
+  P_HALF = O_FREE + 2,                  // [2] leader, 4 softmax warps per CTA: P of the tile's first 64 keys is in TMEM
+  XCHG = P_HALF + 2,                    // local, 128 tile-B softmax threads: (O_B, m_B, l_B) of a dual item are in shared memory
   NUM_BARS
 };
 static_assert(NUM_BARS <= 36, "barrier array too small");
@@ -824,6 +829,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
     for (int x = 0; x < 2; ++x) {
       mbar_init(bar(S_FULL + x), 1); mbar_init(bar(P_FULL + x), 8); mbar_init(bar(O_FULL + x), 1); mbar_init(bar(O_FREE + x), 8);
     }
+    mbar_init(bar(P_HALF), 8); mbar_init(bar(P_HALF + 1), 8);
     mbar_init(bar(XCHG), 128);
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
@@ -979,7 +985,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
       const uint32_t k_lo = ((smem_u32(sm.k[0]) >> 4) & 0x3FFF) | (1u << 16);          // + stage * 1024
       const uint32_t v_lo = ((smem_u32(sm.v[0]) >> 4) & 0x3FFF) | (1u << 16);          // + stage * 1024
       uint32_t k_st = 0, k_ph = 0, v_st = 0, v_ph = 0;   // next K / V stage to consume and its full-barrier parity
-      uint32_t ph = 0;   // bit 0,1: P_FULL parity of tile A,B; bit 2,3: O_FREE; bit 4: Q_READY; bit 5: V_FIX
+      uint32_t ph = 0;   // bit 0,1: P_FULL parity of tile A,B; bit 2,3: O_FREE; bit 4: Q_READY; bit 5: V_FIX; bit 6,7: P_HALF
       for (uint32_t it_n = 0;; ++it_n) {
         const int slot = it_n & (kRing - 1);
         w.wait_cl(bar(SCHED_FULL + slot), (it_n / kRing) & 1);
@@ -1034,6 +1040,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
               w.wait(bar(V_FULL + v_st), v_ph);
               w.wait(bar(V_PEER + v_st), v_ph);
               if (vfix && (x ? n_a + j : j) == n - 1) { w.wait(bar(V_FIX), (ph >> 5) & 1); ph ^= 32u; }
+              w.wait(bar(P_HALF + x), (ph >> (6 + x)) & 1); ph ^= 64u << x;
               w.wait(bar(P_FULL + x), (ph >> x) & 1); ph ^= 1u << x;
               if (j == 0) { w.wait(bar(O_FREE + x), ((ph >> (2 + x)) & 1) ^ 1); ph ^= 4u << x; }
               tc_fence_after();
@@ -1076,16 +1083,26 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           for (int x = 0; x < 2; ++x) {
             const int nx = x ? nx1 : n;
             const bool do_pv = i < nx, do_qk = i + 1 < nx;
+            // PV in two halves: the first 64 keys' P is published (P_HALF) while the softmax warps still run the exps of the
+            // other 64, so half of PV is off the P -> PV -> QK -> S chain that bounds a tile slot's period
             if (do_pv) {
-              w.wait(bar(P_FULL + x), (ph >> x) & 1); ph ^= 1u << x;
+              w.wait(bar(P_HALF + x), (ph >> (6 + x)) & 1); ph ^= 64u << x;
               if (i == 0) { w.wait(bar(O_FREE + x), ((ph >> (2 + x)) & 1) ^ 1); ph ^= 4u << x; }
             }
             tc_fence_after();
+            const uint32_t b_lo_v = v_lo + v_st * (kVTileBytes >> 4);
             if (do_pv && elect_one()) {
-              const uint32_t b_lo = v_lo + v_st * (kVTileBytes >> 4);
 #pragma unroll
-              for (int ks = 0; ks < BN / 16; ++ks)
-                umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, b_lo + ks * (2 * kVGroupBytes >> 4), idesc_pv, (i > 0 || ks > 0));
+              for (int ks = 0; ks < 2 * kPEarly; ++ks)
+                umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, b_lo_v + ks * (2 * kVGroupBytes >> 4), idesc_pv, (i > 0 || ks > 0));
+            }
+            __syncwarp();
+            if (do_pv) { w.wait(bar(P_FULL + x), (ph >> x) & 1); ph ^= 1u << x; }
+            tc_fence_after();
+            if (do_pv && elect_one()) {
+#pragma unroll
+              for (int ks = 2 * kPEarly; ks < BN / 16; ++ks)
+                umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, b_lo_v + ks * (2 * kVGroupBytes >> 4), idesc_pv, 1);
               if (i == nx - 1) tc_commit(bar(O_FULL + x));
               TRACE(1, 20 + x);
             }
@@ -1450,6 +1467,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
 #pragma unroll
             for (int c = 0; c < 16; ++c) pk[c] = 0u;
             tmem_st16(t_s + 16 * h, pk);
+            if (h == kPEarly - 1) { tmem_wait_st(); tc_fence_before(); __syncwarp(); if (lane == 0) mbar_arrive_cl(lbar(P_HALF + x)); }
             continue;
           }
 #pragma unroll
@@ -1461,6 +1479,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
             pk[c] = pack_bf16(p0, p1);
           }
           tmem_st16(t_s + 16 * h, pk);
+          if (h == kPEarly - 1) { tmem_wait_st(); tc_fence_before(); __syncwarp(); if (lane == 0) mbar_arrive_cl(lbar(P_HALF + x)); }   // first keys: PV may start
         }
         {
           float a0, a1;
