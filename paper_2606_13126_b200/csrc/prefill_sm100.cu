@@ -1097,6 +1097,8 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
                 umma_ts(tmem + (2 + x) * BN, tmem + x * BN + ks * 8, b_lo_v + ks * (2 * kVGroupBytes >> 4), idesc_pv, (i > 0 || ks > 0));
             }
             __syncwarp();
+            // the next K tile is waited for HERE, while the softmax warps still work on P: off the P -> PV -> QK -> S chain
+            if (do_qk && !k_waited) { w.wait(bar(K_READY + k_st), k_ph); k_waited = true; }
             if (do_pv) { w.wait(bar(P_FULL + x), (ph >> x) & 1); ph ^= 1u << x; }
             tc_fence_after();
             if (do_pv && elect_one()) {
@@ -1107,8 +1109,6 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
               TRACE(1, 20 + x);
             }
             __syncwarp();
-            // the next K tile is only needed now: the PV above is already running while this waits on the rotation
-            if (do_qk && !k_waited) { w.wait(bar(K_READY + k_st), k_ph); k_waited = true; tc_fence_after(); }
             if (elect_one()) {
               if (x == 1) tc_commit(bar(V_EMPTY + v_st));
               if (do_qk) qk(x, k_st);
