@@ -74,6 +74,13 @@ constexpr int kKStages = MINIPIC_KSTAGES, kVStages = MINIPIC_VSTAGES, kRing = 4;
 //    is what bounds the period, not the dependency chain;
 //  * named-barrier ping-pong that makes the tile-A and tile-B warps of a scheduler take turns in the exp phase: 2.09 ms;
 //  * 2, 3 or 4 K / V stages: 2.034 - 2.048 ms (no effect).
+// Measured after the early P publish (config 5 at 2.00 ms):
+//  * Q tile B rotated by the four K rotation warps as soon as the Q tile lands (they are idle then), tile A by its softmax
+//    warps: 2.08 ms, config 3 0.353 -> 0.410 ms - the rotation warps then run late on K tile 2 of short items;
+//  * mbarrier.test_wait (no suspend) in the issuer's waits for P: 2.014 ms - the spinning warp takes issue slots from the
+//    softmax warps of its scheduler;  2 or 3 chunks of P published early instead of 1: 2.015 / 1.999 ms;
+//  * dual items: tile-A warps read O_B straight from TMEM (no 64 KB exchange buffer): config 3 0.375 -> 0.392 ms, slot B's
+//    accumulator stays busy until the deferred epilogue; with the freed shared memory 3 - 4 K / V stages: no effect.
 // Two restructurings of the softmax were measured on config 5 (2.38 ms at the time) and dropped:
 //  * every 2nd / 3rd / 4th exp2 pair on the FMA pipe (Cody-Waite + cubic minimax) instead of MUFU: 2.59 / 2.56 / 2.45 ms -
 //    the softmax warps are issue / latency bound, not MUFU bound, at this tile period;
