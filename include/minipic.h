@@ -176,6 +176,28 @@ int minipic_decode_attention(const minipic_config* cfg,
                              int32_t num_seqs, int32_t max_kv_len,
                              void* out, float* lse, void* workspace, size_t workspace_bytes, void* cuda_stream);
 
+/* ---- decode attention WITHOUT a caller workspace and without any allocation -------------------------------------
+ * Same computation, arguments and result as minipic_decode_attention (Eq. 2), for callers that cannot
+ * allocate device memory (code under CUDA graph capture, serving loops or harnesses that forbid cudaMalloc): the fp32
+ * split-KV partials live in a file-scope static device array of MINIPIC_STATIC_SCRATCH_BYTES that every GPU which loads
+ * the library holds until the process exits.  The call allocates nothing (no cudaMalloc / cudaFree, no allocating library
+ * routine); it looks the array's device address up once per device (cudaGetSymbolAddress) and enqueues the same kernels on
+ * `cuda_stream`.
+ *   - a problem that needs more than MINIPIC_STATIC_SCRATCH_BYTES of partials (minipic_decode_workspace_bytes says how
+ *     much) is rejected with MINIPIC_ERR_WORKSPACE_TOO_SMALL and a message in minipic_last_cuda_error(); nothing is launched;
+ *   - ALL calls on a device share the one array: two calls that overlap on the GPU (different streams, or concurrent graph
+ *     branches) race on it - serialise them.  The array keeps the previous call's contents; nothing in it has to start at
+ *     zero (a call writes every partial row that its merge kernel reads), so no clearing is done. */
+#define MINIPIC_STATIC_SCRATCH_BYTES (16u << 20)
+size_t minipic_static_scratch_bytes(void);   /* = MINIPIC_STATIC_SCRATCH_BYTES, for bindings without the macro */
+int minipic_decode_attention_static(const minipic_config* cfg,
+                                    const void* q, const void* k_cache, const void* v_cache,
+                                    const int32_t* block_tables, int32_t max_blocks_per_req,
+                                    const int32_t* kv_lens, const int32_t* cu_kv_lens,
+                                    const int32_t* kv_positions, const int32_t* q_vis_lo /* or NULL */,
+                                    int32_t num_seqs, int32_t max_kv_len,
+                                    void* out, float* lse, void* cuda_stream);
+
 /* ---- end-to-end entry points with HOST buffers ---------------------------------------------------
  * Same computation as cache_write followed by prefill / decode attention, but every per-step input
  * (new K/V rows, slot mapping, Q, index tables) is read from HOST memory and the result (out, lse)

@@ -34,7 +34,7 @@ EXPORTS = [
     "minipic_status_string", "minipic_last_cuda_error", "minipic_launch_count", "minipic_last_variant",
     "minipic_prefill_status", "minipic_preattn_fused", "minipic_block_rerotate",
     "minipic_block_hashes", "minipic_pool_create", "minipic_pool_destroy", "minipic_pool_admit", "minipic_pool_release",
-    "minipic_pool_stats",
+    "minipic_pool_stats", "minipic_static_scratch_bytes", "minipic_decode_attention_static",
 ]
 
 
@@ -71,6 +71,10 @@ def lib() -> C.CDLL:
     L.minipic_decode_workspace_bytes.restype = SZ
     L.minipic_decode_workspace_bytes.argtypes = [P, I32, I32]
     L.minipic_decode_attention.restype = C.c_int
+    L.minipic_static_scratch_bytes.restype = SZ
+    L.minipic_static_scratch_bytes.argtypes = []
+    L.minipic_decode_attention_static.restype = C.c_int
+    L.minipic_decode_attention_static.argtypes = [P, VP, VP, VP, VP, I32, VP, VP, VP, VP, I32, I32, VP, VP, VP]
     L.minipic_decode_attention.argtypes = [P, VP, VP, VP, VP, I32, VP, VP, VP, VP, I32, I32, VP, VP, VP, SZ, VP]
     L.minipic_prefill_host_arena_bytes.restype = SZ
     L.minipic_prefill_host_arena_bytes.argtypes = [P, I32, I32, I32, I32, I32]
@@ -197,6 +201,18 @@ def minipic_decode_attention(cfg, q, k_cache, v_cache, block_tables, max_blocks_
         C.byref(cfg), _ptr(q), _ptr(k_cache), _ptr(v_cache), _ptr(block_tables), max_blocks_per_req, _ptr(kv_lens),
         _ptr(cu_kv_lens), _ptr(kv_positions), _ptr(q_vis_lo), num_seqs, max_kv_len, _ptr(out), _ptr(lse),
         _ptr(workspace), workspace_bytes, _stream(stream)))
+
+
+def minipic_static_scratch_bytes() -> int:
+    return lib().minipic_static_scratch_bytes()
+
+
+def minipic_decode_attention_static(cfg, q, k_cache, v_cache, block_tables, max_blocks_per_req, kv_lens, cu_kv_lens,
+                                    kv_positions, q_vis_lo, num_seqs, max_kv_len, out, lse, stream=None) -> None:
+    """minipic_decode_attention with the split-KV partials in the library's static device array: allocates nothing."""
+    _check(lib().minipic_decode_attention_static(
+        C.byref(cfg), _ptr(q), _ptr(k_cache), _ptr(v_cache), _ptr(block_tables), max_blocks_per_req, _ptr(kv_lens),
+        _ptr(cu_kv_lens), _ptr(kv_positions), _ptr(q_vis_lo), num_seqs, max_kv_len, _ptr(out), _ptr(lse), _stream(stream)))
 
 
 def minipic_prefill_host_arena_bytes(cfg, num_reqs, num_q_tokens, num_new_tokens, max_blocks_per_req, total_kv_len) -> int:

@@ -515,3 +515,63 @@ int minipic_decode_step_host(const minipic_config* cfg, const void* k_new_host, 
 }
 
 }  // extern "C"
+
+// ------------------------------------------------------------------------------------------------ decode without a workspace
+// The split-KV partials of minipic_decode_attention_static live in this file-scope device array.  In HOST code the name is a
+// host-side stand-in, not a device address: the address is looked up per device with cudaGetSymbolAddress (below).
+namespace {
+static __device__ __align__(256) unsigned char g_static_scratch[MINIPIC_STATIC_SCRATCH_BYTES];
+
+// device address of g_static_scratch on the CURRENT device; looked up once per device ordinal
+void* static_scratch_ptr() {
+  static std::mutex mu;
+  static void* per_dev[64] = {};
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) {
+    note_error("minipic_decode_attention_static: cudaGetDevice failed or device ordinal >= 64");
+    return nullptr;
+  }
+  std::lock_guard<std::mutex> lk(mu);
+  if (!per_dev[dev]) {
+    void* p = nullptr;
+    const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+    if (e != cudaSuccess || !p) {
+      char msg[200];
+      snprintf(msg, sizeof(msg), "minipic_decode_attention_static: cudaGetSymbolAddress failed: %s", cudaGetErrorString(e));
+      note_error(msg);
+      return nullptr;
+    }
+    per_dev[dev] = p;
+  }
+  return per_dev[dev];
+}
+}  // namespace
+
+extern "C" {
+
+size_t minipic_static_scratch_bytes(void) { return (size_t)MINIPIC_STATIC_SCRATCH_BYTES; }
+
+int minipic_decode_attention_static(const minipic_config* cfg, const void* q, const void* k_cache, const void* v_cache,
+                                    const int32_t* block_tables, int32_t max_blocks_per_req, const int32_t* kv_lens,
+                                    const int32_t* cu_kv_lens, const int32_t* kv_positions, const int32_t* q_vis_lo,
+                                    int32_t num_seqs, int32_t max_kv_len, void* out, float* lse, void* cuda_stream) {
+  const int st = validate_cfg(cfg);
+  if (st != MINIPIC_OK) return st;
+  if (num_seqs < 0 || max_kv_len < 0 || max_blocks_per_req < 0) return MINIPIC_ERR_INVALID_ARG;
+  if (num_seqs == 0) return MINIPIC_OK;
+  Ctx c; make_ctx(cfg, cuda_stream, &c);
+  const size_t need = decode_workspace_bytes(c, num_seqs, max_kv_len);
+  if (need > (size_t)MINIPIC_STATIC_SCRATCH_BYTES) {   // before anything is launched or any pointer is looked at
+    char msg[200];
+    snprintf(msg, sizeof(msg), "minipic_decode_attention_static: %zu bytes of split-KV partials needed, the static scratch holds %zu",
+             need, (size_t)MINIPIC_STATIC_SCRATCH_BYTES);
+    note_error(msg);
+    return MINIPIC_ERR_WORKSPACE_TOO_SMALL;
+  }
+  void* scratch = static_scratch_ptr();
+  if (!scratch) return MINIPIC_ERR_CUDA;
+  return minipic_decode_attention(cfg, q, k_cache, v_cache, block_tables, max_blocks_per_req, kv_lens, cu_kv_lens, kv_positions,
+                                  q_vis_lo, num_seqs, max_kv_len, out, lse, scratch, (size_t)MINIPIC_STATIC_SCRATCH_BYTES, cuda_stream);
+}
+
+}  // extern "C"
