@@ -79,6 +79,11 @@ constexpr int kKStages = MINIPIC_KSTAGES, kVStages = MINIPIC_VSTAGES, kRing = 4;
 //    warps: 2.08 ms, config 3 0.353 -> 0.410 ms - the rotation warps then run late on K tile 2 of short items;
 //  * mbarrier.test_wait (no suspend) in the issuer's waits for P: 2.014 ms - the spinning warp takes issue slots from the
 //    softmax warps of its scheduler;  2 or 3 chunks of P published early instead of 1: 2.015 / 1.999 ms;
+//  * Q double buffer in the 64 KB that the non-dual kernels do not need for the exchange buffer, the producer fetching the NEXT
+//    item's Q tiles during the current item (rotation still at the boundary, by the softmax warps): config 5 2.012 -> 2.001 ms,
+//    span-only input 2.310 -> 2.298 ms, dense causal 1.034 -> 1.048 ms; with Q and K pre-rotated 1.895 -> 1.840 ms - the boundary
+//    is the Q rotation itself, not the load.  On top of that, rotating the next item's Q rows in the softmax warps' wait for their
+//    next S tile ("idle" time): 2.198 ms - that wait is when the other tile slot's softmax has the sub-partition to itself;
 //  * dual items: tile-A warps read O_B straight from TMEM (no 64 KB exchange buffer): config 3 0.375 -> 0.392 ms, slot B's
 //    accumulator stays busy until the deferred epilogue; with the freed shared memory 3 - 4 K / V stages: no effect.
 // Two restructurings of the softmax were measured on config 5 (2.38 ms at the time) and dropped:
