@@ -99,11 +99,13 @@ __global__ void __launch_bounds__(256) preattn_fused_kernel(const uint4* __restr
   }
 }
 
+// ncu (r2): with plain __launch_bounds__(256) the unrolled loop took 168 registers = ONE block per SM (12 % occupancy, 0.57 of
+// HBM).  Now: at least 4 blocks per SM (<= 64 registers), the V copy issued as its own loads -> stores ahead of the K rotation.
 template <typename T>
-__global__ void __launch_bounds__(256) block_rerotate_kernel(uint4* __restrict__ k_cache, uint4* __restrict__ v_cache,
-                                                             const int* __restrict__ src, const int* __restrict__ dst,
-                                                             const int* __restrict__ delta, long long num_pairs, int hkv,
-                                                             int d, RopeParams rp) {
+__global__ void __launch_bounds__(256, 4) block_rerotate_kernel(uint4* __restrict__ k_cache, uint4* __restrict__ v_cache,
+                                                                const int* __restrict__ src, const int* __restrict__ dst,
+                                                                const int* __restrict__ delta, long long num_pairs, int hkv,
+                                                                int d, RopeParams rp) {
   constexpr int VE = Vec<T>::VE;
   const int vph = d / 2 / VE, vpr = 2 * vph;
   const int rows = hkv * kBlock;                       // (head, token) rows of one block
@@ -111,16 +113,29 @@ __global__ void __launch_bounds__(256) block_rerotate_kernel(uint4* __restrict__
   for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
     const long long p = i / (hkv * vph);
     const int h = (int)(i / vph % hkv), ci = (int)(i % vph);
+    const size_t so = ((size_t)__ldg(src + p) * rows + (size_t)h * kBlock) * vpr + ci, dofs = ((size_t)__ldg(dst + p) * rows + (size_t)h * kBlock) * vpr + ci;
+    // ---- V: a plain copy, four rows (8 vectors) in flight
+#pragma unroll 1
+    for (int r0 = 0; r0 < kBlock; r0 += 4) {
+      uint4 t[8];
+#pragma unroll
+      for (int r = 0; r < 4; ++r) { t[2 * r] = ldg_stream16(v_cache + so + (size_t)(r0 + r) * vpr); t[2 * r + 1] = ldg_stream16(v_cache + so + (size_t)(r0 + r) * vpr + vph); }
+#pragma unroll
+      for (int r = 0; r < 4; ++r) { v_cache[dofs + (size_t)(r0 + r) * vpr] = t[2 * r]; v_cache[dofs + (size_t)(r0 + r) * vpr + vph] = t[2 * r + 1]; }
+    }
+    // ---- K: dst <- R(delta) src
     float c[VE], s[VE];
     trig<VE>(rp, (long long)__ldg(delta + p), ci * VE, c, s);
-    const size_t so = ((size_t)__ldg(src + p) * rows + (size_t)h * kBlock) * vpr, dofs = ((size_t)__ldg(dst + p) * rows + (size_t)h * kBlock) * vpr;
-#pragma unroll 4
-    for (int r = 0; r < kBlock; ++r) {
-      uint4 lo = ldg_stream16(k_cache + so + (size_t)r * vpr + ci), hi = ldg_stream16(k_cache + so + (size_t)r * vpr + vph + ci);
-      const uint4 vlo = ldg_stream16(v_cache + so + (size_t)r * vpr + ci), vhi = ldg_stream16(v_cache + so + (size_t)r * vpr + vph + ci);
-      rotate_pair<T, VE>(lo, hi, c, s);
-      k_cache[dofs + (size_t)r * vpr + ci] = lo; k_cache[dofs + (size_t)r * vpr + vph + ci] = hi;
-      v_cache[dofs + (size_t)r * vpr + ci] = vlo; v_cache[dofs + (size_t)r * vpr + vph + ci] = vhi;
+#pragma unroll 1
+    for (int r0 = 0; r0 < kBlock; r0 += 4) {
+      uint4 lo[4], hi[4];
+#pragma unroll
+      for (int r = 0; r < 4; ++r) { lo[r] = ldg_stream16(k_cache + so + (size_t)(r0 + r) * vpr); hi[r] = ldg_stream16(k_cache + so + (size_t)(r0 + r) * vpr + vph); }
+#pragma unroll
+      for (int r = 0; r < 4; ++r) {
+        rotate_pair<T, VE>(lo[r], hi[r], c, s);
+        k_cache[dofs + (size_t)(r0 + r) * vpr] = lo[r]; k_cache[dofs + (size_t)(r0 + r) * vpr + vph] = hi[r];
+      }
     }
   }
 }
