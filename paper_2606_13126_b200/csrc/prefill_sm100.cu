@@ -84,6 +84,9 @@ constexpr int kKStages = MINIPIC_KSTAGES, kVStages = MINIPIC_VSTAGES, kRing = 4;
 //    span-only input 2.310 -> 2.298 ms, dense causal 1.034 -> 1.048 ms; with Q and K pre-rotated 1.895 -> 1.840 ms - the boundary
 //    is the Q rotation itself, not the load.  On top of that, rotating the next item's Q rows in the softmax warps' wait for their
 //    next S tile ("idle" time): 2.198 ms - that wait is when the other tile slot's softmax has the sub-partition to itself;
+//  * slot B writes the previous item's rows BEFORE it rotates its Q rows (slot A after), so that the two slots' softmaxes start
+//    an item half a period apart instead of in phase: 2.13 ms (and the two-step loop that keeps one copy of each code path costs
+//    3 % by itself, 2.08 ms, with the old order);
 //  * dual items: tile-A warps read O_B straight from TMEM (no 64 KB exchange buffer): config 3 0.375 -> 0.392 ms, slot B's
 //    accumulator stays busy until the deferred epilogue; with the freed shared memory 3 - 4 K / V stages: no effect.
 // Two restructurings of the softmax were measured on config 5 (2.38 ms at the time) and dropped:
