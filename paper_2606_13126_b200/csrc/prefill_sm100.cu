@@ -87,6 +87,9 @@ constexpr int kKStages = MINIPIC_KSTAGES, kVStages = MINIPIC_VSTAGES, kRing = 4;
 //  * slot B writes the previous item's rows BEFORE it rotates its Q rows (slot A after), so that the two slots' softmaxes start
 //    an item half a period apart instead of in phase: 2.13 ms (and the two-step loop that keeps one copy of each code path costs
 //    3 % by itself, 2.08 ms, with the old order);
+//  * Q rotation with the lane owning a TOKEN (row 8 rsub + k: for G = 8 one exact restart per item, no angle-addition steps, -sin
+//    formed once; ~30 % fewer instructions in the loop that takes ~3.8 K of the ~8.4 K cycles of an item boundary): span-only
+//    input 2.311 -> 2.271 ms, but dense causal 1.033 -> 1.058 ms and config 5 2.012 -> 2.027 ms;
 //  * dual items: tile-A warps read O_B straight from TMEM (no 64 KB exchange buffer): config 3 0.375 -> 0.392 ms, slot B's
 //    accumulator stays busy until the deferred epilogue; with the freed shared memory 3 - 4 K / V stages: no effect.
 // Two restructurings of the softmax were measured on config 5 (2.38 ms at the time) and dropped:
