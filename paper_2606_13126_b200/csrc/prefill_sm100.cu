@@ -224,18 +224,21 @@ struct Waiter {
     }
   }
 };
-// Debug-only event trace (-DMINIPIC_TRACE, never in the shipped library): CTA 0 records (tag, SM clock) per role.
+// Debug-only event trace (-DMINIPIC_TRACE, never in the shipped library): CTA 0 records (tag, SM clock) per role.  One thread
+// per role; its running count is a register (a global read-modify-write per event costs ~700 cycles and distorts the timeline).
+// Roles: 0 scheduler, 1 MMA issuer, 2 rotation warp 0, 3 / 4 softmax warp 0 of tile slot A / B, 5 Q / K producer, 6 V producer.
+// Tags: 40 S_FULL seen, 44 S in registers, 45 row max done, 46 exps done, 41 P_FULL; 48 / 49 before / after the Q_FULL wait, 47 Q rows
+// rotated, 42 / 43 epilogue in / out, 1000 + 4 n + dual + 2 part = item start (n KV tiles).
 #ifdef MINIPIC_TRACE
 constexpr int kTraceRoles = 8, kTraceLen = 8192;
 __device__ long long g_trace[kTraceRoles][kTraceLen][2];
 __device__ int g_trace_n[kTraceRoles];
-__device__ __forceinline__ void trace_ev(int role, int tag) {
+__device__ __forceinline__ void trace_ev(int role, int tag, int& n) {
   if (blockIdx.x != 0) return;
-  const int n = g_trace_n[role];
-  if (n < kTraceLen) { g_trace[role][n][0] = tag; g_trace[role][n][1] = clock64(); g_trace_n[role] = n + 1; }
+  if (n < kTraceLen) { g_trace[role][n][0] = tag; g_trace[role][n][1] = clock64(); ++n; g_trace_n[role] = n; }
 }
-#define TRACE(role, tag) trace_ev(role, tag)
-#define TRACE_L0(role, tag) do { if (lane == 0) trace_ev(role, tag); } while (0)
+#define TRACE(role, tag) trace_ev(role, tag, trace_n)
+#define TRACE_L0(role, tag) do { if (lane == 0) trace_ev(role, tag, trace_n); } while (0)
 #else
 #define TRACE(role, tag) do { } while (0)
 #define TRACE_L0(role, tag) do { } while (0)
@@ -840,6 +843,9 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
     sm.step1[threadIdx.x - 64] = prm.step1[threadIdx.x - 64];
     sm.step4[threadIdx.x - 64] = prm.step4[threadIdx.x - 64];
   }
+#ifdef MINIPIC_TRACE
+  int trace_n = 0;
+#endif
   if (threadIdx.x == 0) {
     if (smem_u32(smem_raw) & 1023u) atomicCAS(&prm.hdr->err, 0, 2);   // swizzled tiles need a 1024-byte aligned base
     for (int s = 0; s < kRing; ++s) { mbar_init(bar(SCHED_FULL + s), 1); mbar_init(bar(SCHED_EMPTY + s), 30); }
@@ -948,7 +954,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
             if (__any_sync(0xffffffffu, w.dead)) break;   // a timed-out wait: stop issuing, let the kernel drain
             if (lane < kKeysCta / kBlock) tma_load_4d(smem_u32(sm.k[st]) + lane * 4096, &tmap_k, bar(K_FULL + st), 0, 0, 0, y);
             ++kc;
-            TRACE_L0(0, 2);
+            TRACE_L0(5, 2);
           }
           if (i == 0) {  // this CTA's Q rows: (token, head-in-group), tile A then tile B
             const int ntile = it.dual ? (it.ntok_a > 0 ? 1 : 0) : (it.ntok_b > 0 ? 2 : (it.ntok_a > 0 ? 1 : 0));   // dual: both slots read tile 0
@@ -959,7 +965,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
               tma_load_3d(smem_u32(sm.q[x]) + h * kHalfBytes, &tmap_q, bar(Q_FULL), 64 * h, it.kvh * G, it.t0 + it.tb + x * TOK);
             }
             ++qc;
-            TRACE_L0(0, 3);
+            TRACE_L0(5, 3);
           }
           y = y_next;
         }
@@ -991,7 +997,7 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           if (__any_sync(0xffffffffu, w.dead)) break;
           if (lane < BN / kBlock) tma_load_4d(smem_u32(sm.v[st]) + lane * 2048, &tmap_v, bar(V_FULL + st), 0, 0, rank, y);
           ++vc;
-          TRACE_L0(0, 4);
+          TRACE_L0(6, 4);
           y = y_next;
         }
       }
@@ -1372,7 +1378,9 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
           const int tk = min((32 * rw) / G + min(lane, NTW - 1), it.ntok_x(x) - 1);
           qpx = __ldg(a.kv_positions + it.kv_off + min(it.idx0 + tile_t + tk, it.kv_len - 1));
         }
+        if ((warp & 3) == 0) TRACE_L0(3 + x, 48);
         w.wait(bar(Q_FULL), qc & 1); ++qc;
+        if ((warp & 3) == 0) TRACE_L0(3 + x, 49);
         if (rot_q) {
           Rot8 rot;
           uint64_t c1[4], s1[4], ns1[4];
@@ -1401,8 +1409,10 @@ prefill_sm100_kernel(const __grid_constant__ CUtensorMap tmap_q, const __grid_co
         __syncwarp();
         if (lane == 0) mbar_arrive_cl(lbar(Q_READY + x));
       }
+      if ((warp & 3) == 0) TRACE_L0(3 + x, 47);
       if (pe.valid) epilogue();   // previous item of this tile
       if (stop) break;
+      if ((warp & 3) == 0) TRACE_L0(3 + x, 1000 + 4 * n + (it.dual ? 1 : 0) + (it.part > 0 ? 2 : 0));
       const bool row_ok = tok_in < it.ntok_x(x);
       const int idx_first = it.idx0 + tile_t;                               // lowest query index of this tile
       const int idx_row = min(it.idx0 + tile_t + tok_in, it.kv_len - 1);    // highest visible key of this row
