@@ -466,6 +466,18 @@ def test_config3_full_sampled():
     assert gk.tobytes() == kc.tobytes() and gv.tobytes() == vc.tobytes()
 
 
+def test_question_over_context_full_size():
+    """The bench's `question64_ctx32k` extra at full size: ONE request's 64-token question over 32 K cached tokens, cut into
+    KV-range chunks over ~70 CTA pairs and merged.  Every query row, one head per KV head, against the oracle."""
+    w = W.question_over_context()
+    assert w.num_q_tokens == 64 and w.max_kv_len > 32000
+    dw = DeviceWorkload(w, cache_fill=0x7FC1)
+    dw.step(); torch.cuda.synchronize()
+    assert _split_groups(dw) > 0
+    st = compare(dw, rows=np.arange(64), heads=np.array([0, 5, 10, 15, 16, 21, 26, 31]), expect_variant="prefill_sm100_tcgen05")
+    assert st["entries"] == 64 * 8
+
+
 def test_config4_full_sampled():
     w = W.config4()
     dw = DeviceWorkload(w)
