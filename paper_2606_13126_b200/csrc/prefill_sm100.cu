@@ -89,7 +89,9 @@ constexpr int kKStages = MINIPIC_KSTAGES, kVStages = MINIPIC_VSTAGES, kRing = 4;
 //    3 % by itself, 2.08 ms, with the old order);
 //  * Q rotation with the lane owning a TOKEN (row 8 rsub + k: for G = 8 one exact restart per item, no angle-addition steps, -sin
 //    formed once; ~30 % fewer instructions in the loop that takes ~3.8 K of the ~8.4 K cycles of an item boundary): span-only
-//    input 2.311 -> 2.271 ms, but dense causal 1.033 -> 1.058 ms and config 5 2.012 -> 2.027 ms;
+//    input 2.311 -> 2.271 ms, but dense causal 1.033 -> 1.058 ms and config 5 2.012 -> 2.027 ms; the Q rotation as a
+//    __noinline__ function (to keep it from disturbing the tile loop's register allocation): dense 1.074 ms, with the
+//    token-per-lane mapping inside 1.113 ms - the call's ABI costs the tile loop more than the inlined code did;
 //  * (again, on this kernel, after ncu showed the exp phase waiting at the MUFU cadence) every 4th / 3rd / 2nd exp2 pair as a
 //    packed-f32x2 cubic on the FMA pipe: dense causal 1.032 -> 1.148 / 1.149 / 1.294 ms, config 5 2.013 -> 2.106 / 2.137 / 2.198 ms;
 //    only with K pre-rotated (idle rotation warps) does it gain (0.953 -> 0.939 ms): the FMA pipe is what the rotation needs;
