@@ -635,9 +635,13 @@ __global__ void __launch_bounds__(256) split_merge_kernel(const PlanHeader* hdr,
   asm volatile("griddepcontrol.wait;" ::: "memory");   // launched as a programmatic dependent of the attention grid
   const int n_groups = *(volatile const int*)&hdr->n_groups;
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
-  for (int g = 0; g < n_groups; ++g) {   // every block takes a slice of every group's rows (there are few groups)
+  if (n_groups == 0) return;
+  // blocks are dealt out to the groups: bpg blocks share the rows of one group, all groups run side by side (one group: the
+  // whole grid works on it; more groups than blocks: a block walks through several)
+  const int bpg = max(1, (int)gridDim.x / n_groups), gstep = max(1, (int)gridDim.x / bpg), part = blockIdx.x % bpg;
+  for (int g = blockIdx.x / bpg; g < n_groups; g += gstep) {
     const SplitGroup sg = groups[g];
-    for (int rowi = blockIdx.x * 8 + wib; rowi < sg.ntok * hq; rowi += gridDim.x * 8) {
+    for (int rowi = part * 8 + wib; rowi < sg.ntok * hq; rowi += bpg * 8) {
       const int j = rowi / hq, h = rowi % hq;
       // all loads first (nsplit <= kSplitMax, fixed trip count): two memory round trips per row instead of one per chunk
       float ls[kSplitMax];
