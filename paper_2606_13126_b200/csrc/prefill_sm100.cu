@@ -356,12 +356,8 @@ __host__ __device__ constexpr uint32_t instr_desc(bool b_mn) {
 }
 
 // ------------------------------------------------------------------------------------------------ a2: plan
-__device__ __forceinline__ bool tile_starts(const PrefillArgs& a, int t, int r, int tok) {
-  if (t == __ldg(a.cu_q_lens + r)) return true;
-  const int i1 = __ldg(a.q_seq_idx + t), i0 = __ldg(a.q_seq_idx + t - 1);
-  const int l1 = __ldg(a.q_vis_lo + t), l0 = __ldg(a.q_vis_lo + t - 1);
-  return i1 != i0 + 1 || l1 != l0 || ((i1 - max(l1, 0)) % tok) == 0;
-}
+// A token starts a new item if it is the first of its request, if it does not continue the previous token (sequence index + 1,
+// same vis_lo), or every `tok` tokens counted from its span start (plan_kernel evaluates this rule branch-free).
 
 // ONE launch (a2).  Every block marks its 256 query tokens: the start flags of those tokens and of the next `tok` ones go
 // into a shared bitmask, so a starting token finds the length of its item with a find-first-set instead of a sequential
@@ -370,6 +366,7 @@ __device__ __forceinline__ bool tile_starts(const PrefillArgs& a, int t, int r, 
 // (SplitGroup; only when the host allows it), and sorts all descriptors by DESCENDING cost - a counting sort in shared
 // memory, longest item first - for the persistent kernel's atomic work counter to walk.
 constexpr int kPlanThreads = 256, kPlanMaxTok = 512;   // tok = 4 * 128 / G <= 512
+constexpr int kPlanSingleThreads = 1024, kPlanSingleMaxTok = 4096;   // one-block plan for small inputs (see plan_kernel)
 constexpr int kPlanCache = 2560;                         // descriptors the last block keeps in shared memory when it may split
 constexpr int kSplitMinSteps = 4, kSplitMax = 16;      // a chunk runs at least 4 tile steps; at most 16 chunks per item
 __device__ __forceinline__ int tile_cost(const TileDesc& td) { return td.pad ? (td.n_kv + 1) >> 1 : td.n_kv; }   // tile steps
@@ -400,20 +397,40 @@ __device__ __forceinline__ TileDesc load_desc(const TileDesc* p) {   // written 
   for (int e = 0; e < (int)(sizeof(TileDesc) / sizeof(int)); ++e) dst[e] = __ldcg(src + e);
   return td;
 }
-__global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanArgs pa) {
-  constexpr int kWords = (kPlanThreads + kPlanMaxTok) / 32;
+// kSingle: ONE block of kT = 1024 threads does everything for a small input (the host decides: at most kPlanSingleMaxTok
+// query tokens).  No ticket, no header memset before the launch, item count and (cost, tiles, tokens) of every item stay in shared
+// memory: about half the dependent L2 round trips of the multi-block version, which are what a plan of a few hundred items costs.
+#ifdef MINIPIC_PLAN_TIMES
+__device__ long long g_plan_t[16];
+#define PLAN_T(i) do { if (threadIdx.x == 0) g_plan_t[i] = clock64(); } while (0)
+#else
+#define PLAN_T(i) do { } while (0)
+#endif
+template <int kT, bool kSingle>
+__global__ void __launch_bounds__(kT) plan_kernel(PrefillArgs a, PlanArgs pa) {
+  constexpr int kRounds = ((kSingle ? kPlanSingleMaxTok : kT) + kPlanMaxTok + kT - 1) / kT;   // rounds of kT tokens that cover the block + the lookahead
+  constexpr int kWords = kRounds * (kT / 32);
   __shared__ unsigned sflag[kWords];
-  __shared__ int s_last, s_groups, s_slots;
-  __shared__ int wsum[kPlanThreads / 32];
-  __shared__ int red[3], cand_items[8], cand_max[8], s_nlong, long_idx[kPlanThreads];
+  __shared__ int s_last, s_groups, s_slots, s_nraw;
+  __shared__ int wsum[kT / 32];
+  __shared__ int red[3], wred[3][32], cand_items[8], cand_max[8], s_nlong, long_idx[kT];
   __shared__ unsigned short s_cost[kPlanCache], s_nkv[kPlanCache], s_ntk[kPlanCache];
   __shared__ int shist[kMaxBins];
   const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-  const int b0 = blockIdx.x * kPlanThreads;
   const int tok = pa.tok;
   PlanHeader* hdr = pa.hdr;
+  PLAN_T(0);
   asm volatile("griddepcontrol.launch_dependents;" ::: "memory");   // the attention grid may start its prologue (see its scheduler)
   if (blockIdx.x == 0 && tid == 0) hdr->magic = kPlanMagic;
+  if (kSingle && tid == 0) {   // no memset ran before this launch: the counters the other kernels read start here
+    hdr->next_item = 0; hdr->err = 0; hdr->n_groups = 0; hdr->part_used = 0;
+    s_nraw = 0;
+  }
+  if (kSingle) __syncthreads();
+  int* const n_raw_ctr = kSingle ? &s_nraw : &hdr->n_raw;
+  // the block's tokens: kT of them, or (kSingle) all - then a thread marks and makes items for several tokens, kT apart
+  const int span = kSingle ? ((a.num_q_tokens + kT - 1) / kT) * kT : kT;
+  const int b0 = kSingle ? 0 : (int)blockIdx.x * kT;
   auto request_of = [&](int t) {
     int lo_r = 0, hi_r = a.num_reqs;
     while (hi_r - lo_r > 1) {
@@ -422,73 +439,119 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanA
     }
     return lo_r;
   };
-  int my_r = 0;
-  for (int c = 0; c * kPlanThreads < kPlanThreads + tok; ++c) {
-    const int t = b0 + c * kPlanThreads + tid;
-    bool f = true;                       // tokens past the end count as starts (sentinel)
-    if (t < a.num_q_tokens) {
+  // straight-line on purpose: every round's loads are issued (clamped indices, no branches) before any of them is used, so that
+  // the rounds cost one memory round trip together instead of two each
+  bool fl[kRounds];
+  {
+    int tc[kRounds], rr[kRounds], tq[kRounds], i1[kRounds], i0[kRounds], l1[kRounds], l0[kRounds];
+    const int t_last = max(a.num_q_tokens - 1, 0);
+#pragma unroll
+    for (int c = 0; c < kRounds; ++c) { tc[c] = min(b0 + c * kT + tid, t_last); rr[c] = request_of(tc[c]); }
+#pragma unroll
+    for (int c = 0; c < kRounds; ++c) {
+      const int tm = max(tc[c] - 1, 0);
+      tq[c] = __ldg(a.cu_q_lens + rr[c]);
+      i1[c] = __ldg(a.q_seq_idx + tc[c]); i0[c] = __ldg(a.q_seq_idx + tm);
+      l1[c] = __ldg(a.q_vis_lo + tc[c]); l0[c] = __ldg(a.q_vis_lo + tm);
+    }
+#pragma unroll
+    for (int c = 0; c < kRounds; ++c) {
+      const int t = b0 + c * kT + tid;
+      // the item-start rule (above); tokens past the end count as starts (sentinel)
+      fl[c] = t >= a.num_q_tokens || t == tq[c] || i1[c] != i0[c] + 1 || l1[c] != l0[c] || ((i1[c] - max(l1[c], 0)) % tok) == 0;
+    }
+  }
+#pragma unroll
+  for (int c = 0; c < kRounds; ++c) {
+    if (c * kT < span + tok) {
+      const unsigned m = __ballot_sync(0xffffffffu, fl[c]);
+      if (lane == 0) sflag[c * (kT / 32) + wid] = m;
+    }
+  }
+  __syncthreads();
+#pragma unroll
+  for (int c2 = 0; c2 < (kSingle ? kPlanSingleMaxTok / kT : 1); ++c2) {   // unrolled for the same reason
+    const int li = c2 * kT + tid, t = b0 + li;   // li: index within the block's tokens = bit index in sflag
+    if (c2 * kT < span && t < a.num_q_tokens && ((sflag[li >> 5] >> (li & 31)) & 1u)) {
+      int nxt = -1;                        // index of the next start after li
+      unsigned wbits = sflag[li >> 5] & ~((2u << (li & 31)) - 1u);
+      for (int wi = li >> 5; nxt < 0; ++wi) {
+        if (wbits) nxt = wi * 32 + __ffs(wbits) - 1;
+        else wbits = sflag[wi + 1];        // a start exists within `tok` tokens (item length rule / end sentinel)
+      }
+      const int n = min(nxt - li, tok);
       const int r = request_of(t);
-      if (c == 0) my_r = r;
-      f = tile_starts(a, t, r, tok);
+      TileDesc td;
+      td.t0 = t; td.ntok = n; td.r = r; td.idx0 = __ldg(a.q_seq_idx + t); td.lo = max(__ldg(a.q_vis_lo + t), 0);
+      td.kv_len = __ldg(a.kv_lens + r);
+      td.kv_off = __ldg(a.cu_kv_lens + r);
+      const int kv_lo = td.lo & ~(kBlock - 1);
+      td.kv_hi = min(td.idx0 + n, td.kv_len);
+      td.n_kv = td.kv_hi > kv_lo ? (td.kv_hi - kv_lo + BN - 1) / BN : 0;
+      td.pad = dual_flag(pa.dual_ok, n, tok, td.n_kv);
+      td.part = 0; td.rsv = 0;
+      const int slot = atomicAdd(n_raw_ctr, 1);
+      pa.tmp[slot] = td;
+      if (kSingle && slot < kPlanCache) {
+        s_cost[slot] = (unsigned short)min(tile_cost(td), 65535); s_nkv[slot] = (unsigned short)min(td.n_kv, 65535); s_ntk[slot] = (unsigned short)td.ntok;
+      }
     }
-    const unsigned m = __ballot_sync(0xffffffffu, f);
-    if (lane == 0) sflag[c * (kPlanThreads / 32) + wid] = m;
   }
-  __syncthreads();
-  const int t = b0 + tid;
-  if (t < a.num_q_tokens && ((sflag[tid >> 5] >> (tid & 31)) & 1u)) {
-    int nxt = -1;                        // local index of the next start after tid
-    unsigned wbits = sflag[tid >> 5] & ~((2u << (tid & 31)) - 1u);
-    for (int wi = tid >> 5; nxt < 0; ++wi) {
-      if (wbits) nxt = wi * 32 + __ffs(wbits) - 1;
-      else wbits = sflag[wi + 1];        // a start exists within `tok` tokens (item length rule / end sentinel)
-    }
-    const int n = min(nxt - tid, tok);
-    const int r = my_r;
-    TileDesc td;
-    td.t0 = t; td.ntok = n; td.r = r; td.idx0 = __ldg(a.q_seq_idx + t); td.lo = max(__ldg(a.q_vis_lo + t), 0);
-    td.kv_len = __ldg(a.kv_lens + r);
-    td.kv_off = __ldg(a.cu_kv_lens + r);
-    const int kv_lo = td.lo & ~(kBlock - 1);
-    td.kv_hi = min(td.idx0 + n, td.kv_len);
-    td.n_kv = td.kv_hi > kv_lo ? (td.kv_hi - kv_lo + BN - 1) / BN : 0;
-    td.pad = dual_flag(pa.dual_ok, n, tok, td.n_kv);
-    td.part = 0; td.rsv = 0;
-    pa.tmp[atomicAdd(&hdr->n_raw, 1)] = td;
-  }
+  if (kSingle) __syncthreads();
   // ---- last block: balance (KV-range splits) and counting sort of all descriptors, longest first
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) s_last = atomicAdd(&hdr->ticket, 1) == (int)gridDim.x - 1;
-  __syncthreads();
-  if (!s_last) return;
-  __threadfence();
-  const int n_raw = *(volatile int*)&hdr->n_raw;
+  if (!kSingle) {
+    __threadfence();
+    __syncthreads();
+    if (tid == 0) s_last = atomicAdd(&hdr->ticket, 1) == (int)gridDim.x - 1;
+    __syncthreads();
+    if (!s_last) return;
+    __threadfence();
+  }
+  const int n_raw = kSingle ? s_nraw : *(volatile int*)&hdr->n_raw;
+  PLAN_T(1);
   auto block_reduce = [&](int v0, int v1, int vmax) {   // red[0], red[1] = block-wide sums, red[2] = block-wide max (>= 0)
-    __syncthreads();
-    if (tid < 3) red[tid] = 0;
-    __syncthreads();
+    // two levels of shuffles through wred, no shared-memory atomics (32 warps on three addresses took ~3 us per call)
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
       v0 += __shfl_xor_sync(0xffffffffu, v0, o); v1 += __shfl_xor_sync(0xffffffffu, v1, o);
       vmax = max(vmax, __shfl_xor_sync(0xffffffffu, vmax, o));
     }
-    if (lane == 0) { atomicAdd(&red[0], v0); atomicAdd(&red[1], v1); atomicMax(&red[2], vmax); }
+    __syncthreads();   // the previous call's red[] has been read by everyone
+    if (lane == 0) { wred[0][wid] = v0; wred[1][wid] = v1; wred[2][wid] = vmax; }
+    __syncthreads();
+    if (wid == 0) {
+      int a0 = lane < kT / 32 ? wred[0][lane] : 0, a1 = lane < kT / 32 ? wred[1][lane] : 0, am = lane < kT / 32 ? wred[2][lane] : 0;
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) {
+        a0 += __shfl_xor_sync(0xffffffffu, a0, o); a1 += __shfl_xor_sync(0xffffffffu, a1, o);
+        am = max(am, __shfl_xor_sync(0xffffffffu, am, o));
+      }
+      if (lane == 0) { red[0] = a0; red[1] = a1; red[2] = am; }
+    }
     __syncthreads();
   };
   int tsplit = 0x3fffffff;
+  PLAN_T(2);
   constexpr int kCand = 8;   // candidate chunk lengths
   if (pa.split_pairs > 0 && n_raw <= kPlanCache) {   // kPlanCache descriptors: more than any small grid has
     int steps = 0, cmax_all = 0;
-    for (int i = tid; i < n_raw; i += kPlanThreads) {
-      const TileDesc td = load_desc(pa.tmp + i);
-      const int c = tile_cost(td);
-      s_cost[i] = (unsigned short)min(c, 65535); s_nkv[i] = (unsigned short)min(td.n_kv, 65535); s_ntk[i] = (unsigned short)td.ntok;
+    for (int i = tid; i < n_raw; i += kT) {
+      int c;
+      if (kSingle) c = s_cost[i];   // filled when the item was made
+      else {
+        const TileDesc td = load_desc(pa.tmp + i);
+        c = tile_cost(td);
+        s_cost[i] = (unsigned short)min(c, 65535); s_nkv[i] = (unsigned short)min(td.n_kv, 65535); s_ntk[i] = (unsigned short)td.ntok;
+      }
       steps += c; cmax_all = max(cmax_all, c);
     }
+    PLAN_T(3);
     block_reduce(steps, 0, cmax_all);
-    const long long all_steps = (long long)red[0] * pa.hkv;
-    const int per_pair = max(kSplitMinSteps, (int)((all_steps + pa.split_pairs - 1) / pa.split_pairs));
+    PLAN_T(4);
+    // float arithmetic on purpose: every thread evaluates this, and 64-bit integer divisions cost ~500 cycles each (they were
+    // 4 us of a 13 us plan); it is a heuristic, and every thread gets the same bits
+    const float all_steps = (float)red[0] * (float)pa.hkv;
+    const int per_pair = max(kSplitMinSteps, (int)ceilf(all_steps / (float)pa.split_pairs));
     const int cstep = max(1, per_pair / 8);
     if (2 * red[2] > 3 * per_pair && red[2] < 32767) {   // at least one item is long enough to be cut (and n_kv <= 2 cost fits 16 bits)
       __syncthreads();
@@ -496,19 +559,21 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanA
       if (tid == 0) { s_nlong = 0; s_groups = 0; s_slots = 0; }
       __syncthreads();
       int short_max = 0;
-      for (int i = tid; i < n_raw; i += kPlanThreads) {
+      for (int i = tid; i < n_raw; i += kT) {
         const int c = s_cost[i];
-        if (2 * c > 3 * per_pair) { const int j = atomicAdd(&s_nlong, 1); if (j < kPlanThreads) long_idx[j] = i; }
+        if (2 * c > 3 * per_pair) { const int j = atomicAdd(&s_nlong, 1); if (j < kT) long_idx[j] = i; }
         else short_max = max(short_max, c);
       }
+      PLAN_T(5);
       block_reduce(0, 0, short_max);
+      PLAN_T(6);
       short_max = red[2];
       const int n_long = s_nlong;
-      if (n_long <= kPlanThreads) {
+      if (n_long <= kT) {
         // a few candidate chunk lengths: keep the one with the shortest estimated makespan - rounds of items x mean item cost,
         // but at least the longest item - so that e.g. 8 long items become 72 chunks on 74 pairs rather than 80.  One task per
         // (long item, candidate); the short items count 1 each whatever the candidate.
-        for (int task = tid; task < n_long * kCand; task += kPlanThreads) {
+        for (int task = tid; task < n_long * kCand; task += kT) {
           const int k = task % kCand, i = long_idx[task / kCand];
           int ct;
           const int ns = split_count(s_cost[i], s_nkv[i], per_pair + k * cstep, &ct);
@@ -516,12 +581,19 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanA
           atomicMax(&cand_max[k], dual_flag(pa.dual_ok, s_ntk[i], tok, ct) ? (ct + 1) >> 1 : ct);
         }
         __syncthreads();
-        long long best = 0x7fffffffffffffffLL;
-        for (int k = 0; k < kCand; ++k) {
-          const long long n_it = (long long)cand_items[k] * pa.hkv, rounds = (n_it + pa.split_pairs - 1) / pa.split_pairs;
-          // + 1024: the fixed cost of an item (Q load + rotation, pipeline fill, epilogue) is about one tile step
-          const long long est = max((long long)max(cand_max[k], short_max) * 1024, rounds * (all_steps * 1024 / n_it)) + rounds * 1024;
-          if (est < best) { best = est; tsplit = per_pair + k * cstep; }
+        PLAN_T(7);
+        {   // candidate k is evaluated by lane k of every warp (the serial loop with its divisions took ~5 K cycles)
+          float est = 3.0e38f;
+          if (lane < kCand) {
+            const int n_it = cand_items[lane] * pa.hkv, rounds = (n_it + pa.split_pairs - 1) / pa.split_pairs;   // <= 2560 x 16 x hkv items
+            // + rounds: the fixed cost of an item (Q load + rotation, pipeline fill, epilogue) is about one tile step
+            est = fmaxf((float)max(cand_max[lane], short_max), (float)rounds * (all_steps / (float)n_it)) + (float)rounds;
+          }
+          float mn = est;
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) mn = fminf(mn, __shfl_xor_sync(0xffffffffu, mn, o));
+          const unsigned eq = __ballot_sync(0xffffffffu, lane < kCand && est == mn);
+          tsplit = per_pair + (__ffs(eq) - 1) * cstep;   // the first (shortest chunk) of equally good candidates
         }
         int slots = 0, extra = 0;
         if (tid < n_long) {
@@ -536,13 +608,14 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanA
     }
     __syncthreads();
   }
-  for (int i = tid; i < kMaxBins; i += kPlanThreads) shist[i] = 0;
+  PLAN_T(8);
+  for (int i = tid; i < kMaxBins; i += kT) shist[i] = 0;
   if (tid == 0) { s_groups = 0; s_slots = 0; }
   __syncthreads();
   // pass 1: histogram of the (chunk) costs - from the shared-memory copy when pass 0 made one (only then can items be cut)
   const bool cached = pa.split_pairs > 0 && n_raw <= kPlanCache;
   if (cached) {
-    for (int i = tid; i < n_raw; i += kPlanThreads) {
+    for (int i = tid; i < n_raw; i += kT) {
       const int cost = s_cost[i], n_kv = s_nkv[i], ntok = s_ntk[i];
       int ct;
       const int ns = split_count(cost, n_kv, tsplit, &ct);
@@ -553,22 +626,23 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanA
       }
     }
   } else {   // large grids (thousands of items, nothing is cut): four descriptors in flight per thread, two words of each
-    for (int i0 = tid; i0 < n_raw; i0 += 4 * kPlanThreads) {
+    for (int i0 = tid; i0 < n_raw; i0 += 4 * kT) {
       int nk[4], pd[4];
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
-        const int i = min(i0 + u * kPlanThreads, n_raw - 1);
+        const int i = min(i0 + u * kT, n_raw - 1);
         const int* src = reinterpret_cast<const int*>(pa.tmp + i);
         nk[u] = __ldcg(src + 5); pd[u] = __ldcg(src + 9);
       }
 #pragma unroll
       for (int u = 0; u < 4; ++u)
-        if (i0 + u * kPlanThreads < n_raw) atomicAdd(&shist[min(pd[u] ? (nk[u] + 1) >> 1 : nk[u], kMaxBins - 1)], 1);
+        if (i0 + u * kT < n_raw) atomicAdd(&shist[min(pd[u] ? (nk[u] + 1) >> 1 : nk[u], kMaxBins - 1)], 1);
     }
   }
   __syncthreads();
+  PLAN_T(9);
   // exclusive prefix over the bins in DESCENDING cost order: rank = kMaxBins - 1 - bin
-  constexpr int PER = kMaxBins / kPlanThreads;   // 16 ranks per thread
+  constexpr int PER = kMaxBins / kT;   // 16 ranks per thread
   int v[PER], tot = 0;
 #pragma unroll
   for (int e = 0; e < PER; ++e) { v[e] = shist[kMaxBins - 1 - (PER * tid + e)]; tot += v[e]; }
@@ -584,20 +658,21 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanA
   for (int w2 = 0; w2 < wid; ++w2) base += wsum[w2];
 #pragma unroll
   for (int e = 0; e < PER; ++e) { shist[kMaxBins - 1 - (PER * tid + e)] = base; base += v[e]; }
-  if (tid == kPlanThreads - 1) hdr->n_tiles = base;   // total number of descriptors after the splits
+  if (tid == kT - 1) hdr->n_tiles = base;   // total number of descriptors after the splits
   __syncthreads();
+  PLAN_T(10);
   // pass 2: scatter
   if (!cached) {   // plain scatter, four 48-byte descriptors in flight per thread
-    for (int i0 = tid; i0 < n_raw; i0 += 4 * kPlanThreads) {
+    for (int i0 = tid; i0 < n_raw; i0 += 4 * kT) {
       uint4 v[4][3];
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
-        const uint4* src = reinterpret_cast<const uint4*>(pa.tmp + min(i0 + u * kPlanThreads, n_raw - 1));
+        const uint4* src = reinterpret_cast<const uint4*>(pa.tmp + min(i0 + u * kT, n_raw - 1));
         v[u][0] = __ldcg(src); v[u][1] = __ldcg(src + 1); v[u][2] = __ldcg(src + 2);
       }
 #pragma unroll
       for (int u = 0; u < 4; ++u) {
-        if (i0 + u * kPlanThreads >= n_raw) continue;
+        if (i0 + u * kT >= n_raw) continue;
         const int n_kv = (int)v[u][1].y, cost = v[u][2].y ? (n_kv + 1) >> 1 : n_kv;   // ints 5 (n_kv) and 9 (pad)
         uint4* dst = reinterpret_cast<uint4*>(pa.sorted + atomicAdd(&shist[min(cost, kMaxBins - 1)], 1));
         dst[0] = v[u][0]; dst[1] = v[u][1]; dst[2] = v[u][2];
@@ -605,7 +680,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanA
     }
     return;   // no groups: the header's counters stay 0
   }
-  for (int i = tid; i < n_raw; i += kPlanThreads) {
+  for (int i = tid; i < n_raw; i += kT) {
     const TileDesc td = load_desc(pa.tmp + i);
     int ct;
     const int ns = split_count(tile_cost(td), td.n_kv, tsplit, &ct);
@@ -625,6 +700,7 @@ __global__ void __launch_bounds__(kPlanThreads) plan_kernel(PrefillArgs a, PlanA
   }
   __syncthreads();
   if (tid == 0) { hdr->n_groups = s_groups; hdr->part_used = s_slots; }
+  PLAN_T(11);
 }
 
 // a9 for split items: out[t, h] = sum_s w_s O_s / sum_s w_s with w_s = e^{lse_s - max}, lse = max + ln sum_s w_s.  One warp
@@ -1659,6 +1735,9 @@ bool make_cache_tensor_map(CUtensorMap* m, const void* cache, int num_blocks, in
              CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
              CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
+#ifdef MINIPIC_PLAN_TIMES
+extern "C" int minipic_debug_plan_times(long long* host) { cudaDeviceSynchronize(); return (int)cudaMemcpyFromSymbol(host, g_plan_t, sizeof(long long) * 16); }
+#endif
 #ifdef MINIPIC_TRACE
 extern "C" int minipic_debug_trace_copy(long long* host, int* counts) {
   cudaDeviceSynchronize();
@@ -1743,12 +1822,14 @@ bool launch_prefill_sm100(const Ctx& c, const PrefillArgs& a) {
     part_cap = (int)std::min<size_t>(kPartSlotsMax, (a.workspace_bytes - wl.part - 256) / slot_bytes(c));
   float* part_lse = (float*)(ws + wl.part);
   float* part_o = (float*)(ws + up256(wl.part + (size_t)part_cap * c.hq * sizeof(float)));
-  if (cudaMemsetAsync(hdr, 0, sizeof(PlanHeader), c.stream) != cudaSuccess) return false;
+  const bool plan_single = a.num_q_tokens <= kPlanSingleMaxTok;
+  if (!plan_single && cudaMemsetAsync(hdr, 0, sizeof(PlanHeader), c.stream) != cudaSuccess) return false;
   if (a.num_q_tokens > 0) {
     PlanArgs pa;
     pa.tok = tok2; pa.dual_ok = dual_ok; pa.split_pairs = part_cap > 0 ? pairs : 0; pa.hkv = c.hkv; pa.part_cap = part_cap;
     pa.sorted_cap = wl.sorted_cap; pa.hdr = hdr; pa.tmp = tmp; pa.sorted = sorted; pa.groups = groups;
-    plan_kernel<<<(a.num_q_tokens + kPlanThreads - 1) / kPlanThreads, kPlanThreads, 0, c.stream>>>(a, pa);
+    if (plan_single) plan_kernel<kPlanSingleThreads, true><<<1, kPlanSingleThreads, 0, c.stream>>>(a, pa);
+    else plan_kernel<kPlanThreads, false><<<(a.num_q_tokens + kPlanThreads - 1) / kPlanThreads, kPlanThreads, 0, c.stream>>>(a, pa);
     note_launch(1);
   }
   Params prm;
